@@ -1,0 +1,175 @@
+/*
+ * econojax.h -- C ABI of the B200-native batched EconoJax environment step.
+ *
+ * What it computes: the environment transition of EconoJax (arXiv 2410.22165; "P:n" =
+ * PAPER.md line n, "G#" = the readings listed in DESIGN.md section 3) for E independent
+ * economies of N population agents + 1 government: gather, craft,
+ * order placement with escrow, per-resource matching with price-time priority
+ * at the price of the order placed last, order expiry (P:162,
+ * P:275), bracketed tax collection and uniform redistribution at period ends (P:173,
+ * P:190-195), isoelastic utility rewards (Eq.1-2), government welfare reward
+ * (Eq.3-5), population observations and government statistics mean / std /
+ * median (Fig.1).
+ *
+ * Conventions
+ *  - Every function returns 0 (EJ_OK) or a negative EJ_ERR_* code; ej_last_error() gives a
+ *    static/handle-owned string naming the offending field.  No exceptions, no errno.
+ *  - "device pointer" = memory of the CUDA device that was current at ej_create; it is owned
+ *    by the caller, must be 16-byte aligned, is not retained after the call returns, but must
+ *    stay alive until the handle's stream has executed the call (calls are asynchronous on
+ *    the stream set by ej_set_stream, default stream 0).  "host pointer" = ordinary memory.
+ *  - There is no CPU fallback: every step of the path runs in the sm_100a kernels of
+ *    csrc/econojax.cu.  Without a CUDA device ej_create returns EJ_ERR_CUDA.
+ *  - An out-of-range or currently invalid action is NOT an API error: it is a no-op for that
+ *    agent (no labor) and bumps the env's `invalid` counter (G2).  Stepping a finished env
+ *    (t == episode_length) changes nothing, returns rewards 0 and done = 1 (G28).
+ */
+#ifndef ECONOJAX_H
+#define ECONOJAX_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define EJ_OK 0
+#define EJ_ERR_PARAM (-1)  /* bad argument or parameter field; ej_last_error names it */
+#define EJ_ERR_NOMEM (-2)  /* device or host allocation failed */
+#define EJ_ERR_CUDA (-3)   /* CUDA runtime error (text in ej_last_error) */
+#define EJ_ERR_STATE (-4)  /* call not valid in the handle's state (e.g. step before reset) */
+
+#define EJ_MAX_PRICES 16
+#define EJ_MAX_BRACKETS 16
+#define EJ_MAX_RATE_LEVELS 32
+#define EJ_MAX_RESOURCES 16
+#define EJ_MAX_AGENTS 1024
+#define EJ_MAX_ACTIVE_ORDERS 32
+
+#define EJ_CRAFT_SINGLE 0        /* the paper's single craft action (30/86 actions P:350) */
+#define EJ_CRAFT_PER_RESOURCE 1  /* "convert r" variant of BASELINE.json (G3) */
+#define EJ_SKILL_UNIFORM01 0
+#define EJ_SKILL_PARETO_CLIP 1   /* Pareto(alpha=4) clipped to [lo, hi] (G29) */
+
+/* Environment parameters (Table 2, unless noted).  POD, versioned by struct_size. */
+typedef struct ej_params {
+    uint32_t struct_size;                   /* = sizeof(ej_params) */
+    int32_t num_prices;                     /* P, 1..16 */
+    int32_t prices[EJ_MAX_PRICES];          /* strictly ascending positive integers (G4) */
+    int32_t episode_length;                 /* T, 1..65535 */
+    int32_t tax_period;                     /* >= 1 */
+    int32_t num_brackets;                   /* B = thresholds + 1, 1..16 */
+    float thresholds[EJ_MAX_BRACKETS];      /* B-1 used, strictly ascending, > 0 (G32) */
+    int32_t num_rate_levels;                /* L, 1..32 (21) */
+    float rate_table[EJ_MAX_RATE_LEVELS];   /* tax rate of government level k (G5) */
+    int32_t allow_noop;
+    float starting_coin;
+    int32_t order_expiry;                   /* steps an order stays live, >= 1 (G14) */
+    int32_t max_active_orders;              /* M per agent, 1..32, N*M < 65535 */
+    int32_t book_cap;                       /* K per (resource, side); 0 = unbounded (G15) */
+    int32_t craft_units;                    /* R_kappa */
+    int32_t craft_distinct;                 /* R_d <= R */
+    int32_t craft_mode;                     /* EJ_CRAFT_* (G3) */
+    float labor_craft, labor_gather, labor_trade;
+    float eta;                              /* != 1 */
+    float omega;
+    float craft_scale;                      /* "scaled by a constant" P:158 (G6) */
+    int32_t taxes_enabled;
+    int32_t skill_init;                     /* EJ_SKILL_* */
+    float skill_clip_lo, skill_clip_hi;
+    float obs_scale_coin, obs_scale_count, obs_scale_price, obs_scale_labor; /* G25 */
+    uint32_t env_id_base;                   /* global id of local env 0: every random draw is keyed by
+                                               the global env id, so results do not depend on E or on
+                                               how envs are sharded over GPUs (multi-GPU: DESIGN.md 7) */
+} ej_params;
+
+typedef struct ej_env ej_env;
+
+/* Sizes and offsets derived from (E, N, R, params).  All counts in elements unless "bytes". */
+typedef struct ej_layout_info {
+    int32_t E, N, R, P, B, L;
+    int32_t A;                  /* number of discrete actions R + (1|R) + 2RP + noop */
+    int32_t base_craft, base_buy, base_sell, noop_action; /* first index of each action group; noop = -1 if off */
+    int32_t D_pop;              /* 6 + 8R + B floats per agent */
+    int32_t D_gov;              /* 3(3+R) + B + 2 floats per env */
+    int32_t D_gov_pad;          /* D_gov rounded up to a multiple of 4 */
+    size_t gov_obs_offset;      /* floats: start of the government region in an obs buffer (multiple of 4) */
+    size_t obs_floats;          /* total floats of one obs buffer: gov_obs_offset + E*D_gov_pad */
+    size_t rew_floats;          /* E*(N+1) */
+    size_t state_words;         /* int32 words per env of the canonical dump (ej_get_state) */
+    size_t device_state_bytes;  /* library-owned device bytes per env */
+    size_t smem_bytes;          /* dynamic shared memory per CTA of the step kernel */
+    int32_t threads_per_env;    /* CTA size */
+} ej_layout_info;
+
+/* Optional inputs/outputs of ej_rollout; all device pointers, any may be NULL. */
+typedef struct ej_rollout_io {
+    uint32_t struct_size;             /* = sizeof(ej_rollout_io) */
+    int32_t ring_depth;               /* >= 1: step s of the call writes ring slot s % ring_depth */
+    const int32_t* actions_in;        /* [T][E][N]; NULL = draw with the Philox/CDF generator (G30) */
+    const int32_t* gov_actions_in;    /* [T][E][B] level indices; NULL = draw */
+    float* obs_ring;                  /* [ring_depth][obs_floats] */
+    float* rew_ring;                  /* [ring_depth][E][N+1] */
+    uint8_t* done_ring;               /* [ring_depth][E] */
+    int32_t* actions_ring;            /* [ring_depth][E][N] actions actually applied */
+    int32_t* gov_actions_ring;        /* [ring_depth][E][B] */
+} ej_rollout_io;
+
+/* Validate, allocate library-owned device state for E envs on the current CUDA device.
+ * Errors: EJ_ERR_PARAM (field named), EJ_ERR_NOMEM, EJ_ERR_CUDA.  *out is NULL on failure;
+ * a failed create leaves its message readable through ej_last_error(NULL). */
+int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out);
+int ej_destroy(ej_env* h);
+/* cudaStream_t (as void*) all later calls are enqueued on. */
+int ej_set_stream(ej_env* h, void* cuda_stream);
+int ej_layout(const ej_env* h, ej_layout_info* out);
+const char* ej_last_error(const ej_env* h);
+
+/* Full re-initialisation (G29, G30): coin = starting_coin, everything else 0, books
+ * empty, rates 0, t = 0, skills drawn from Philox(seed; global env, agent).  Same (params,
+ * seed) => bit-identical state. */
+int ej_reset(ej_env* h, uint64_t seed);
+
+/* Observation of the current state (e.g. right after reset) into obs_out (device, obs_floats). */
+int ej_observe(ej_env* h, float* obs_out);
+
+/* One step of all E envs (order of effects G1: actions -> match -> expire -> tax -> rewards ->
+ * observations -> t++).
+ *  actions      device [E][N] int32 action indices (layout ej_layout_info.base_*)
+ *  gov_actions  device [E][B] int32 rate-level indices; read every step, applied at period ends (G18)
+ *  obs_out      device, one buffer of obs_floats floats with two regions: population
+ *               [E][N][D_pop] dense, then government [E][D_gov_pad] at gov_obs_offset; or NULL
+ *  rew_out      device [E][N+1] float, last = government; or NULL
+ *  done_out     device [E] uint8; or NULL */
+int ej_step(ej_env* h, const int32_t* actions, const int32_t* gov_actions, float* obs_out, float* rew_out,
+            uint8_t* done_out);
+
+/* Same step with HOST buffers (pinned or pageable): copies actions host->device, steps, copies
+ * observations / rewards / done device->host, and synchronises the stream before returning. */
+int ej_step_host(ej_env* h, const int32_t* actions, const int32_t* gov_actions, float* obs_out, float* rew_out,
+                 uint8_t* done_out);
+
+/* T steps in ONE persistent launch: each env's state stays in shared memory for the whole
+ * call.  Actions come from io->actions_in / gov_actions_in or, when NULL, from the Philox/CDF
+ * generator (ej_set_action_cdf; uniform over the A actions by default).  io may be NULL
+ * (no outputs).  No auto-reset: envs that reach episode_length stay done (G28). */
+int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* io);
+
+/* Cumulative uint32 thresholds of the rollout's action generator: action = smallest a with
+ * x < cdf[a], x = Philox word 0; the last entry is read as 2^32.  cdf is a HOST pointer [A]. */
+int ej_set_action_cdf(ej_env* h, const uint32_t* cdf, int32_t A);
+
+/* Canonical, representation-free state dump of envs [env_begin, env_begin+env_count) into /
+ * from a HOST buffer of env_count*state_words int32 words (layout: DESIGN.md "Canonical state
+ * dump").  Both synchronise the stream.  Cold path: used by tests and checkpointing. */
+int ej_get_state(ej_env* h, int32_t env_begin, int32_t env_count, int32_t* words, size_t n_words);
+int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t* words, size_t n_words);
+
+/* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
+int64_t ej_launch_count(const ej_env* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

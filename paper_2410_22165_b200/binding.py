@@ -1,0 +1,302 @@
+"""Thin ctypes binding of ``include/econojax.h`` -- argument marshalling only.
+
+Every function below has the name and the arguments of the C entry point it calls; pointers
+are passed as integers (``tensor.data_ptr()`` for device memory owned by PyTorch,
+``ndarray.ctypes.data`` for host memory).  ``Env`` is a small convenience wrapper that owns
+the handle and allocates the PyTorch tensors.  There is no CPU fallback: if the CUDA library
+is missing, ``lib()`` raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MAX_PRICES, MAX_BRACKETS, MAX_RATE_LEVELS = 16, 16, 32
+EJ_OK, EJ_ERR_PARAM, EJ_ERR_NOMEM, EJ_ERR_CUDA, EJ_ERR_STATE = 0, -1, -2, -3, -4
+
+
+class EjParams(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32),
+        ("num_prices", C.c_int32), ("prices", C.c_int32 * MAX_PRICES),
+        ("episode_length", C.c_int32), ("tax_period", C.c_int32),
+        ("num_brackets", C.c_int32), ("thresholds", C.c_float * MAX_BRACKETS),
+        ("num_rate_levels", C.c_int32), ("rate_table", C.c_float * MAX_RATE_LEVELS),
+        ("allow_noop", C.c_int32), ("starting_coin", C.c_float), ("order_expiry", C.c_int32),
+        ("max_active_orders", C.c_int32), ("book_cap", C.c_int32),
+        ("craft_units", C.c_int32), ("craft_distinct", C.c_int32), ("craft_mode", C.c_int32),
+        ("labor_craft", C.c_float), ("labor_gather", C.c_float), ("labor_trade", C.c_float),
+        ("eta", C.c_float), ("omega", C.c_float), ("craft_scale", C.c_float),
+        ("taxes_enabled", C.c_int32), ("skill_init", C.c_int32),
+        ("skill_clip_lo", C.c_float), ("skill_clip_hi", C.c_float),
+        ("obs_scale_coin", C.c_float), ("obs_scale_count", C.c_float),
+        ("obs_scale_price", C.c_float), ("obs_scale_labor", C.c_float),
+        ("env_id_base", C.c_uint32),
+    ]
+
+
+class EjLayoutInfo(C.Structure):
+    _fields_ = [
+        ("E", C.c_int32), ("N", C.c_int32), ("R", C.c_int32), ("P", C.c_int32), ("B", C.c_int32), ("L", C.c_int32),
+        ("A", C.c_int32), ("base_craft", C.c_int32), ("base_buy", C.c_int32), ("base_sell", C.c_int32),
+        ("noop_action", C.c_int32), ("D_pop", C.c_int32), ("D_gov", C.c_int32), ("D_gov_pad", C.c_int32),
+        ("gov_obs_offset", C.c_size_t), ("obs_floats", C.c_size_t), ("rew_floats", C.c_size_t),
+        ("state_words", C.c_size_t), ("device_state_bytes", C.c_size_t), ("smem_bytes", C.c_size_t),
+        ("threads_per_env", C.c_int32),
+    ]
+
+
+class EjRolloutIO(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("ring_depth", C.c_int32),
+        ("actions_in", C.c_void_p), ("gov_actions_in", C.c_void_p),
+        ("obs_ring", C.c_void_p), ("rew_ring", C.c_void_p), ("done_ring", C.c_void_p),
+        ("actions_ring", C.c_void_p), ("gov_actions_ring", C.c_void_p),
+    ]
+
+
+EXPORTS = ("ej_create", "ej_destroy", "ej_set_stream", "ej_layout", "ej_last_error", "ej_reset", "ej_observe",
+           "ej_step", "ej_step_host", "ej_rollout", "ej_set_action_cdf", "ej_get_state", "ej_set_state",
+           "ej_launch_count")
+
+_lib = None
+
+
+def lib():
+    """Load libeconojax.so (building it in-tree if the source is newer).  Raises if unavailable."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path) or os.path.getmtime(path) < os.path.getmtime(_build.SRC):
+            path = _build.build_lib()
+        L = C.CDLL(path)
+        vp = C.c_void_p
+        L.ej_create.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(EjParams), C.POINTER(vp)]
+        L.ej_destroy.argtypes = [vp]
+        L.ej_set_stream.argtypes = [vp, vp]
+        L.ej_layout.argtypes = [vp, C.POINTER(EjLayoutInfo)]
+        L.ej_last_error.argtypes = [vp]; L.ej_last_error.restype = C.c_char_p
+        L.ej_reset.argtypes = [vp, C.c_uint64]
+        L.ej_observe.argtypes = [vp, vp]
+        L.ej_step.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.ej_step_host.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.ej_rollout.argtypes = [vp, C.c_int32, C.POINTER(EjRolloutIO)]
+        L.ej_set_action_cdf.argtypes = [vp, vp, C.c_int32]
+        L.ej_get_state.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_size_t]
+        L.ej_set_state.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_size_t]
+        L.ej_launch_count.argtypes = [vp]; L.ej_launch_count.restype = C.c_int64
+        for name in EXPORTS:
+            if name not in ("ej_last_error", "ej_launch_count"):
+                getattr(L, name).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+class EjError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("econojax error %d: %s" % (code, msg))
+        self.code = code
+
+
+def make_params(d: dict) -> EjParams:
+    """Fill ej_params from a plain dict (see inputs.default_params)."""
+    p = EjParams()
+    p.struct_size = C.sizeof(EjParams)
+    prices = list(d["prices"])
+    p.num_prices = len(prices)
+    for i, v in enumerate(prices[:MAX_PRICES]):
+        p.prices[i] = int(v)
+    thr = list(d["thresholds"])
+    p.num_brackets = len(thr) + 1
+    for i, v in enumerate(thr[:MAX_BRACKETS]):
+        p.thresholds[i] = float(v)
+    table = list(d["rate_table"])
+    p.num_rate_levels = len(table)
+    for i, v in enumerate(table[:MAX_RATE_LEVELS]):
+        p.rate_table[i] = float(v)
+    for name in ("episode_length", "tax_period", "allow_noop", "order_expiry", "max_active_orders", "book_cap",
+                 "craft_units", "craft_distinct", "craft_mode", "taxes_enabled", "skill_init", "env_id_base"):
+        setattr(p, name, int(d[name]))
+    for name in ("starting_coin", "labor_craft", "labor_gather", "labor_trade", "eta", "omega", "craft_scale",
+                 "skill_clip_lo", "skill_clip_hi", "obs_scale_coin", "obs_scale_count", "obs_scale_price",
+                 "obs_scale_labor"):
+        setattr(p, name, float(d[name]))
+    return p
+
+
+def _check(h, rc):
+    if rc != EJ_OK:
+        raise EjError(rc, (lib().ej_last_error(h) or b"").decode())
+
+
+# ---- same-name wrappers: marshalling only ----
+def ej_create(E, N, R, params: EjParams):
+    h = C.c_void_p()
+    rc = lib().ej_create(E, N, R, C.byref(params), C.byref(h))
+    _check(None, rc)
+    return h
+
+
+def ej_destroy(h):
+    _check(h, lib().ej_destroy(h))
+
+
+def ej_set_stream(h, cuda_stream: int):
+    _check(h, lib().ej_set_stream(h, cuda_stream))
+
+
+def ej_layout(h) -> EjLayoutInfo:
+    info = EjLayoutInfo()
+    _check(h, lib().ej_layout(h, C.byref(info)))
+    return info
+
+
+def ej_last_error(h) -> str:
+    return (lib().ej_last_error(h) or b"").decode()
+
+
+def ej_reset(h, seed: int):
+    _check(h, lib().ej_reset(h, C.c_uint64(seed)))
+
+
+def ej_observe(h, obs_out: int):
+    _check(h, lib().ej_observe(h, obs_out))
+
+
+def ej_step(h, actions: int, gov_actions: int, obs_out: int | None, rew_out: int | None, done_out: int | None):
+    _check(h, lib().ej_step(h, actions, gov_actions, obs_out, rew_out, done_out))
+
+
+def ej_step_host(h, actions: int, gov_actions: int, obs_out: int | None, rew_out: int | None, done_out: int | None):
+    _check(h, lib().ej_step_host(h, actions, gov_actions, obs_out, rew_out, done_out))
+
+
+def ej_rollout(h, T: int, io: EjRolloutIO | None):
+    _check(h, lib().ej_rollout(h, T, C.byref(io) if io is not None else None))
+
+
+def ej_set_action_cdf(h, cdf: int, A: int):
+    _check(h, lib().ej_set_action_cdf(h, cdf, A))
+
+
+def ej_get_state(h, env_begin: int, env_count: int, words: int, n_words: int):
+    _check(h, lib().ej_get_state(h, env_begin, env_count, words, n_words))
+
+
+def ej_set_state(h, env_begin: int, env_count: int, words: int, n_words: int):
+    _check(h, lib().ej_set_state(h, env_begin, env_count, words, n_words))
+
+
+def ej_launch_count(h) -> int:
+    return int(lib().ej_launch_count(h))
+
+
+def _dp(t):
+    return None if t is None else t.data_ptr()
+
+
+class Env:
+    """Owns one ej_env handle and the PyTorch tensors its calls read and write."""
+
+    def __init__(self, E: int, N: int, R: int, params: dict, device: str = "cuda:0"):
+        import torch
+
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.params = dict(params)
+        self.h = ej_create(E, N, R, make_params(params))
+        self.info = ej_layout(self.h)
+        for k, _ in EjLayoutInfo._fields_:
+            setattr(self, k, getattr(self.info, k))
+        ej_set_stream(self.h, torch.cuda.current_stream(self.device).cuda_stream)
+
+    def close(self):
+        if getattr(self, "h", None):
+            ej_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def use_current_stream(self):
+        ej_set_stream(self.h, self.torch.cuda.current_stream(self.device).cuda_stream)
+
+    def reset(self, seed: int):
+        ej_reset(self.h, seed)
+
+    # -- tensor allocation helpers --
+    def new_obs(self, depth=None):
+        shape = (self.obs_floats,) if depth is None else (depth, self.obs_floats)
+        return self.torch.zeros(shape, dtype=self.torch.float32, device=self.device)
+
+    def new_rew(self, depth=None):
+        shape = (self.E, self.N + 1) if depth is None else (depth, self.E, self.N + 1)
+        return self.torch.zeros(shape, dtype=self.torch.float32, device=self.device)
+
+    def new_done(self, depth=None):
+        shape = (self.E,) if depth is None else (depth, self.E)
+        return self.torch.zeros(shape, dtype=self.torch.uint8, device=self.device)
+
+    def split_obs(self, obs):
+        """Views (pop [.., E, N, D_pop], gov [.., E, D_gov]) of an obs buffer or ring."""
+        lead = obs.shape[:-1]
+        pop = obs[..., : self.E * self.N * self.D_pop].reshape(*lead, self.E, self.N, self.D_pop)
+        gov = obs[..., self.gov_obs_offset:].reshape(*lead, self.E, self.D_gov_pad)[..., : self.D_gov]
+        return pop, gov
+
+    def observe(self, obs=None):
+        obs = self.new_obs() if obs is None else obs
+        ej_observe(self.h, obs.data_ptr())
+        return obs
+
+    def step(self, actions, gov_actions, obs=None, rew=None, done=None, want_obs=True):
+        t = self.torch
+        assert actions.dtype == t.int32 and actions.is_cuda and actions.is_contiguous() and actions.numel() == self.E * self.N
+        assert gov_actions.dtype == t.int32 and gov_actions.is_cuda and gov_actions.is_contiguous() and gov_actions.numel() == self.E * self.B
+        if obs is None and want_obs:
+            obs = self.new_obs()
+        rew = self.new_rew() if rew is None else rew
+        done = self.new_done() if done is None else done
+        ej_step(self.h, actions.data_ptr(), gov_actions.data_ptr(), _dp(obs), _dp(rew), _dp(done))
+        return obs, rew, done
+
+    def step_host(self, actions: np.ndarray, gov_actions: np.ndarray, obs: np.ndarray | None, rew: np.ndarray | None,
+                  done: np.ndarray | None):
+        ej_step_host(self.h, actions.ctypes.data, gov_actions.ctypes.data,
+                     None if obs is None else obs.ctypes.data, None if rew is None else rew.ctypes.data,
+                     None if done is None else done.ctypes.data)
+
+    def rollout(self, T, ring_depth=1, actions_in=None, gov_actions_in=None, obs_ring=None, rew_ring=None,
+                done_ring=None, actions_ring=None, gov_actions_ring=None):
+        io = EjRolloutIO()
+        io.struct_size = C.sizeof(EjRolloutIO)
+        io.ring_depth = ring_depth
+        io.actions_in, io.gov_actions_in = _dp(actions_in), _dp(gov_actions_in)
+        io.obs_ring, io.rew_ring, io.done_ring = _dp(obs_ring), _dp(rew_ring), _dp(done_ring)
+        io.actions_ring, io.gov_actions_ring = _dp(actions_ring), _dp(gov_actions_ring)
+        ej_rollout(self.h, T, io)
+
+    def set_action_cdf(self, cdf: np.ndarray):
+        cdf = np.ascontiguousarray(cdf, np.uint32)
+        ej_set_action_cdf(self.h, cdf.ctypes.data, int(cdf.shape[0]))
+
+    def get_state(self, env_begin=0, env_count=None) -> np.ndarray:
+        n = self.E - env_begin if env_count is None else env_count
+        w = np.zeros((n, self.state_words), np.int32)
+        ej_get_state(self.h, env_begin, n, w.ctypes.data, w.size)
+        return w
+
+    def set_state(self, words: np.ndarray, env_begin=0):
+        words = np.ascontiguousarray(words, np.int32)
+        ej_set_state(self.h, env_begin, words.shape[0], words.ctypes.data, words.size)
+
+    def launch_count(self) -> int:
+        return ej_launch_count(self.h)
