@@ -48,7 +48,7 @@ struct DevCfg {
     int E, N, R, P, B, L, M, Mp_log2, K, T, period, expiry;
     int craft_units, craft_distinct, craft_mode, allow_noop, taxes_enabled, skill_init;
     int A, base_craft, base_buy, base_sell, n_levels, n_groups, D_pop, D_gov, D_gov_pad;
-    int N4, Npad, n_metrics, n_warps, shrow_len;
+    int N4, Npad, n_metrics, n_warps, shrow_len, stage_obs;
     int prices[EJ_MAX_PRICES];
     float thresholds[EJ_MAX_BRACKETS];
     float rate_table[EJ_MAX_RATE_LEVELS];
@@ -60,7 +60,7 @@ struct DevCfg {
     int o_head, o_tail, o_cnt, o_pool, blob_bytes;
     // scratch section offsets (bytes from the shared-memory base; all after the blob)
     int o_key, o_cinfo, o_cslot, o_credit, o_sale, o_mb, o_ma, o_bucket, o_sorted;
-    int o_gcnt, o_goff, o_take, o_roff, o_resq, o_resoff, o_red, o_sortbuf, o_shrow, o_med, o_misc, o_cdf;
+    int o_gcnt, o_goff, o_take, o_roff, o_resq, o_resoff, o_red, o_redq, o_hist, o_hovf, o_stage, o_sortbuf, o_shrow, o_med, o_misc, o_cdf;
     int smem_bytes;
     unsigned long long gov_obs_offset, obs_floats;
 };
@@ -97,7 +97,9 @@ struct Sm {
     uint32_t* sorted;
     int *gcnt, *goff, *take, *roff, *resq, *resoff;
     double* red;
-    float *sortbuf, *shrow, *med;
+    float* redq;
+    int *hist, *hovf;
+    float *stage, *sortbuf, *shrow, *med;
     unsigned long long* misc;  // [0] tax pool (2^-20 coin), [1] as int: total trades of the step
     uint32_t* cdf;
 };
@@ -135,6 +137,10 @@ __device__ __forceinline__ Sm carve(const DevCfg& c, uint8_t* s) {
     m.resq = (int*)(s + c.o_resq);
     m.resoff = (int*)(s + c.o_resoff);
     m.red = (double*)(s + c.o_red);
+    m.redq = (float*)(s + c.o_redq);
+    m.hist = (int*)(s + c.o_hist);
+    m.hovf = (int*)(s + c.o_hovf);
+    m.stage = (float*)(s + c.o_stage);
     m.sortbuf = (float*)(s + c.o_sortbuf);
     m.shrow = (float*)(s + c.o_shrow);
     m.med = (float*)(s + c.o_med);
@@ -168,29 +174,43 @@ __device__ __forceinline__ double warp_sum(double v) {
     for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = __fadd_rn(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
 
-// Block-wide bitonic sort of one float per thread (ascending by thread index).  Strides below
-// 32 are warp shuffles, larger ones go through a double-buffered shared array.
-__device__ __forceinline__ float block_sort(float x, int tid, int Npad, float* buf) {
+// Block-wide bitonic sort network, NV values per thread sorted independently (ascending by
+// thread index), fully unrolled: strides below 32 are warp shuffles, larger ones go through a
+// double-buffered shared array (one barrier per such stage).
+template <int NPAD, int NV>
+__device__ __forceinline__ void block_sort(float (&x)[NV], int tid, float* buf) {
     int pb = 0;
-    for (int k = 2; k <= Npad; k <<= 1) {
+#pragma unroll
+    for (int k = 2; k <= NPAD; k <<= 1) {
+#pragma unroll
         for (int j = k >> 1; j > 0; j >>= 1) {
-            float y;
+            float y[NV];
             if (j >= 32) {
-                float* b = buf + pb * Npad;
-                b[tid] = x;
+                float* b = buf + pb * (NV * NPAD);
+#pragma unroll
+                for (int v = 0; v < NV; ++v) b[v * NPAD + tid] = x[v];
                 __syncthreads();
-                y = b[tid ^ j];
+#pragma unroll
+                for (int v = 0; v < NV; ++v) y[v] = b[v * NPAD + (tid ^ j)];
                 pb ^= 1;
             } else {
-                y = __shfl_xor_sync(0xffffffffu, x, j);
+#pragma unroll
+                for (int v = 0; v < NV; ++v) y[v] = __shfl_xor_sync(0xffffffffu, x[v], j);
             }
-            const bool up = (tid & k) == 0, lower = (tid & j) == 0;
-            x = (up == lower) ? fminf(x, y) : fmaxf(x, y);
+            const bool keep_min = ((tid & k) == 0) == ((tid & j) == 0);
+#pragma unroll
+            for (int v = 0; v < NV; ++v) x[v] = keep_min ? fminf(x[v], y[v]) : fmaxf(x[v], y[v]);
         }
     }
-    return x;
 }
+
+constexpr int HB = 128;  // histogram bins of the integer-metric medians (inventories)
 
 // Government statistics (mean, std, median of coin, labor, income, inv[r]; Fig.1 P:31, P:426,
 // G26), welfare (Eq.3-5, G22/G23), population rewards (Eq.1-2) and both
@@ -198,33 +218,50 @@ __device__ __forceinline__ float block_sort(float x, int tid, int Npad, float* b
 //   tq       clock shown by the timers
 //   mode     0 = step (rewards from pre-step values, update u_g_prev), 1 = finished env
 //            (rewards 0), 2 = observe only (no rewards, u_g_prev untouched)
+// Float metrics: sums in binary64 (warp shuffles), squared deviations in binary32 (a sum of
+// non-negative terms: relative error < 1e-6), medians and the gini numerator from one
+// three-value sorting network.  Integer metrics: exact integer sums (REDUX), medians from a
+// shared-memory histogram (values >= HB fall back to the sorting network).
+template <int NPAD>
 __device__ void stats_rewards_obs(const DevCfg& c, const Sm& m, int tid, int e, int tq, int mode, float coin_pre,
                                   float labor_pre, double cf_pre, float* obs, float* rew) {
-    const int N = c.N, R = c.R, nm = c.n_metrics, nw = c.n_warps;
+    constexpr int NW = NPAD / 32;
+    const int N = c.N, R = c.R, nm = c.n_metrics, N4 = c.N4;
     const bool act = tid < N;
     const int lane = tid & 31, warp = tid >> 5;
+    const double inv_n = 1.0 / (double)N;
+
+    float xf[3] = {0.f, 0.f, 0.f};
+    if (act) { xf[0] = m.coin[tid]; xf[1] = m.labor[tid]; xf[2] = m.income[tid]; }
 
     // ---- population reward: u(post) - u(pre), u = coin term - labor (Eq.1-2) ----
     if (mode == 0 && act) {
-        const float cpost = m.coin[tid];
         double cf_post = cf_pre;
-        if (__float_as_uint(cpost) != __float_as_uint(coin_pre)) {
-            cf_post = coin_utility(cpost, 1.0 - (double)c.eta);
+        if (__float_as_uint(xf[0]) != __float_as_uint(coin_pre)) {
+            cf_post = coin_utility(xf[0], 1.0 - (double)c.eta);
             m.cf[tid] = cf_post;
         }
-        const double u_post = cf_post - (double)m.labor[tid];
+        const double u_post = cf_post - (double)xf[1];
         const double u_pre = cf_pre - (double)labor_pre;
         if (rew) rew[(size_t)e * (N + 1) + tid] = (float)(u_post - u_pre);
     } else if (mode == 1 && act && rew) {
         rew[(size_t)e * (N + 1) + tid] = 0.0f;
     }
 
-    // ---- pass 1: sums ----
-    for (int k = 0; k < nm; ++k) {
-        float x = 0.0f;
-        if (act) x = k == 0 ? m.coin[tid] : k == 1 ? m.labor[tid] : k == 2 ? m.income[tid] : (float)m.inv[(k - 3) * c.N4 + tid];
-        const double s = warp_sum((double)x);
-        if (lane == 0) m.red[k * nw + warp] = s;
+    // ---- pass 1: sums (per-warp partials), histograms of the integer metrics ----
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double s = warp_sum((double)xf[k]);
+        if (lane == 0) m.red[k * NW + warp] = s;
+    }
+    for (int r = 0; r < R; ++r) {
+        const int v = act ? m.inv[r * N4 + tid] : 0;
+        const int s = __reduce_add_sync(0xffffffffu, v);
+        if (lane == 0) m.red[(3 + r) * NW + warp] = (double)s;
+        if (act) {
+            if (v < HB) atomicAdd(&m.hist[r * HB + v], 1);
+            else m.hovf[r] = 1;
+        }
     }
     // shared tail of the population rows: market statistics, rates, timers
     if (tid < R) {
@@ -244,47 +281,145 @@ __device__ void stats_rewards_obs(const DevCfg& c, const Sm& m, int tid, int e, 
         o[3] = __fmul_rn((float)na, c.s_count);
         o[4] = __fmul_rn((float)m.hdr->last_price[r], c.s_price);
     }
-    if (tid < c.B) m.shrow[5 * R + tid] = m.hdr->rates[tid];
-    if (tid == 0) {
+    if (tid >= 32 && tid < 32 + c.B) m.shrow[5 * R + tid - 32] = m.hdr->rates[tid - 32];
+    if (NPAD == 32 && tid < c.B) m.shrow[5 * R + tid] = m.hdr->rates[tid];
+    if (tid == NPAD - 1) {
         m.shrow[5 * R + c.B] = __fdiv_rn((float)(tq % c.period), (float)c.period);
         m.shrow[5 * R + c.B + 1] = __fdiv_rn((float)tq, (float)c.T);
     }
-    __syncthreads();
-
-    // ---- pass 2: squared deviations; sort; medians; gini numerator ----
-    for (int k = 0; k < nm; ++k) {
-        double s1 = 0.0;
-        for (int w = 0; w < nw; ++w) s1 += m.red[k * nw + w];
-        const double mean = s1 / (double)N;
-        float x = 0.0f;
-        if (act) x = k == 0 ? m.coin[tid] : k == 1 ? m.labor[tid] : k == 2 ? m.income[tid] : (float)m.inv[(k - 3) * c.N4 + tid];
-        double d = act ? (double)x - mean : 0.0;
-        const double s2 = warp_sum(d * d);
-        if (lane == 0) m.red[(nm + k) * nw + warp] = s2;
-        const float xs = block_sort(act ? x : INFINITY, tid, c.Npad, m.sortbuf);
-        if (tid == (N >> 1) - 1) m.med[2 * k] = xs;
-        if (tid == (N >> 1)) m.med[2 * k + 1] = xs;
-        if (k == 0) {  // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)   (G23)
-            const double g = act ? (double)(2 * tid - N + 1) * (double)xs : 0.0;
-            const double gs = warp_sum(g);
-            if (lane == 0) m.red[2 * nm * nw + warp] = gs;
+    // private part of the population rows, staged in shared memory
+    const bool staged = c.stage_obs && obs;
+    if (staged) {
+        if (act) {
+            float* o = m.stage + tid * c.D_pop;
+            int k = 0;
+            o[k++] = __fmul_rn(xf[0], c.s_coin);
+            for (int r = 0; r < R; ++r) o[k++] = __fmul_rn((float)m.inv[r * N4 + tid], c.s_count);
+            o[k++] = __fmul_rn((float)m.esc_coin[tid], c.s_coin);
+            for (int r = 0; r < R; ++r) o[k++] = __fmul_rn((float)m.esc_res[r * N4 + tid], c.s_count);
+            for (int r = 0; r < R; ++r) o[k++] = m.SG[r * N4 + tid];
+            o[k++] = m.SC[tid];
+            o[k++] = __fmul_rn(xf[1], c.s_labor);
         }
     }
     __syncthreads();
 
+    // ---- pass 2: means, squared deviations, sort, medians, gini numerator ----
+    // every warp redundantly reduces the per-warp partials: lane k owns metric k
+    double mean_l = 0.0;
+    if (lane < nm) {
+        double s = 0.0;
+#pragma unroll
+        for (int w = 0; w < NW; ++w) s += m.red[lane * NW + w];
+        mean_l = s * inv_n;
+    }
+#pragma unroll
+    for (int k = 0; k < 3; ++k) {
+        const double mean = __shfl_sync(0xffffffffu, mean_l, k);
+        const float d = act ? (float)((double)xf[k] - mean) : 0.0f;
+        const float q = warp_sum(__fmul_rn(d, d));
+        if (lane == 0) m.redq[k * NW + warp] = q;
+    }
+    for (int r = 0; r < R; ++r) {
+        const double mean = __shfl_sync(0xffffffffu, mean_l, 3 + r);
+        const float d = act ? (float)((double)m.inv[r * N4 + tid] - mean) : 0.0f;
+        const float q = warp_sum(__fmul_rn(d, d));
+        if (lane == 0) m.redq[(3 + r) * NW + warp] = q;
+    }
+    if (staged && act) {  // shared tail of this agent's row
+        float* o = m.stage + tid * c.D_pop + (3 * R + 4);
+        for (int k = 0; k < c.shrow_len; ++k) o[k] = m.shrow[k];
+    }
+    {
+        float xs[3] = {act ? xf[0] : INFINITY, act ? xf[1] : INFINITY, act ? xf[2] : INFINITY};
+        block_sort<NPAD, 3>(xs, tid, m.sortbuf);
+        if (tid == (N >> 1) - 1) { m.med[0] = xs[0]; m.med[2] = xs[1]; m.med[4] = xs[2]; }
+        if (tid == (N >> 1)) { m.med[1] = xs[0]; m.med[3] = xs[1]; m.med[5] = xs[2]; }
+        // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)   (G23)
+        const double g = act ? (double)(2 * tid - N + 1) * (double)xs[0] : 0.0;
+        const double gs = warp_sum(g);
+        if (lane == 0) m.red[nm * NW + warp] = gs;
+    }
+    for (int r = 0; r < R; ++r) {  // rare: an inventory >= HB, median from the sorting network
+        if (m.hovf[r]) {
+            float xs[1] = {act ? (float)m.inv[r * N4 + tid] : INFINITY};
+            block_sort<NPAD, 1>(xs, tid, m.sortbuf);
+            if (tid == (N >> 1) - 1) m.med[2 * (3 + r)] = xs[0];
+            if (tid == (N >> 1)) m.med[2 * (3 + r) + 1] = xs[0];
+        }
+    }
+    if (staged) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+
     // ---- finals ----
     float* gov = obs ? obs + c.gov_obs_offset + (size_t)e * c.D_gov_pad : nullptr;
-    if (tid < nm) {
-        const int k = tid;
-        double s1 = 0.0, s2 = 0.0;
-        for (int w = 0; w < nw; ++w) s1 += m.red[k * nw + w];
-        for (int w = 0; w < nw; ++w) s2 += m.red[(nm + k) * nw + w];
-        const double mean = s1 / (double)N;
-        const double sd = sqrt(s2 / (double)N);
-        float med;
-        if (N & 1) med = m.med[2 * k + 1];
-        else med = __fmul_rn(0.5f, __fadd_rn(m.med[2 * k], m.med[2 * k + 1]));
-        const float scale = (k == 0 || k == 2) ? c.s_coin : (k == 1 ? c.s_labor : c.s_count);
+    if (staged && tid == 0) {  // one bulk store of the env's contiguous [N][D_pop] block
+        float* dst = obs + (size_t)e * N * c.D_pop;
+        const uint32_t src = (uint32_t)__cvta_generic_to_shared(m.stage);
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(N * c.D_pop * 4) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    // integer medians from the histograms: warp w handles metrics w, w + NW, ...
+    for (int r = warp; r < R; r += NW) {
+        float lo_v, hi_v;
+        if (!m.hovf[r]) {
+            int4 h4 = ((int4*)(m.hist + r * HB))[lane];
+            ((int4*)(m.hist + r * HB))[lane] = make_int4(0, 0, 0, 0);
+            const int c0 = h4.x, c1 = c0 + h4.y, c2 = c1 + h4.z, c3 = c2 + h4.w;
+            int incl = c3;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += y;
+            }
+            const int excl = incl - c3;
+            int vals[2];
+#pragma unroll
+            for (int j = 0; j < 2; ++j) {  // value of 0-based rank q = smallest v with cum(v) > q
+                const int q = (N >> 1) - 1 + j;
+                const unsigned ball = __ballot_sync(0xffffffffu, incl > q);
+                const int src = __ffs(ball) - 1;
+                const int ex = __shfl_sync(0xffffffffu, excl, src < 0 ? 0 : src);
+                const int a0 = __shfl_sync(0xffffffffu, c0, src < 0 ? 0 : src), a1 = __shfl_sync(0xffffffffu, c1, src < 0 ? 0 : src),
+                          a2 = __shfl_sync(0xffffffffu, c2, src < 0 ? 0 : src);
+                const int rel = q - ex;
+                vals[j] = (src < 0 ? 0 : src) * 4 + (rel < a0 ? 0 : rel < a1 ? 1 : rel < a2 ? 2 : 3);
+            }
+            lo_v = (float)vals[0];
+            hi_v = (float)vals[1];
+        } else {
+            for (int b = lane; b < HB; b += 32) m.hist[r * HB + b] = 0;
+            lo_v = m.med[2 * (3 + r)];
+            hi_v = m.med[2 * (3 + r) + 1];
+            __syncwarp();
+            if (lane == 0) m.hovf[r] = 0;
+        }
+        if (lane == 0) {
+            const int k = 3 + r;
+            double s1 = 0.0;
+            float s2 = 0.0f;
+            for (int w = 0; w < NW; ++w) s1 += m.red[k * NW + w];
+            for (int w = 0; w < NW; ++w) s2 = __fadd_rn(s2, m.redq[k * NW + w]);
+            const double mean = s1 * inv_n;
+            const double sd = sqrt((double)s2 * inv_n);
+            const float med = (N & 1) ? hi_v : __fmul_rn(0.5f, __fadd_rn(lo_v, hi_v));
+            if (gov) {
+                gov[3 * k + 0] = (float)(mean * (double)c.s_count);
+                gov[3 * k + 1] = (float)(sd * (double)c.s_count);
+                gov[3 * k + 2] = __fmul_rn(med, c.s_count);
+            }
+        }
+    }
+    if (tid >= NPAD - 3) {  // float metrics: coin, labor, income
+        const int k = tid - (NPAD - 3);
+        double s1 = 0.0;
+        float s2 = 0.0f;
+        for (int w = 0; w < NW; ++w) s1 += m.red[k * NW + w];
+        for (int w = 0; w < NW; ++w) s2 = __fadd_rn(s2, m.redq[k * NW + w]);
+        const double mean = s1 * inv_n;
+        const double sd = sqrt((double)s2 * inv_n);
+        const float med = (N & 1) ? m.med[2 * k + 1] : __fmul_rn(0.5f, __fadd_rn(m.med[2 * k], m.med[2 * k + 1]));
+        const float scale = k == 1 ? c.s_labor : c.s_coin;
         if (gov) {
             gov[3 * k + 0] = (float)(mean * (double)scale);
             gov[3 * k + 1] = (float)(sd * (double)scale);
@@ -292,11 +427,11 @@ __device__ void stats_rewards_obs(const DevCfg& c, const Sm& m, int tid, int e, 
         }
     }
     if (gov)
-        for (int k = tid; k < c.B + 2; k += blockDim.x) gov[3 * nm + k] = m.shrow[5 * R + k];
+        for (int k = tid; k < c.B + 2; k += NPAD) gov[3 * nm + k] = m.shrow[5 * R + k];
     if (tid == 0 && mode != 2) {
         double prod = 0.0, gn = 0.0;
-        for (int w = 0; w < nw; ++w) prod += m.red[w];
-        for (int w = 0; w < nw; ++w) gn += m.red[2 * nm * nw + w];
+        for (int w = 0; w < NW; ++w) prod += m.red[w];
+        for (int w = 0; w < NW; ++w) gn += m.red[nm * NW + w];
         double gini = 0.0;
         if (N > 1 && prod != 0.0) gini = gn / ((double)N * prod);
         const double eq = (double)c.omega * (1.0 - gini) + (1.0 - (double)c.omega);
@@ -309,19 +444,19 @@ __device__ void stats_rewards_obs(const DevCfg& c, const Sm& m, int tid, int e, 
         }
     }
 
-    // ---- population observation rows, coalesced over the env's contiguous [N][D_pop] block ----
-    if (obs) {
+    // ---- population rows when they cannot go out as one bulk store: coalesced loop ----
+    if (obs && !staged) {
         const int D = c.D_pop, priv = 3 * R + 4, total = N * D;
         float* dst = obs + (size_t)e * total;
-        for (int idx = tid; idx < total; idx += blockDim.x) {
+        for (int idx = tid; idx < total; idx += NPAD) {
             const int i = idx / D, k = idx - i * D;
             float v;
             if (k >= priv) v = m.shrow[k - priv];
             else if (k == 0) v = __fmul_rn(m.coin[i], c.s_coin);
-            else if (k <= R) v = __fmul_rn((float)m.inv[(k - 1) * c.N4 + i], c.s_count);
+            else if (k <= R) v = __fmul_rn((float)m.inv[(k - 1) * N4 + i], c.s_count);
             else if (k == R + 1) v = __fmul_rn((float)m.esc_coin[i], c.s_coin);
-            else if (k <= 2 * R + 1) v = __fmul_rn((float)m.esc_res[(k - R - 2) * c.N4 + i], c.s_count);
-            else if (k <= 3 * R + 1) v = m.SG[(k - 2 * R - 2) * c.N4 + i];
+            else if (k <= 2 * R + 1) v = __fmul_rn((float)m.esc_res[(k - R - 2) * N4 + i], c.s_count);
+            else if (k <= 3 * R + 1) v = m.SG[(k - 2 * R - 2) * N4 + i];
             else if (k == 3 * R + 2) v = m.SC[i];
             else v = __fmul_rn(m.labor[i], c.s_labor);
             dst[idx] = v;
@@ -331,15 +466,19 @@ __device__ void stats_rewards_obs(const DevCfg& c, const Sm& m, int tid, int e, 
 
 // One environment step on the state in shared memory (G1: actions -> match -> expire -> tax ->
 // rewards -> observations -> t++).
+template <int NPAD>
 __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const int32_t* actions, const int32_t* gov_actions,
                          float* obs, float* rew, uint8_t* done, int32_t* actions_out, int32_t* gov_out) {
     const int N = c.N, R = c.R, P = c.P, N4 = c.N4;
     const bool act = tid < N;
     const int t = m.hdr->t;
     const uint32_t gid = c.env_id_base + (uint32_t)e;
+    // the previous step's bulk store must have read the staging tile before it is rewritten
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 
     if (t >= c.T) {  // G28: finished env
-        stats_rewards_obs(c, m, tid, e, t, 1, 0.f, 0.f, 0.0, obs, rew);
+        __syncthreads();
+        stats_rewards_obs<NPAD>(c, m, tid, e, t, 1, 0.f, 0.f, 0.0, obs, rew);
         if (tid == 0 && done) done[e] = 1;
         __syncthreads();
         return;
@@ -572,11 +711,11 @@ __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const int
         }
         if (tid <= R) m.resoff[tid] = incl - q;  // resoff[R] = total (lanes >= R hold q = 0)
     }
-    for (int g = tid; g < c.n_groups; g += blockDim.x) m.gcnt[g] = 0;  // ready for the next step
+    for (int g = tid; g < c.n_groups; g += NPAD) m.gcnt[g] = 0;  // ready for the next step
     __syncthreads();  // #6
 
     // pop matched heads, then expired heads (G14), one thread per level
-    for (int l = tid; l < c.n_levels; l += blockDim.x) {
+    for (int l = tid; l < c.n_levels; l += NPAD) {
         const int book = l / P, pidx = l - book * P, r = book >> 1, side = book & 1;
         const int price = c.prices[pidx];
         const int tk = m.take[l];
@@ -697,7 +836,7 @@ __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const int
     }
 
     // ---------------- P5 rewards, P6 observations, clock ----------------
-    stats_rewards_obs(c, m, tid, e, t + 1, 0, coin_pre, labor_pre, cf_pre, obs, rew);
+    stats_rewards_obs<NPAD>(c, m, tid, e, t + 1, 0, coin_pre, labor_pre, cf_pre, obs, rew);
     if (tid == 0) {
         m.hdr->t = t + 1;
         if (done) done[e] = (uint8_t)(t + 1 == c.T);
@@ -705,50 +844,54 @@ __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const int
     __syncthreads();
 }
 
-template <int MAXT>
-__global__ void __launch_bounds__(MAXT) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
+template <int NPAD>
+__global__ void __launch_bounds__(NPAD) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const StepIO io) {
     extern __shared__ __align__(16) uint8_t smem[];
     const int e = blockIdx.x, tid = threadIdx.x;
     const Sm m = carve(c, smem);
     uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
-    for (int i = tid; i < c.blob_bytes / 16; i += blockDim.x) ((uint4*)smem)[i] = blob[i];
-    for (int i = tid; i < (c.smem_bytes - c.blob_bytes) / 4; i += blockDim.x) ((uint32_t*)(smem + c.blob_bytes))[i] = 0u;
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)smem)[i] = blob[i];
+    for (int i = tid; i < (c.smem_bytes - c.blob_bytes) / 4; i += NPAD) ((uint32_t*)(smem + c.blob_bytes))[i] = 0u;
     __syncthreads();
     if (!io.actions)
-        for (int i = tid; i < c.A; i += blockDim.x) m.cdf[i] = io.cdf[i];
+        for (int i = tid; i < c.A; i += NPAD) m.cdf[i] = io.cdf[i];
     __syncthreads();
     const size_t EN = (size_t)c.E * c.N, EB = (size_t)c.E * c.B;
     for (int s = 0; s < io.n_steps; ++s) {
         const int slot = s % io.ring_depth;
-        env_step(c, m, tid, e, io.actions ? io.actions + s * EN : nullptr, io.gov_actions ? io.gov_actions + s * EB : nullptr,
+        env_step<NPAD>(c, m, tid, e, io.actions ? io.actions + s * EN : nullptr, io.gov_actions ? io.gov_actions + s * EB : nullptr,
                  io.obs ? io.obs + (size_t)slot * c.obs_floats : nullptr, io.rew ? io.rew + (size_t)slot * (EN + c.E) : nullptr,
                  io.done ? io.done + (size_t)slot * c.E : nullptr, io.actions_out ? io.actions_out + slot * EN : nullptr,
                  io.gov_out ? io.gov_out + slot * EB : nullptr);
     }
     __syncthreads();
-    for (int i = tid; i < c.blob_bytes / 16; i += blockDim.x) blob[i] = ((uint4*)smem)[i];
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)smem)[i];
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
-template <int MAXT>
-__global__ void __launch_bounds__(MAXT) ej_observe_kernel(const __grid_constant__ DevCfg c, const uint8_t* __restrict__ state,
+template <int NPAD>
+__global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant__ DevCfg c, const uint8_t* __restrict__ state,
                                                           float* obs) {
     extern __shared__ __align__(16) uint8_t smem[];
     const int e = blockIdx.x, tid = threadIdx.x;
     const Sm m = carve(c, smem);
     const uint4* blob = (const uint4*)(state + (size_t)e * c.blob_bytes);
-    for (int i = tid; i < c.blob_bytes / 16; i += blockDim.x) ((uint4*)smem)[i] = blob[i];
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)smem)[i] = blob[i];
     __syncthreads();
-    stats_rewards_obs(c, m, tid, e, m.hdr->t, 2, 0.f, 0.f, 0.0, obs, nullptr);
+    for (int i = tid; i < (c.smem_bytes - c.blob_bytes) / 4; i += NPAD) ((uint32_t*)(smem + c.blob_bytes))[i] = 0u;
+    __syncthreads();
+    stats_rewards_obs<NPAD>(c, m, tid, e, m.hdr->t, 2, 0.f, 0.f, 0.0, obs, nullptr);
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // Reset (G29, G30): one CTA per env builds the blob in shared memory and stores it.
-template <int MAXT>
-__global__ void __launch_bounds__(MAXT) ej_reset_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state) {
+template <int NPAD>
+__global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state) {
     extern __shared__ __align__(16) uint8_t smem[];
     const int e = blockIdx.x, tid = threadIdx.x;
     const Sm m = carve(c, smem);
-    for (int i = tid; i < c.blob_bytes / 4; i += blockDim.x) ((uint32_t*)smem)[i] = 0u;
+    for (int i = tid; i < c.blob_bytes / 4; i += NPAD) ((uint32_t*)smem)[i] = 0u;
     __syncthreads();
     const uint32_t gid = c.env_id_base + (uint32_t)e;
     if (tid < c.N) {
@@ -770,7 +913,7 @@ __global__ void __launch_bounds__(MAXT) ej_reset_kernel(const __grid_constant__ 
             else m.SC[tid] = v;
         }
     }
-    for (int l = tid; l < c.n_levels; l += blockDim.x) { m.head[l] = (uint16_t)NIL; m.tail[l] = (uint16_t)NIL; }
+    for (int l = tid; l < c.n_levels; l += NPAD) { m.head[l] = (uint16_t)NIL; m.tail[l] = (uint16_t)NIL; }
     if (tid == 0) {  // all coins equal: gini = 0, prod = N * coin (exact)
         const double prod = (double)c.N * (double)c.starting_coin;
         const double eq = (double)c.omega * (1.0 - 0.0) + (1.0 - (double)c.omega);
@@ -778,7 +921,7 @@ __global__ void __launch_bounds__(MAXT) ej_reset_kernel(const __grid_constant__ 
     }
     __syncthreads();
     uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
-    for (int i = tid; i < c.blob_bytes / 16; i += blockDim.x) blob[i] = ((uint4*)smem)[i];
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)smem)[i];
 }
 
 // ------------------------------------------------------------------------------------------
@@ -859,21 +1002,34 @@ void build_layout(DevCfg& c) {
     c.o_roff = take(nl * 4);
     c.o_resq = take(32 * 4);
     c.o_resoff = take(32 * 4);
-    c.o_red = take((2 * c.n_metrics + 1) * c.n_warps * 8);
-    c.o_sortbuf = take(2 * c.Npad * 4);
+    c.o_red = take((c.n_metrics + 1) * c.n_warps * 8);
+    c.o_redq = take(c.n_metrics * c.n_warps * 4);
+    c.o_hist = take(R * HB * 4);
+    c.o_hovf = take(EJ_MAX_RESOURCES * 4);
+    c.o_sortbuf = take(2 * 3 * c.Npad * 4);
     c.o_shrow = take(c.shrow_len * 4);
     c.o_med = take(2 * c.n_metrics * 4);
     c.o_misc = take(16);
     c.o_cdf = take(c.A * 4);
+    c.o_stage = o;
+    c.stage_obs = 0;
+    if ((c.N * c.D_pop) % 4 == 0 && o + c.N * c.D_pop * 4 <= 100 * 1024) {  // bulk-store staging tile
+        c.stage_obs = 1;
+        take(c.N * c.D_pop * 4);
+    }
     c.smem_bytes = o;
 }
 
 template <typename F>
 int for_block_size(int Npad, F&& f) {
-    if (Npad <= 128) return f(std::integral_constant<int, 128>());
-    if (Npad <= 256) return f(std::integral_constant<int, 256>());
-    if (Npad <= 512) return f(std::integral_constant<int, 512>());
-    return f(std::integral_constant<int, 1024>());
+    switch (Npad) {
+        case 32: return f(std::integral_constant<int, 32>());
+        case 64: return f(std::integral_constant<int, 64>());
+        case 128: return f(std::integral_constant<int, 128>());
+        case 256: return f(std::integral_constant<int, 256>());
+        case 512: return f(std::integral_constant<int, 512>());
+        default: return f(std::integral_constant<int, 1024>());
+    }
 }
 
 int launch_step(ej_env* h, const StepIO& io) {
