@@ -1,0 +1,947 @@
+// ej_device.cuh -- device side of the batched EconoJax environment step (sm_100a).
+//
+// One CTA per economy; thread i is population agent i.  The whole state of an economy (agent
+// arrays, per-level FIFO order books, order pool) is one contiguous "blob" that is copied into
+// shared memory at kernel start and written back at kernel end; ej_rollout keeps it there for
+// T steps.  Citations: "P:n" = PAPER.md line n, "G#" = DESIGN.md section 3 readings.
+//
+// Arithmetic contract (G31): agent state is binary32 and every state-changing float operation
+// is ONE correctly rounded operation (__fadd_rn / __fmul_rn / __fsub_rn / __fdiv_rn: never
+// contracted to FMA); cross-agent accumulations are integers (order-free, atomics allowed);
+// rewards and statistics are evaluated in binary64 where cancellation matters.
+//
+// Order book: every (resource, side, price) level is a FIFO in arrival order
+// because the price grid is discrete and an older step always precedes a newer one (G11), so
+// both kinds of removal -- matching (best price first, then earliest arrival) and
+// expiry (oldest first) -- pop queue heads.  Levels are singly linked lists threaded
+// through a pool in which agent i owns slots [i*Mp, i*Mp+M): an agent places at most one order
+// per step and holds at most M, so slot allocation is a private bitmask operation.
+//
+// Barriers per step (book_cap == 0): arrivals pushed | linked | level pops | trades settled |
+// state final | outputs staged.  Government statistics are warp-specialised: one warp owns one
+// metric, holds all N values in registers (N/32 per lane) and needs no block barrier.
+#pragma once
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include "../../include/econojax.h"
+
+namespace {
+
+constexpr uint32_t NIL = 0xFFFFu;      // null slot of the order pool
+constexpr uint32_t FULL = 0xffffffffu;
+constexpr int HB = 128;                // histogram bins of the integer-metric medians
+
+struct EnvHdr {
+    int32_t t;
+    int32_t n_trades, n_placed, n_invalid, n_expired, n_bad_gov;
+    int32_t pad0[2];
+    double u_g_prev;
+    double pad1;
+    float rates[EJ_MAX_BRACKETS];
+    int32_t last_price[EJ_MAX_RESOURCES];
+};
+static_assert(sizeof(EnvHdr) % 16 == 0, "EnvHdr must keep 16-byte alignment");
+
+struct DevCfg {
+    int E, N, R, P, B, L, M, Mp_log2, K, T, period, expiry;
+    int craft_units, craft_distinct, craft_mode, allow_noop, taxes_enabled, skill_init;
+    int A, base_craft, base_buy, base_sell, n_levels, n_groups, D_pop, D_gov, D_gov_pad;
+    int N4, Npad, n_metrics, n_warps, shrow_len, stage_obs;
+    int prices[EJ_MAX_PRICES];
+    float thresholds[EJ_MAX_BRACKETS];
+    float rate_table[EJ_MAX_RATE_LEVELS];
+    float starting_coin, labor_craft, labor_gather, labor_trade, eta, omega, craft_scale;
+    float clip_lo, clip_hi, s_coin, s_count, s_price, s_labor;
+    double inv_n;  // 1 / N
+    uint32_t env_id_base, seed_lo, seed_hi;
+    // blob section offsets (bytes from the blob base)
+    int o_coin, o_labor, o_income, o_SC, o_esc_coin, o_mask, o_cf, o_SG, o_inv, o_esc_res;
+    int o_head, o_tail, o_cnt, o_pool, blob_bytes;
+    // scratch section offsets (bytes from the shared-memory base; all after the blob)
+    int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma, o_bucket, o_sorted;
+    int o_gcnt, o_goff, o_resq, o_hist, o_shrow, o_govrow, o_misc, o_cdf, o_stage;
+    int smem_bytes;
+    unsigned long long gov_obs_offset, obs_floats;
+};
+
+struct StepIO {
+    const int32_t* actions;      // [n_steps][E][N] or null (generate)
+    const int32_t* gov_actions;  // [n_steps][E][B] or null (generate)
+    float* obs;                  // ring of obs buffers or null
+    float* rew;                  // ring [E][N+1] or null
+    uint8_t* done;               // ring [E] or null
+    int32_t* actions_out;        // ring [E][N] or null
+    int32_t* gov_out;            // ring [E][B] or null
+    const uint32_t* cdf;         // [A] device
+    int n_steps, ring_depth;
+};
+
+struct Sm {
+    EnvHdr* hdr;
+    float *coin, *labor, *income, *SC;
+    int* esc_coin;
+    uint32_t* mask;
+    double* cf;
+    float* SG;
+    int *inv, *esc_res;
+    uint16_t *head, *tail;
+    int* cnt;  // [2][n_levels]: buffer (t & 1) is current
+    uint32_t* pool;
+    uint32_t* key;
+    int* cinfo;
+    uint32_t *cslot, *anext, *ahead;
+    int *credit, *sale;
+    uint32_t *mb, *ma;
+    unsigned long long* bucket;
+    uint32_t* sorted;
+    int *gcnt, *goff, *resq, *hist;
+    float *shrow, *govrow;
+    unsigned long long* misc;  // [0] tax pool in 2^-20 coin
+    uint32_t* cdf;
+    float* stage;
+};
+
+__device__ __forceinline__ Sm carve(const DevCfg& c, uint8_t* s) {
+    Sm m;
+    m.hdr = (EnvHdr*)s;
+    m.coin = (float*)(s + c.o_coin);
+    m.labor = (float*)(s + c.o_labor);
+    m.income = (float*)(s + c.o_income);
+    m.SC = (float*)(s + c.o_SC);
+    m.esc_coin = (int*)(s + c.o_esc_coin);
+    m.mask = (uint32_t*)(s + c.o_mask);
+    m.cf = (double*)(s + c.o_cf);
+    m.SG = (float*)(s + c.o_SG);
+    m.inv = (int*)(s + c.o_inv);
+    m.esc_res = (int*)(s + c.o_esc_res);
+    m.head = (uint16_t*)(s + c.o_head);
+    m.tail = (uint16_t*)(s + c.o_tail);
+    m.cnt = (int*)(s + c.o_cnt);
+    m.pool = (uint32_t*)(s + c.o_pool);
+    m.key = (uint32_t*)(s + c.o_key);
+    m.cinfo = (int*)(s + c.o_cinfo);
+    m.cslot = (uint32_t*)(s + c.o_cslot);
+    m.anext = (uint32_t*)(s + c.o_anext);
+    m.ahead = (uint32_t*)(s + c.o_ahead);
+    m.credit = (int*)(s + c.o_credit);
+    m.sale = (int*)(s + c.o_sale);
+    m.mb = (uint32_t*)(s + c.o_mb);
+    m.ma = (uint32_t*)(s + c.o_ma);
+    m.bucket = (unsigned long long*)(s + c.o_bucket);
+    m.sorted = (uint32_t*)(s + c.o_sorted);
+    m.gcnt = (int*)(s + c.o_gcnt);
+    m.goff = (int*)(s + c.o_goff);
+    m.resq = (int*)(s + c.o_resq);
+    m.hist = (int*)(s + c.o_hist);
+    m.shrow = (float*)(s + c.o_shrow);
+    m.govrow = (float*)(s + c.o_govrow);
+    m.misc = (unsigned long long*)(s + c.o_misc);
+    m.cdf = (uint32_t*)(s + c.o_cdf);
+    m.stage = (float*)(s + c.o_stage);
+    return m;
+}
+
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), G30.
+__device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
+                                              uint32_t k1, uint32_t& o0, uint32_t& o1, uint32_t& o2, uint32_t& o3) {
+#pragma unroll
+    for (int round = 0; round < 10; ++round) {
+        const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+        const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = hi1 ^ c1 ^ k0, n2 = hi0 ^ c3 ^ k1;
+        c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    o0 = c0; o1 = c1; o2 = c2; o3 = c3;
+}
+
+__device__ __forceinline__ float u01(uint32_t x) { return (float)(x >> 8) * (1.0f / 16777216.0f); }
+
+// Coin term of Eq.1: (C^(1-eta) - 1) / (1-eta), binary64.
+__device__ __forceinline__ double coin_utility(float C, double a) { return (pow((double)C, a) - 1.0) / a; }
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+    return v;
+}
+__device__ __forceinline__ float warp_sum(float v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = __fadd_rn(v, __shfl_xor_sync(FULL, v, o));
+    return v;
+}
+
+// Bitonic sorting network over 32*EPL values held by one warp, element idx = q*32 + lane,
+// ascending in idx.  Strides >= 32 are register-to-register (direction known at compile time),
+// strides < 32 are warp shuffles.  No barriers.
+template <int EPL>
+__device__ __forceinline__ void warp_sort(float (&x)[EPL], int lane) {
+    constexpr int NP = 32 * EPL;
+#pragma unroll
+    for (int k = 2; k <= NP; k <<= 1) {
+#pragma unroll
+        for (int j = k >> 1; j > 0; j >>= 1) {
+            if (j >= 32) {
+                const int dq = j >> 5;
+#pragma unroll
+                for (int q = 0; q < EPL; ++q) {
+                    if ((q & dq) == 0) {
+                        const int q2 = q | dq;
+                        const bool up = (k >= NP) ? true : (((q << 5) & k) == 0);
+                        const float lo = fminf(x[q], x[q2]), hi = fmaxf(x[q], x[q2]);
+                        x[q] = up ? lo : hi;
+                        x[q2] = up ? hi : lo;
+                    }
+                }
+            } else {
+                const bool lane_lower = (lane & j) == 0;
+#pragma unroll
+                for (int q = 0; q < EPL; ++q) {
+                    const float y = __shfl_xor_sync(FULL, x[q], j);
+                    bool up;
+                    if (k >= NP) up = true;
+                    else if (k >= 32) up = (((q << 5) & k) == 0);
+                    else up = (lane & k) == 0;
+                    x[q] = (up == lane_lower) ? fminf(x[q], y) : fmaxf(x[q], y);
+                }
+            }
+        }
+    }
+}
+
+// Element of rank `rank` (0-based) of a sorted warp-held array.
+template <int EPL>
+__device__ __forceinline__ float warp_pick(const float (&x)[EPL], int rank) {
+    const int q = rank >> 5;
+    float v = x[0];
+#pragma unroll
+    for (int qq = 1; qq < EPL; ++qq) v = (q == qq) ? x[qq] : v;
+    return __shfl_sync(FULL, v, rank & 31);
+}
+
+__device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm& m, int k, double mean, float q_sum, float lo, float hi,
+                                           float scale) {
+    const float sd = __fsqrt_rn((float)((double)q_sum * c.inv_n));
+    const float med = (c.N & 1) ? hi : __fmul_rn(0.5f, __fadd_rn(lo, hi));
+    m.govrow[3 * k + 0] = (float)(mean * (double)scale);
+    m.govrow[3 * k + 1] = __fmul_rn(sd, scale);
+    m.govrow[3 * k + 2] = __fmul_rn(med, scale);
+}
+
+// One warp computes mean, std, median (Fig.1, G26) of one float metric; for coin
+// also the welfare u_g = eq * prod (Eq.3-5; G22, G23) and the government reward.
+// Sum in binary64; squared deviations in binary32 (non-negative terms: relative error < 1e-6).
+//   mode 0 = step, 1 = finished env (reward 0), 2 = observe only
+template <int EPL>
+__device__ __forceinline__ void metric_float(const DevCfg& c, const Sm& m, const float* arr, int lane, int k, int mode, int e,
+                                             float* rew) {
+    const int N = c.N;
+    float x[EPL];
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) {
+        const int idx = q * 32 + lane;
+        x[q] = idx < N ? arr[idx] : INFINITY;
+        s += idx < N ? (double)x[q] : 0.0;
+    }
+    s = warp_sum(s);
+    const double mean = s * c.inv_n;
+    float qs = 0.0f;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) {
+        const float d = (q * 32 + lane) < N ? (float)((double)x[q] - mean) : 0.0f;
+        qs = __fadd_rn(qs, __fmul_rn(d, d));
+    }
+    qs = warp_sum(qs);
+    warp_sort<EPL>(x, lane);
+    const float lo = warp_pick<EPL>(x, N >= 2 ? (N >> 1) - 1 : 0), hi = warp_pick<EPL>(x, N >> 1);
+    if (k == 0 && mode != 2) {
+        // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)  =>  gini * prod = gn / N   (G23)
+        double g = 0.0;
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) {
+            const int idx = q * 32 + lane;
+            g += idx < N ? (double)(2 * idx - N + 1) * (double)x[q] : 0.0;
+        }
+        g = warp_sum(g);
+        if (lane == 0) {
+            // u_g = (omega (1 - gini) + (1 - omega)) prod = prod - omega * gini * prod; gini = 0 when
+            // prod = 0 or N = 1 (then gn = 0 as well)
+            const double ug = s - (double)c.omega * (g * c.inv_n);
+            if (mode == 0) {
+                if (rew) rew[(size_t)e * (N + 1) + N] = (float)(ug - m.hdr->u_g_prev);
+                m.hdr->u_g_prev = ug;
+            } else if (rew) {
+                rew[(size_t)e * (N + 1) + N] = 0.0f;
+            }
+        }
+    }
+    if (lane == 0) gov_triple(c, m, k, mean, qs, lo, hi, k == 1 ? c.s_labor : c.s_coin);
+}
+
+// Same for an integer metric (inventory of one resource): exact integer sum (REDUX), median
+// from a per-warp shared-memory histogram when every value is below HB, else from the sorting
+// network.
+template <int EPL>
+__device__ __forceinline__ void metric_int(const DevCfg& c, const Sm& m, const int* arr, int lane, int k, int* hist) {
+    const int N = c.N;
+    int v[EPL];
+    int s = 0, mx = 0;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) {
+        const int idx = q * 32 + lane;
+        v[q] = idx < N ? arr[idx] : -1;
+        s += idx < N ? v[q] : 0;
+        mx = max(mx, v[q]);
+    }
+    s = __reduce_add_sync(FULL, s);
+    mx = __reduce_max_sync(FULL, mx);
+    const double mean = (double)s * c.inv_n;
+    float qs = 0.0f;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) {
+        const float d = v[q] >= 0 ? (float)((double)v[q] - mean) : 0.0f;
+        qs = __fadd_rn(qs, __fmul_rn(d, d));
+    }
+    qs = warp_sum(qs);
+    float lo, hi;
+    if (mx < HB) {
+        ((int4*)hist)[lane] = make_int4(0, 0, 0, 0);
+        __syncwarp();
+#pragma unroll
+        for (int q = 0; q < EPL; ++q)
+            if (v[q] >= 0) atomicAdd(&hist[v[q]], 1);
+        __syncwarp();
+        const int4 h4 = ((int4*)hist)[lane];
+        const int c0 = h4.x, c1 = c0 + h4.y, c2 = c1 + h4.z, c3 = c2 + h4.w;
+        int incl = c3;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(FULL, incl, o);
+            if (lane >= o) incl += y;
+        }
+        const int excl = incl - c3;
+        int vals[2];
+#pragma unroll
+        for (int j = 0; j < 2; ++j) {  // value of 0-based rank r = smallest value with cum(value) > r
+            const int rk = max((N >> 1) - 1 + j, 0);
+            const unsigned ball = __ballot_sync(FULL, incl > rk);
+            const int src = __ffs(ball) - 1;
+            const int rel = rk - __shfl_sync(FULL, excl, src);
+            const int a0 = __shfl_sync(FULL, c0, src), a1 = __shfl_sync(FULL, c1, src), a2 = __shfl_sync(FULL, c2, src);
+            vals[j] = src * 4 + (rel < a0 ? 0 : rel < a1 ? 1 : rel < a2 ? 2 : 3);
+        }
+        lo = (float)vals[0];
+        hi = (float)vals[1];
+    } else {
+        float x[EPL];
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) x[q] = v[q] >= 0 ? (float)v[q] : INFINITY;
+        warp_sort<EPL>(x, lane);
+        lo = warp_pick<EPL>(x, N >= 2 ? (N >> 1) - 1 : 0);
+        hi = warp_pick<EPL>(x, N >> 1);
+    }
+    if (lane == 0) gov_triple(c, m, k, mean, qs, lo, hi, c.s_count);
+}
+
+// Shared tail of the population rows: market statistics of the post-step books.
+__device__ __forceinline__ void write_market_row(const DevCfg& c, const Sm& m, int r, const int* cnt) {
+    int best_bid = 0, best_ask = 0, nb = 0, na = 0;
+    for (int p = 0; p < c.P; ++p) {
+        const int cb = cnt[(r * 2 + 0) * c.P + p], ca = cnt[(r * 2 + 1) * c.P + p];
+        nb += cb;
+        na += ca;
+        if (cb > 0) best_bid = c.prices[p];
+        if (ca > 0 && best_ask == 0) best_ask = c.prices[p];
+    }
+    float* o = m.shrow + r * 5;
+    o[0] = __fmul_rn((float)best_bid, c.s_price);
+    o[1] = __fmul_rn((float)best_ask, c.s_price);
+    o[2] = __fmul_rn((float)nb, c.s_count);
+    o[3] = __fmul_rn((float)na, c.s_count);
+    o[4] = __fmul_rn((float)m.hdr->last_price[r], c.s_price);
+}
+__device__ __forceinline__ void write_timers(const DevCfg& c, const Sm& m, int tq) {
+    m.shrow[5 * c.R + c.B] = __fdiv_rn((float)(tq % c.period), (float)c.period);
+    m.shrow[5 * c.R + c.B + 1] = __fdiv_rn((float)tq, (float)c.T);
+}
+
+// Rewards, government statistics and both observation blocks of the state in shared memory.
+// Called after a block barrier that made the state (and m.shrow) final.
+//   mode     0 = step, 1 = finished env (rewards 0), 2 = observe only
+//   rows     0 = rewrite only the columns that change every step, 1 = also the tax rates,
+//            2 = every column (first step of a launch: skills)
+template <int NPAD>
+__device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
+                        double cf_pre, float* obs, float* rew) {
+    constexpr int NW = NPAD / 32, EPL = NPAD / 32;
+    const int N = c.N, R = c.R, N4 = c.N4;
+    const bool act = tid < N;
+    const int lane = tid & 31, warp = tid >> 5;
+    const bool staged = c.stage_obs && obs;
+
+    if (act) {
+        const float coin = m.coin[tid], labor = m.labor[tid];
+        // ---- population reward: u(post) - u(pre), u = coin term - labor (Eq.1-2) ----
+        if (mode == 0) {
+            double cf_post = cf_pre;
+            if (__float_as_uint(coin) != __float_as_uint(coin_pre)) {
+                cf_post = coin_utility(coin, 1.0 - (double)c.eta);
+                m.cf[tid] = cf_post;
+            }
+            if (rew) rew[(size_t)e * (N + 1) + tid] = (float)((cf_post - (double)labor) - (cf_pre - (double)labor_pre));
+        } else if (mode == 1 && rew) {
+            rew[(size_t)e * (N + 1) + tid] = 0.0f;
+        }
+        // ---- this agent's observation row (G25) in the staging tile ----
+        if (staged) {
+            float* o = m.stage + tid * c.D_pop;
+            o[0] = __fmul_rn(coin, c.s_coin);
+            for (int r = 0; r < R; ++r) o[1 + r] = __fmul_rn((float)m.inv[r * N4 + tid], c.s_count);
+            o[R + 1] = __fmul_rn((float)m.esc_coin[tid], c.s_coin);
+            for (int r = 0; r < R; ++r) o[R + 2 + r] = __fmul_rn((float)m.esc_res[r * N4 + tid], c.s_count);
+            o[3 * R + 3] = __fmul_rn(labor, c.s_labor);
+            float* tl = o + 3 * R + 4;
+            for (int k = 0; k < 5 * R; ++k) tl[k] = m.shrow[k];
+            tl[5 * R + c.B] = m.shrow[5 * R + c.B];
+            tl[5 * R + c.B + 1] = m.shrow[5 * R + c.B + 1];
+            if (rows >= 1)
+                for (int b = 0; b < c.B; ++b) tl[5 * R + b] = m.shrow[5 * R + b];
+            if (rows >= 2) {
+                for (int r = 0; r < R; ++r) o[2 * R + 2 + r] = m.SG[r * N4 + tid];
+                o[3 * R + 2] = m.SC[tid];
+            }
+        }
+    }
+
+    // ---- government statistics: metric k is owned by one warp ----
+#pragma unroll
+    for (int k = 0; k < 3; ++k)
+        if ((k % NW) == warp) metric_float<EPL>(c, m, k == 0 ? m.coin : k == 1 ? m.labor : m.income, lane, k, mode, e, rew);
+    for (int r = 0; r < R; ++r) {
+        const int w = NW - 1 - (r % NW);
+        if (w == warp) metric_int<EPL>(c, m, m.inv + r * N4, lane, 3 + r, m.hist + (r % NW) * HB);
+    }
+    for (int k = tid; k < c.B + 2; k += NPAD) m.govrow[3 * c.n_metrics + k] = m.shrow[5 * R + k];
+
+    if (obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+
+    if (obs && tid == 0) {  // bulk stores: the env's contiguous [N][D_pop] tile and its government row
+        if (staged) {
+            float* dst = obs + (size_t)e * N * c.D_pop;
+            const uint32_t src = (uint32_t)__cvta_generic_to_shared(m.stage);
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(N * c.D_pop * 4) : "memory");
+        }
+        float* gdst = obs + c.gov_obs_offset + (size_t)e * c.D_gov_pad;
+        const uint32_t gsrc = (uint32_t)__cvta_generic_to_shared(m.govrow);
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(gsrc), "r"(c.D_gov_pad * 4) : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+    }
+    // ---- population rows when they cannot go out as one bulk store: coalesced loop ----
+    if (obs && !staged) {
+        const int D = c.D_pop, priv = 3 * R + 4, total = N * D;
+        float* dst = obs + (size_t)e * total;
+        for (int idx = tid; idx < total; idx += NPAD) {
+            const int i = idx / D, k = idx - i * D;
+            float v;
+            if (k >= priv) v = m.shrow[k - priv];
+            else if (k == 0) v = __fmul_rn(m.coin[i], c.s_coin);
+            else if (k <= R) v = __fmul_rn((float)m.inv[(k - 1) * N4 + i], c.s_count);
+            else if (k == R + 1) v = __fmul_rn((float)m.esc_coin[i], c.s_coin);
+            else if (k <= 2 * R + 1) v = __fmul_rn((float)m.esc_res[(k - R - 2) * N4 + i], c.s_count);
+            else if (k <= 3 * R + 1) v = m.SG[(k - 2 * R - 2) * N4 + i];
+            else if (k == 3 * R + 2) v = m.SC[i];
+            else v = __fmul_rn(m.labor[i], c.s_labor);
+            dst[idx] = v;
+        }
+    }
+}
+
+struct StepPtrs {
+    const int32_t* actions;
+    const int32_t* gov_actions;
+    float* obs;
+    float* rew;
+    uint8_t* done;
+    int32_t* actions_out;
+    int32_t* gov_out;
+};
+
+// One environment step on the state in shared memory (G1: actions -> match -> expire -> tax ->
+// rewards -> observations -> t++).  `first` = first step of this launch (full observation rows).
+template <int NPAD>
+__device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const StepPtrs& io, bool first) {
+    const int N = c.N, R = c.R, P = c.P, N4 = c.N4, nl = c.n_levels;
+    const bool act = tid < N;
+    const int t = m.hdr->t;
+    const uint32_t gid = c.env_id_base + (uint32_t)e;
+    // the previous step's bulk stores must have read the staging tile before it is rewritten
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+
+    if (t >= c.T) {  // G28: finished env
+        if (tid < R) write_market_row(c, m, tid, m.cnt + (t & 1) * nl);
+        if (tid < c.B) m.shrow[5 * R + tid] = m.hdr->rates[tid];
+        if (tid == NPAD - 1) write_timers(c, m, t);
+        __syncthreads();
+        outputs<NPAD>(c, m, tid, e, 1, 2, 0.f, 0.f, 0.0, io.obs, io.rew);
+        if (tid == 0 && io.done) io.done[e] = 1;
+        __syncthreads();
+        return;
+    }
+    int* cnt_cur = m.cnt + (t & 1) * nl;
+    int* cnt_nxt = m.cnt + ((t & 1) ^ 1) * nl;
+
+    // ---------------- P1 actions (one action per agent per step) ----------------
+    uint32_t x0 = 0, x1 = 0, x2 = 0, x3 = 0;
+    int a = -1;
+    if (act) {
+        philox4x32_10(gid, (uint32_t)tid, (uint32_t)t, 0u, c.seed_lo, c.seed_hi, x0, x1, x2, x3);
+        if (io.actions) {
+            a = io.actions[(size_t)e * N + tid];
+        } else {  // smallest a with x0 < cdf[a]; last entry read as 2^32 (G30)
+            int lo = 0, hi = c.A - 1;
+            while (lo < hi) {
+                const int mid = (lo + hi) >> 1;
+                if (x0 < m.cdf[mid]) hi = mid;
+                else lo = mid + 1;
+            }
+            a = lo;
+        }
+        if (io.actions_out) io.actions_out[(size_t)e * N + tid] = a;
+        m.key[tid] = x2;
+    }
+    // government levels for the period boundary
+    int gov_lvl = -1;
+    const bool boundary = c.taxes_enabled && ((t + 1) % c.period == 0);
+    if (tid < c.B && (boundary || io.gov_out)) {
+        if (io.gov_actions) {
+            gov_lvl = io.gov_actions[(size_t)e * c.B + tid];
+        } else {
+            uint32_t g0, g1, g2, g3;
+            philox4x32_10(gid, (uint32_t)N, (uint32_t)t, (uint32_t)(1 + tid / 4), c.seed_lo, c.seed_hi, g0, g1, g2, g3);
+            const uint32_t gx = (tid & 3) == 0 ? g0 : (tid & 3) == 1 ? g1 : (tid & 3) == 2 ? g2 : g3;
+            gov_lvl = (int)(((unsigned long long)gx * (unsigned long long)c.L) >> 32);
+        }
+        if (io.gov_out) io.gov_out[(size_t)e * c.B + tid] = gov_lvl;
+    }
+
+    float coin_pre = 0.f, labor_pre = 0.f;
+    double cf_pre = 0.0;
+    int lvl = -1, grp = 0, pos = 0, price_c = 0, r_c = 0, side_c = 0;
+    uint32_t slot = 0, mymask = 0, old_tail = NIL;
+    if (act) {
+        coin_pre = m.coin[tid];
+        labor_pre = m.labor[tid];
+        cf_pre = m.cf[tid];
+        mymask = m.mask[tid];
+        bool invalid = false;
+        if (a < 0 || a >= c.A) {
+            invalid = true;  // G2
+        } else if (a < R) {  // gather: floor(SG + rho), rho = u * 1.1 (G8)
+            const float rho = __fmul_rn(u01(x1), 1.1f);
+            const float s = __fadd_rn(m.SG[a * N4 + tid], rho);
+            m.inv[a * N4 + tid] += (int)floorf(s);
+            m.labor[tid] = __fadd_rn(labor_pre, c.labor_gather);
+        } else if (a < c.base_buy) {  // craft
+            bool ok;
+            if (c.craft_mode == EJ_CRAFT_PER_RESOURCE) {
+                const int r = a - R;
+                ok = m.inv[r * N4 + tid] >= c.craft_units;
+                if (ok) m.inv[r * N4 + tid] -= c.craft_units;
+            } else {
+                int enough = 0;
+                for (int r = 0; r < R; ++r) enough += m.inv[r * N4 + tid] >= c.craft_units;
+                ok = enough >= c.craft_distinct;
+                if (ok) {  // the R_d most-held resources, ties to the lowest index (G7)
+                    uint32_t used = 0;
+                    for (int k = 0; k < c.craft_distinct; ++k) {
+                        int best = -1, bestv = 0;
+                        for (int r = 0; r < R; ++r) {
+                            if ((used >> r) & 1u) continue;
+                            const int v = m.inv[r * N4 + tid];
+                            if (best < 0 || v > bestv) { best = r; bestv = v; }
+                        }
+                        used |= 1u << best;
+                        m.inv[best * N4 + tid] = bestv - c.craft_units;
+                    }
+                }
+            }
+            if (ok) {
+                const float pay = __fmul_rn(m.SC[tid], c.craft_scale);
+                m.coin[tid] = __fadd_rn(coin_pre, pay);
+                m.income[tid] = __fadd_rn(m.income[tid], pay);
+                m.labor[tid] = __fadd_rn(labor_pre, c.labor_craft);
+            } else {
+                invalid = true;
+            }
+        } else if (a < c.base_sell + R * P) {  // market order
+            side_c = a >= c.base_sell;
+            const int k = a - (side_c ? c.base_sell : c.base_buy);
+            r_c = k / P;
+            const int pidx = k - r_c * P;
+            price_c = c.prices[pidx];
+            bool ok = __popc(mymask) < c.M;
+            if (side_c == 0) ok = ok && (coin_pre >= (float)price_c);
+            else ok = ok && (m.inv[r_c * N4 + tid] >= 1);
+            if (ok) {
+                lvl = (r_c * 2 + side_c) * P + pidx;
+                slot = ((uint32_t)tid << c.Mp_log2) + (uint32_t)(__ffs(~mymask) - 1);
+                m.cslot[tid] = slot;
+                old_tail = m.tail[lvl];  // read before anyone links (tails change after barrier #1)
+                if (c.K) {
+                    grp = r_c * 2 + side_c;
+                    pos = atomicAdd(&m.gcnt[grp], 1);
+                    m.cinfo[tid] = lvl;
+                } else {  // push on the level's arrival stack
+                    m.anext[tid] = atomicExch(&m.ahead[lvl], (uint32_t)tid);
+                }
+            } else {
+                invalid = true;
+            }
+        }  // else NO-OP
+        if (invalid) atomicAdd(&m.hdr->n_invalid, 1);
+    }
+    __syncthreads();  // #1 arrivals registered
+
+    // Arrival order of this step's candidates: (key, agent) (G11).  Each candidate finds its rank
+    // among the step's arrivals on its level and its successor; with a book cap also its rank on
+    // the book, counted from the book size at step start (G15).
+    int lrank = 0;
+    bool accepted = false;
+    uint32_t nxt = NIL;
+    if (c.K == 0) {
+        if (lvl >= 0) {
+            int succ = -1;
+            uint32_t sk = 0;
+            uint32_t j = m.ahead[lvl];
+            while (j != NIL) {
+                if ((int)j != tid) {
+                    const uint32_t kj = m.key[j];
+                    const bool later = (kj > x2) || (kj == x2 && (int)j > tid);
+                    if (!later) ++lrank;
+                    else if (succ < 0 || kj < sk || (kj == sk && (int)j < succ)) { succ = (int)j; sk = kj; }
+                }
+                j = m.anext[j];
+            }
+            if (succ >= 0) nxt = m.cslot[succ];
+            accepted = true;
+        }
+    } else {
+        // exclusive scan of the per-book candidate counts (warp 0)
+        if (tid < 32) {
+            int carry = 0;
+            for (int base = 0; base < c.n_groups; base += 32) {
+                const int g = base + tid;
+                const int v = g < c.n_groups ? m.gcnt[g] : 0;
+                int incl = v;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int y = __shfl_up_sync(FULL, incl, o);
+                    if (tid >= o) incl += y;
+                }
+                if (g < c.n_groups) m.goff[g] = carry + incl - v;
+                carry += __shfl_sync(FULL, incl, 31);
+            }
+        }
+        __syncthreads();
+        const unsigned long long mine = ((unsigned long long)x2 << 32) | (unsigned long long)tid;
+        if (lvl >= 0) m.bucket[m.goff[grp] + pos] = mine;
+        __syncthreads();
+        int before = 0, gbase = 0, gn = 0;
+        if (lvl >= 0) {
+            gbase = m.goff[grp];
+            gn = m.gcnt[grp];
+            int brank = 0;
+            for (int k = 0; k < gn; ++k) {
+                const unsigned long long o = m.bucket[gbase + k];
+                const int lj = m.cinfo[(int)(o & 0xFFFFFFFFu)];
+                const bool earlier = o < mine, same = lj == lvl;
+                brank += earlier;
+                lrank += same && earlier;
+                before += (lj < lvl) || (same && earlier);
+            }
+            int n_rest = 0;
+            for (int p = 0; p < P; ++p) n_rest += cnt_cur[grp * P + p];
+            accepted = n_rest + brank < c.K;
+            m.sorted[gbase + before] = (uint32_t)tid | (accepted ? 0x10000u : 0u);
+        }
+        __syncthreads();
+        if (lvl >= 0 && accepted && before + 1 < gn) {
+            const uint32_t s = m.sorted[gbase + before + 1];
+            const int j = (int)(s & 0xFFFFu);
+            if ((s & 0x10000u) && m.cinfo[j] == lvl) nxt = m.cslot[j];
+        }
+        for (int g = tid; g < c.n_groups; g += NPAD) m.gcnt[g] = 0;  // ready for the next step
+    }
+
+    if (lvl >= 0) {
+        if (accepted) {
+            m.pool[slot] = nxt | (((uint32_t)t & 0xFFFFu) << 16);
+            if (lrank == 0) {
+                if (old_tail != NIL) m.pool[old_tail] = (m.pool[old_tail] & 0xFFFF0000u) | slot;
+                else m.head[lvl] = (uint16_t)slot;
+            }
+            if (nxt == NIL) m.tail[lvl] = (uint16_t)slot;
+            atomicAdd(&cnt_cur[lvl], 1);
+            m.mask[tid] = mymask | (1u << (slot & ((1u << c.Mp_log2) - 1u)));
+            if (side_c == 0) {  // escrow
+                m.coin[tid] = __fsub_rn(coin_pre, (float)price_c);
+                m.esc_coin[tid] += price_c;
+            } else {
+                m.inv[r_c * N4 + tid] -= 1;
+                m.esc_res[r_c * N4 + tid] += 1;
+            }
+            m.labor[tid] = __fadd_rn(labor_pre, c.labor_trade);
+            atomicAdd(&m.hdr->n_placed, 1);
+        } else {
+            atomicAdd(&m.hdr->n_invalid, 1);
+        }
+    }
+    __syncthreads();  // #2 books hold this step's arrivals
+
+    // ---------------- P2 match + P3 expire (G14) ----------------
+    // One thread per level.  Trades of a resource: q = max_p min(#bids >= p, #asks <= p); the
+    // q best bids and q best asks are popped from the queue heads, then the expired heads.
+    for (int l = tid; l < nl; l += NPAD) {
+        const int book = l / P, pidx = l - book * P, r = book >> 1, side = book & 1;
+        const int price = c.prices[pidx];
+        const int lb = (r * 2) * P, la = lb + P;
+        int totB = 0;
+        for (int p = 0; p < P; ++p) totB += cnt_cur[lb + p];
+        int q = 0, ale = 0, prefB = 0, alt_me = 0, bgt_me = 0;
+        for (int p = 0; p < P; ++p) {
+            if (p == pidx) alt_me = ale;
+            ale += cnt_cur[la + p];
+            const int cb = cnt_cur[lb + p];
+            q = max(q, min(totB - prefB, ale));
+            prefB += cb;
+            if (p == pidx) bgt_me = totB - prefB;
+        }
+        const int better = side ? alt_me : bgt_me;  // orders ahead of this level on its side
+        int n = cnt_cur[l];
+        const int tk = max(0, min(n, q - better));
+        uint32_t h = m.head[l];
+        if (tk > 0) {
+            uint32_t* dst = (side ? m.ma : m.mb) + r * N4 + better;
+            for (int k = 0; k < tk; ++k) {
+                dst[k] = h | ((uint32_t)pidx << 16);
+                h = m.pool[h] & 0xFFFFu;
+            }
+            n -= tk;
+        }
+        int nexp = 0;
+        while (h != NIL) {
+            const uint32_t pe = m.pool[h];
+            const uint32_t age = ((uint32_t)t - (pe >> 16)) & 0xFFFFu;
+            if ((int)age < c.expiry) break;
+            const int owner = (int)(h >> c.Mp_log2);
+            if (side == 0) {
+                atomicSub(&m.esc_coin[owner], price);
+                atomicAdd(&m.credit[owner], price);
+            } else {
+                atomicSub(&m.esc_res[r * N4 + owner], 1);
+                atomicAdd(&m.inv[r * N4 + owner], 1);
+            }
+            atomicAnd(&m.mask[owner], ~(1u << (h & ((1u << c.Mp_log2) - 1u))));
+            ++nexp;
+            --n;
+            h = pe & 0xFFFFu;
+        }
+        if (tk > 0 || nexp > 0) {
+            m.head[l] = (uint16_t)h;
+            if (h == NIL) m.tail[l] = (uint16_t)NIL;
+            if (nexp) atomicAdd(&m.hdr->n_expired, nexp);
+        }
+        cnt_nxt[l] = n;
+        if (c.K == 0) m.ahead[l] = NIL;
+        if (side == 0 && pidx == 0) m.resq[r] = q;
+    }
+    __syncthreads();  // #3 matched lists complete
+
+    // settle trade i of resource r: bid rank i with ask rank i, at the price of the later arrival
+    {
+        int total = 0;
+        for (int r = 0; r < R; ++r) {
+            const int q = m.resq[r];
+            total += q;
+            if (tid < q) {
+                const uint32_t eb = m.mb[r * N4 + tid], ea = m.ma[r * N4 + tid];
+                const uint32_t sb = eb & 0xFFFFu, sa = ea & 0xFFFFu;
+                const int pb = c.prices[eb >> 16], pa = c.prices[ea >> 16];
+                const int ob = (int)(sb >> c.Mp_log2), oa = (int)(sa >> c.Mp_log2);
+                const uint32_t age_b = ((uint32_t)t - (m.pool[sb] >> 16)) & 0xFFFFu;
+                const uint32_t age_a = ((uint32_t)t - (m.pool[sa] >> 16)) & 0xFFFFu;
+                bool bid_later;
+                if (age_b != age_a) bid_later = age_b < age_a;
+                else if (m.key[ob] != m.key[oa]) bid_later = m.key[ob] > m.key[oa];
+                else bid_later = ob > oa;
+                const int pi = bid_later ? pb : pa;
+                const uint32_t bitmask = (1u << c.Mp_log2) - 1u;
+                atomicSub(&m.esc_coin[ob], pb);
+                if (pb - pi) atomicAdd(&m.credit[ob], pb - pi);  // refund of the escrowed excess
+                atomicAdd(&m.inv[r * N4 + ob], 1);
+                atomicAnd(&m.mask[ob], ~(1u << (sb & bitmask)));
+                atomicSub(&m.esc_res[r * N4 + oa], 1);
+                atomicAdd(&m.credit[oa], pi);
+                atomicAdd(&m.sale[oa], pi);
+                atomicAnd(&m.mask[oa], ~(1u << (sa & bitmask)));
+                if (tid == q - 1) m.hdr->last_price[r] = pi;
+            }
+        }
+        if (tid == 0) m.hdr->n_trades += total;
+    }
+    __syncthreads();  // #4 credits complete
+
+    // income from sales (G16), coin credit once per agent
+    if (act) {
+        const int sl = m.sale[tid], cr = m.credit[tid];
+        if (sl > 0) { m.income[tid] = __fadd_rn(m.income[tid], (float)sl); m.sale[tid] = 0; }
+        if (cr > 0) { m.coin[tid] = __fadd_rn(m.coin[tid], (float)cr); m.credit[tid] = 0; }
+    }
+    if (tid >= NPAD - R) write_market_row(c, m, NPAD - 1 - tid, cnt_nxt);
+    if (tid == 0) write_timers(c, m, t + 1);
+
+    // ---------------- P4 tax at period end (G17-G20) ----------------
+    if (boundary) {
+        long long fx = 0;
+        if (act) {
+            const float income = m.income[tid];
+            float tax = 0.0f, lo = 0.0f;
+            for (int b = 0; b < c.B; ++b) {
+                const float hi = (b < c.B - 1) ? c.thresholds[b] : INFINITY;
+                const float top = (income < hi) ? income : hi;
+                float por = __fsub_rn(top, lo);
+                if (por < 0.0f) por = 0.0f;
+                tax = __fadd_rn(tax, __fmul_rn(m.hdr->rates[b], por));
+                lo = hi;
+            }
+            const float coin = m.coin[tid];
+            if (tax > coin) tax = coin;  // G17
+            m.coin[tid] = __fsub_rn(coin, tax);
+            fx = __double2ll_rn((double)tax * 1048576.0);  // G19
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) fx += __shfl_xor_sync(FULL, fx, o);
+        if ((tid & 31) == 0 && fx != 0) atomicAdd(&m.misc[0], (unsigned long long)fx);
+        __syncthreads();
+        if (act) {
+            const float pool = __double2float_rn((double)(long long)m.misc[0] * (1.0 / 1048576.0));
+            const float share = __fdiv_rn(pool, (float)N);  // P:195 "(1/n)"
+            m.coin[tid] = __fadd_rn(m.coin[tid], share);
+            m.income[tid] = 0.0f;
+        }
+        if (tid < c.B) {  // rates of the upcoming period
+            if (gov_lvl < 0 || gov_lvl >= c.L) atomicAdd(&m.hdr->n_bad_gov, 1);
+            else m.hdr->rates[tid] = c.rate_table[gov_lvl];
+        }
+    }
+    if (tid < c.B && (boundary || first)) m.shrow[5 * R + tid] = m.hdr->rates[tid];
+    __syncthreads();  // #5 state final
+    if (tid == 0) {
+        m.hdr->t = t + 1;
+        if (boundary) m.misc[0] = 0ull;
+        if (io.done) io.done[e] = (uint8_t)(t + 1 == c.T);
+    }
+
+    // ---------------- P5 rewards, P6 observations ----------------
+    outputs<NPAD>(c, m, tid, e, 0, first ? 2 : (boundary ? 1 : 0), coin_pre, labor_pre, cf_pre, io.obs, io.rew);
+}
+
+template <int NPAD>
+__global__ void __launch_bounds__(NPAD) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
+                                                       const StepIO io) {
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int e = blockIdx.x, tid = threadIdx.x;
+    const Sm m = carve(c, smem);
+    uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)smem)[i] = blob[i];
+    for (int i = tid; i < (c.o_stage - c.blob_bytes) / 4; i += NPAD) ((uint32_t*)(smem + c.blob_bytes))[i] = 0u;
+    __syncthreads();
+    if (c.K == 0)
+        for (int l = tid; l < c.n_levels; l += NPAD) m.ahead[l] = NIL;
+    if (!io.actions)
+        for (int i = tid; i < c.A; i += NPAD) m.cdf[i] = io.cdf[i];
+    __syncthreads();
+    const size_t EN = (size_t)c.E * c.N, EB = (size_t)c.E * c.B;
+    StepPtrs p;
+    p.actions = io.actions;
+    p.gov_actions = io.gov_actions;
+    int slot = 0;
+    for (int s = 0; s < io.n_steps; ++s) {
+        p.obs = io.obs ? io.obs + (size_t)slot * c.obs_floats : nullptr;
+        p.rew = io.rew ? io.rew + (size_t)slot * (EN + c.E) : nullptr;
+        p.done = io.done ? io.done + (size_t)slot * c.E : nullptr;
+        p.actions_out = io.actions_out ? io.actions_out + slot * EN : nullptr;
+        p.gov_out = io.gov_out ? io.gov_out + slot * EB : nullptr;
+        env_step<NPAD>(c, m, tid, e, p, s == 0);
+        if (p.actions) p.actions += EN;
+        if (p.gov_actions) p.gov_actions += EB;
+        slot = (slot + 1 == io.ring_depth) ? 0 : slot + 1;
+    }
+    __syncthreads();
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)smem)[i];
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+template <int NPAD>
+__global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant__ DevCfg c, const uint8_t* __restrict__ state,
+                                                          float* obs) {
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int e = blockIdx.x, tid = threadIdx.x;
+    const Sm m = carve(c, smem);
+    const uint4* blob = (const uint4*)(state + (size_t)e * c.blob_bytes);
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)smem)[i] = blob[i];
+    __syncthreads();
+    const int t = m.hdr->t;
+    if (tid < c.R) write_market_row(c, m, tid, m.cnt + (t & 1) * c.n_levels);
+    if (tid < c.B) m.shrow[5 * c.R + tid] = m.hdr->rates[tid];
+    if (tid == NPAD - 1) write_timers(c, m, t);
+    __syncthreads();
+    outputs<NPAD>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+}
+
+// Reset (G29, G30): one CTA per env builds the blob in shared memory and stores it.
+template <int NPAD>
+__global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state) {
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int e = blockIdx.x, tid = threadIdx.x;
+    const Sm m = carve(c, smem);
+    for (int i = tid; i < c.blob_bytes / 4; i += NPAD) ((uint32_t*)smem)[i] = 0u;
+    __syncthreads();
+    const uint32_t gid = c.env_id_base + (uint32_t)e;
+    if (tid < c.N) {
+        m.coin[tid] = c.starting_coin;
+        m.cf[tid] = coin_utility(c.starting_coin, 1.0 - (double)c.eta);
+        uint32_t x[4] = {0, 0, 0, 0};
+        for (int d = 0; d <= c.R; ++d) {  // skill draw d: Philox stream 16, "t" field d/4, word d%4
+            if ((d & 3) == 0) philox4x32_10(gid, (uint32_t)tid, (uint32_t)(d >> 2), 16u, c.seed_lo, c.seed_hi, x[0], x[1], x[2], x[3]);
+            const uint32_t w = (d & 3) == 0 ? x[0] : (d & 3) == 1 ? x[1] : (d & 3) == 2 ? x[2] : x[3];
+            float v = u01(w);
+            if (c.skill_init == EJ_SKILL_PARETO_CLIP) {  // Pareto(4) by inversion: 1/sqrt(sqrt(1-u))
+                float rr = __fsqrt_rn(__fsub_rn(1.0f, v));
+                rr = __fsqrt_rn(rr);
+                v = __fdiv_rn(1.0f, rr);
+                if (v < c.clip_lo) v = c.clip_lo;
+                if (v > c.clip_hi) v = c.clip_hi;
+            }
+            if (d < c.R) m.SG[d * c.N4 + tid] = v;
+            else m.SC[tid] = v;
+        }
+    }
+    for (int l = tid; l < c.n_levels; l += NPAD) { m.head[l] = (uint16_t)NIL; m.tail[l] = (uint16_t)NIL; }
+    if (tid == 0) {  // all coins equal: gini = 0, prod = N * coin (exact)
+        const double prod = (double)c.N * (double)c.starting_coin;
+        const double eq = (double)c.omega * (1.0 - 0.0) + (1.0 - (double)c.omega);
+        m.hdr->u_g_prev = eq * prod;
+    }
+    __syncthreads();
+    uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)smem)[i];
+}
+
+}  // namespace
