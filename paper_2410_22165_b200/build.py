@@ -11,6 +11,7 @@ import subprocess
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(_HERE, "csrc", "econojax.cu")
+DEV = os.path.join(_HERE, "csrc", "ej_device.cuh")
 HDR = os.path.join(os.path.dirname(_HERE), "include", "econojax.h")
 LIB = os.path.join(_HERE, "libeconojax.so")
 
@@ -26,7 +27,7 @@ def _nvcc() -> str:
 
 
 def build_lib(force: bool = False, verbose: bool = False) -> str:
-    newest = max(os.path.getmtime(SRC), os.path.getmtime(HDR))
+    newest = max(os.path.getmtime(SRC), os.path.getmtime(DEV), os.path.getmtime(HDR))
     if force or not os.path.exists(LIB) or os.path.getmtime(LIB) < newest:
         tmp = LIB + ".tmp.%d" % os.getpid()
         cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp, SRC]

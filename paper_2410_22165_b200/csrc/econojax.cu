@@ -221,6 +221,8 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     c.n_warps = c.Npad / 32;
     c.shrow_len = 5 * R + c.B + 2;
     c.inv_n = 1.0 / (double)N;
+    c.ua = 1.0 - (double)p->eta;
+    c.inv_ua = 1.0 / c.ua;
     for (int i = 0; i < c.P; ++i) c.prices[i] = p->prices[i];
     for (int i = 0; i + 1 < c.B; ++i) c.thresholds[i] = p->thresholds[i];
     for (int i = 0; i < c.L; ++i) c.rate_table[i] = p->rate_table[i];

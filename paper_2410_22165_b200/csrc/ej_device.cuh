@@ -55,6 +55,7 @@ struct DevCfg {
     float starting_coin, labor_craft, labor_gather, labor_trade, eta, omega, craft_scale;
     float clip_lo, clip_hi, s_coin, s_count, s_price, s_labor;
     double inv_n;  // 1 / N
+    double ua, inv_ua;  // 1 - eta and its reciprocal (Eq.1)
     uint32_t env_id_base, seed_lo, seed_hi;
     // blob section offsets (bytes from the blob base)
     int o_coin, o_labor, o_income, o_SC, o_esc_coin, o_mask, o_cf, o_SG, o_inv, o_esc_res;
@@ -160,8 +161,52 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 
 __device__ __forceinline__ float u01(uint32_t x) { return (float)(x >> 8) * (1.0f / 16777216.0f); }
 
-// Coin term of Eq.1: (C^(1-eta) - 1) / (1-eta), binary64.
-__device__ __forceinline__ double coin_utility(float C, double a) { return (pow((double)C, a) - 1.0) / a; }
+// Coin term of Eq.1: (C^(1-eta) - 1) / (1-eta) in binary64, C >= 0 a binary32 value.
+// C^a = exp(a ln C) with ln m = 2 atanh((m-1)/(m+1)) on m in [sqrt(1/2), sqrt 2) (7 terms:
+// truncation < 5e-13 absolute) and a degree-11 Taylor polynomial of exp on |r| <= ln2 / 2
+// (truncation < 7e-15 relative): relative error of C^a below 1e-12, four orders of magnitude
+// inside what the reward tolerance needs; about 55 instructions, where
+// the library pow() costs ~230.
+__device__ __forceinline__ double coin_utility(float C, double a, double inv_a) {
+    if (C == 0.0f) return -inv_a;  // G36
+    const double x = (double)C;    // exact; normal in binary64 even for a subnormal C
+    int hi = __double2hiint(x);
+    int e = (hi >> 20) - 1023;
+    hi = (hi & 0x000FFFFF) | 0x3FF00000;
+    if (hi >= 0x3FF6A09F) { hi -= 0x00100000; e += 1; }  // m >= ~sqrt 2: halve
+    const double m = __hiloint2double(hi, __double2loint(x));
+    const double d = m + 1.0;
+    double rc = (double)__frcp_rn((float)d);
+    rc = fma(rc, fma(-d, rc, 1.0), rc);  // one Newton step: 1/d to ~4e-15
+    const double s = (m - 1.0) * rc, z = s * s;
+    double q = 1.0 / 13.0;
+    q = fma(q, z, 1.0 / 11.0);
+    q = fma(q, z, 1.0 / 9.0);
+    q = fma(q, z, 1.0 / 7.0);
+    q = fma(q, z, 1.0 / 5.0);
+    q = fma(q, z, 1.0 / 3.0);
+    q = fma(q, z, 1.0);
+    const double lnC = fma((double)e, 0.6931471805599453094, 2.0 * s * q);
+    const double tt = a * lnC;
+    const double nn = rint(tt * 1.4426950408889634074);
+    double r = fma(-nn, 0.693147180369123816490, tt);  // ln2 hi / lo (Cody-Waite)
+    r = fma(-nn, 1.90821492927058770002e-10, r);
+    double y = 1.0 / 39916800.0;
+    y = fma(y, r, 1.0 / 3628800.0);
+    y = fma(y, r, 1.0 / 362880.0);
+    y = fma(y, r, 1.0 / 40320.0);
+    y = fma(y, r, 1.0 / 5040.0);
+    y = fma(y, r, 1.0 / 720.0);
+    y = fma(y, r, 1.0 / 120.0);
+    y = fma(y, r, 1.0 / 24.0);
+    y = fma(y, r, 1.0 / 6.0);
+    y = fma(y, r, 0.5);
+    y = fma(y, r, 1.0);
+    y = fma(y, r, 1.0);
+    const int n = (int)nn;  // |n| <= ~190: the scaled result stays normal
+    y = __hiloint2double(__double2hiint(y) + (n << 20), __double2loint(y));
+    return (y - 1.0) * inv_a;
+}
 
 __device__ __forceinline__ double warp_sum(double v) {
 #pragma unroll
@@ -231,23 +276,47 @@ __device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm& m, int k, 
     m.govrow[3 * k + 2] = __fmul_rn(med, scale);
 }
 
-// One warp computes mean, std, median (Fig.1, G26) of one float metric; for coin
-// also the welfare u_g = eq * prod (Eq.3-5; G22, G23) and the government reward.
-// Sum in binary64; squared deviations in binary32 (non-negative terms: relative error < 1e-6).
+// One warp computes mean, std, median (Fig.1, G26) of metric k (0 coin, 1 labor,
+// 2 income, 3 + r inventory of resource r); for coin also the welfare u_g = eq * prod (Eq.3-5,
+// P:175-188; G22, G23) and the government reward.  Sum in binary64 (integers: exact REDUX sum);
+// squared deviations in binary32 (non-negative terms: relative error < 1e-6).  Median: integer
+// metrics whose values are all below HB use a per-warp shared-memory histogram, everything else
+// the register sorting network.  ONE instance of this code per kernel (the caller loops over k
+// without unrolling): the unrolled network is most of the kernel's instruction footprint.
 //   mode 0 = step, 1 = finished env (reward 0), 2 = observe only
 template <int EPL>
-__device__ __forceinline__ void metric_float(const DevCfg& c, const Sm& m, const float* arr, int lane, int k, int mode, int e,
-                                             float* rew) {
+__device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm& m, int k, int lane, int mode, int e, float* rew,
+                                             int* hist) {
     const int N = c.N;
+    const bool is_int = k >= 3;
+    const float* farr = k == 0 ? m.coin : k == 1 ? m.labor : m.income;
+    const int* iarr = m.inv + (is_int ? k - 3 : 0) * c.N4;
     float x[EPL];
     double s = 0.0;
+    int si = 0, mx = 0;
 #pragma unroll
     for (int q = 0; q < EPL; ++q) {
         const int idx = q * 32 + lane;
-        x[q] = idx < N ? arr[idx] : INFINITY;
-        s += idx < N ? (double)x[q] : 0.0;
+        x[q] = INFINITY;
+        if (idx < N) {
+            if (is_int) {
+                const int v = iarr[idx];
+                x[q] = (float)v;
+                si += v;
+                mx = max(mx, v);
+            } else {
+                x[q] = farr[idx];
+                s += (double)x[q];
+            }
+        }
     }
-    s = warp_sum(s);
+    bool use_hist = false;
+    if (is_int) {
+        s = (double)__reduce_add_sync(FULL, si);
+        use_hist = __reduce_max_sync(FULL, mx) < HB;
+    } else {
+        s = warp_sum(s);
+    }
     const double mean = s * c.inv_n;
     float qs = 0.0f;
 #pragma unroll
@@ -256,64 +325,13 @@ __device__ __forceinline__ void metric_float(const DevCfg& c, const Sm& m, const
         qs = __fadd_rn(qs, __fmul_rn(d, d));
     }
     qs = warp_sum(qs);
-    warp_sort<EPL>(x, lane);
-    const float lo = warp_pick<EPL>(x, N >= 2 ? (N >> 1) - 1 : 0), hi = warp_pick<EPL>(x, N >> 1);
-    if (k == 0 && mode != 2) {
-        // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)  =>  gini * prod = gn / N   (G23)
-        double g = 0.0;
-#pragma unroll
-        for (int q = 0; q < EPL; ++q) {
-            const int idx = q * 32 + lane;
-            g += idx < N ? (double)(2 * idx - N + 1) * (double)x[q] : 0.0;
-        }
-        g = warp_sum(g);
-        if (lane == 0) {
-            // u_g = (omega (1 - gini) + (1 - omega)) prod = prod - omega * gini * prod; gini = 0 when
-            // prod = 0 or N = 1 (then gn = 0 as well)
-            const double ug = s - (double)c.omega * (g * c.inv_n);
-            if (mode == 0) {
-                if (rew) rew[(size_t)e * (N + 1) + N] = (float)(ug - m.hdr->u_g_prev);
-                m.hdr->u_g_prev = ug;
-            } else if (rew) {
-                rew[(size_t)e * (N + 1) + N] = 0.0f;
-            }
-        }
-    }
-    if (lane == 0) gov_triple(c, m, k, mean, qs, lo, hi, k == 1 ? c.s_labor : c.s_coin);
-}
-
-// Same for an integer metric (inventory of one resource): exact integer sum (REDUX), median
-// from a per-warp shared-memory histogram when every value is below HB, else from the sorting
-// network.
-template <int EPL>
-__device__ __forceinline__ void metric_int(const DevCfg& c, const Sm& m, const int* arr, int lane, int k, int* hist) {
-    const int N = c.N;
-    int v[EPL];
-    int s = 0, mx = 0;
-#pragma unroll
-    for (int q = 0; q < EPL; ++q) {
-        const int idx = q * 32 + lane;
-        v[q] = idx < N ? arr[idx] : -1;
-        s += idx < N ? v[q] : 0;
-        mx = max(mx, v[q]);
-    }
-    s = __reduce_add_sync(FULL, s);
-    mx = __reduce_max_sync(FULL, mx);
-    const double mean = (double)s * c.inv_n;
-    float qs = 0.0f;
-#pragma unroll
-    for (int q = 0; q < EPL; ++q) {
-        const float d = v[q] >= 0 ? (float)((double)v[q] - mean) : 0.0f;
-        qs = __fadd_rn(qs, __fmul_rn(d, d));
-    }
-    qs = warp_sum(qs);
     float lo, hi;
-    if (mx < HB) {
+    if (use_hist) {
         ((int4*)hist)[lane] = make_int4(0, 0, 0, 0);
         __syncwarp();
 #pragma unroll
         for (int q = 0; q < EPL; ++q)
-            if (v[q] >= 0) atomicAdd(&hist[v[q]], 1);
+            if (q * 32 + lane < N) atomicAdd(&hist[__float2int_rz(x[q])], 1);
         __syncwarp();
         const int4 h4 = ((int4*)hist)[lane];
         const int c0 = h4.x, c1 = c0 + h4.y, c2 = c1 + h4.z, c3 = c2 + h4.w;
@@ -337,14 +355,32 @@ __device__ __forceinline__ void metric_int(const DevCfg& c, const Sm& m, const i
         lo = (float)vals[0];
         hi = (float)vals[1];
     } else {
-        float x[EPL];
-#pragma unroll
-        for (int q = 0; q < EPL; ++q) x[q] = v[q] >= 0 ? (float)v[q] : INFINITY;
         warp_sort<EPL>(x, lane);
         lo = warp_pick<EPL>(x, N >= 2 ? (N >> 1) - 1 : 0);
         hi = warp_pick<EPL>(x, N >> 1);
+        if (k == 0 && mode != 2) {
+            // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)  =>  gini * prod = gn / N   (G23)
+            double g = 0.0;
+#pragma unroll
+            for (int q = 0; q < EPL; ++q) {
+                const int idx = q * 32 + lane;
+                g += idx < N ? (double)(2 * idx - N + 1) * (double)x[q] : 0.0;
+            }
+            g = warp_sum(g);
+            if (lane == 0) {
+                // u_g = (omega (1 - gini) + (1 - omega)) prod = prod - omega * gini * prod; gini = 0 when
+                // prod = 0 or N = 1 (then gn = 0 as well)
+                const double ug = s - (double)c.omega * (g * c.inv_n);
+                if (mode == 0) {
+                    if (rew) rew[(size_t)e * (N + 1) + N] = (float)(ug - m.hdr->u_g_prev);
+                    m.hdr->u_g_prev = ug;
+                } else if (rew) {
+                    rew[(size_t)e * (N + 1) + N] = 0.0f;
+                }
+            }
+        }
     }
-    if (lane == 0) gov_triple(c, m, k, mean, qs, lo, hi, c.s_count);
+    if (lane == 0) gov_triple(c, m, k, mean, qs, lo, hi, is_int ? c.s_count : k == 1 ? c.s_labor : c.s_coin);
 }
 
 // Shared tail of the population rows: market statistics of the post-step books.
@@ -389,7 +425,7 @@ __device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, 
         if (mode == 0) {
             double cf_post = cf_pre;
             if (__float_as_uint(coin) != __float_as_uint(coin_pre)) {
-                cf_post = coin_utility(coin, 1.0 - (double)c.eta);
+                cf_post = coin_utility(coin, c.ua, c.inv_ua);
                 m.cf[tid] = cf_post;
             }
             if (rew) rew[(size_t)e * (N + 1) + tid] = (float)((cf_post - (double)labor) - (cf_pre - (double)labor_pre));
@@ -417,13 +453,12 @@ __device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, 
         }
     }
 
-    // ---- government statistics: metric k is owned by one warp ----
-#pragma unroll
-    for (int k = 0; k < 3; ++k)
-        if ((k % NW) == warp) metric_float<EPL>(c, m, k == 0 ? m.coin : k == 1 ? m.labor : m.income, lane, k, mode, e, rew);
-    for (int r = 0; r < R; ++r) {
-        const int w = NW - 1 - (r % NW);
-        if (w == warp) metric_int<EPL>(c, m, m.inv + r * N4, lane, 3 + r, m.hist + (r % NW) * HB);
+    // ---- government statistics: metric k is owned by one warp (floats from warp 0 up, integer
+    // metrics from the last warp down) ----
+#pragma unroll 1
+    for (int k = 0; k < c.n_metrics; ++k) {
+        const int w = k < 3 ? k % NW : NW - 1 - ((k - 3) % NW);
+        if (w == warp) metric_stats<EPL>(c, m, k, lane, mode, e, rew, m.hist + (k < 3 ? 0 : (k - 3) % NW) * HB);
     }
     for (int k = tid; k < c.B + 2; k += NPAD) m.govrow[3 * c.n_metrics + k] = m.shrow[5 * R + k];
 
@@ -471,27 +506,15 @@ struct StepPtrs {
     int32_t* gov_out;
 };
 
-// One environment step on the state in shared memory (G1: actions -> match -> expire -> tax ->
-// rewards -> observations -> t++).  `first` = first step of this launch (full observation rows).
+// Phases P1-P4 of one environment step on the state in shared memory (G1: actions -> match ->
+// expire -> tax); returns the pre-step values the rewards need.  `first` = first step of this
+// launch (full observation rows).
 template <int NPAD>
-__device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const StepPtrs& io, bool first) {
+__device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid, int e, const StepPtrs& io, bool first, int t,
+                                          float& coin_pre, float& labor_pre, double& cf_pre, int& rows) {
     const int N = c.N, R = c.R, P = c.P, N4 = c.N4, nl = c.n_levels;
     const bool act = tid < N;
-    const int t = m.hdr->t;
     const uint32_t gid = c.env_id_base + (uint32_t)e;
-    // the previous step's bulk stores must have read the staging tile before it is rewritten
-    if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-
-    if (t >= c.T) {  // G28: finished env
-        if (tid < R) write_market_row(c, m, tid, m.cnt + (t & 1) * nl);
-        if (tid < c.B) m.shrow[5 * R + tid] = m.hdr->rates[tid];
-        if (tid == NPAD - 1) write_timers(c, m, t);
-        __syncthreads();
-        outputs<NPAD>(c, m, tid, e, 1, 2, 0.f, 0.f, 0.0, io.obs, io.rew);
-        if (tid == 0 && io.done) io.done[e] = 1;
-        __syncthreads();
-        return;
-    }
     int* cnt_cur = m.cnt + (t & 1) * nl;
     int* cnt_nxt = m.cnt + ((t & 1) ^ 1) * nl;
 
@@ -529,8 +552,6 @@ __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const Ste
         if (io.gov_out) io.gov_out[(size_t)e * c.B + tid] = gov_lvl;
     }
 
-    float coin_pre = 0.f, labor_pre = 0.f;
-    double cf_pre = 0.0;
     int lvl = -1, grp = 0, pos = 0, price_c = 0, r_c = 0, side_c = 0;
     uint32_t slot = 0, mymask = 0, old_tail = NIL;
     if (act) {
@@ -847,8 +868,34 @@ __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const Ste
         if (io.done) io.done[e] = (uint8_t)(t + 1 == c.T);
     }
 
+    rows = first ? 2 : (boundary ? 1 : 0);
+}
+
+// One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
+// observations.  outputs() has this single call site (instruction footprint).
+template <int NPAD>
+__device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const StepPtrs& io, bool first) {
+    const int t = m.hdr->t;
+    // the previous step's bulk stores must have read the staging tile before it is rewritten
+    if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    float coin_pre = 0.f, labor_pre = 0.f;
+    double cf_pre = 0.0;
+    int mode = 0, rows = 2;
+    if (t >= c.T) {  // G28: finished env
+        if (tid < c.R) write_market_row(c, m, tid, m.cnt + (t & 1) * c.n_levels);
+        if (tid < c.B) m.shrow[5 * c.R + tid] = m.hdr->rates[tid];
+        if (tid == NPAD - 1) write_timers(c, m, t);
+        __syncthreads();
+        mode = 1;
+    } else {
+        step_body<NPAD>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
+    }
     // ---------------- P5 rewards, P6 observations ----------------
-    outputs<NPAD>(c, m, tid, e, 0, first ? 2 : (boundary ? 1 : 0), coin_pre, labor_pre, cf_pre, io.obs, io.rew);
+    outputs<NPAD>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs, io.rew);
+    if (mode == 1) {
+        if (tid == 0 && io.done) io.done[e] = 1;
+        __syncthreads();  // shrow is rewritten at the very start of the next finished step
+    }
 }
 
 template <int NPAD>
@@ -916,7 +963,7 @@ __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ 
     const uint32_t gid = c.env_id_base + (uint32_t)e;
     if (tid < c.N) {
         m.coin[tid] = c.starting_coin;
-        m.cf[tid] = coin_utility(c.starting_coin, 1.0 - (double)c.eta);
+        m.cf[tid] = coin_utility(c.starting_coin, c.ua, c.inv_ua);
         uint32_t x[4] = {0, 0, 0, 0};
         for (int d = 0; d <= c.R; ++d) {  // skill draw d: Philox stream 16, "t" field d/4, word d%4
             if ((d & 3) == 0) philox4x32_10(gid, (uint32_t)tid, (uint32_t)(d >> 2), 16u, c.seed_lo, c.seed_hi, x[0], x[1], x[2], x[3]);
