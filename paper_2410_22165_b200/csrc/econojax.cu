@@ -210,6 +210,7 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     c.base_craft = R; c.base_buy = R + n_craft; c.base_sell = c.base_buy + R * c.P;
     c.A = c.base_sell + R * c.P + c.allow_noop;
     c.n_levels = 2 * R * c.P;
+    c.recipP = (65536 + c.P - 1) / c.P;
     c.n_groups = c.K ? 2 * R : c.n_levels;
     c.D_pop = 6 + 8 * R + c.B;
     c.D_gov = 3 * (3 + R) + c.B + 2;
@@ -478,6 +479,7 @@ int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t*
         const int32_t* w = words + (size_t)k * W;
         size_t q = 0;
         hd->t = w[q++];
+        hd->t_in_period = hd->t % c.period;
         if (w[q] != N || w[q + 1] != R || w[q + 2] != B || w[q + 3] != P || w[q + 4] != cap) return fail(h, EJ_ERR_PARAM, "bad field: %s", "words (shape header mismatch)");
         q += 5;
         if (hd->t < 0 || hd->t > c.T) return fail(h, EJ_ERR_PARAM, "bad field: %s", "words (t)");

@@ -36,9 +36,10 @@ constexpr int HB = 128;                // histogram bins of the integer-metric m
 struct EnvHdr {
     int32_t t;
     int32_t n_trades, n_placed, n_invalid, n_expired, n_bad_gov;
-    int32_t pad0[2];
+    uint32_t med_prev[2];  // bit patterns of the previous lower medians of labor and income (a hint, not state)
     double u_g_prev;
-    double pad1;
+    int32_t t_in_period;  // t % tax_period, kept incrementally (no integer division on the step path)
+    int32_t pad1;
     float rates[EJ_MAX_BRACKETS];
     int32_t last_price[EJ_MAX_RESOURCES];
 };
@@ -47,6 +48,7 @@ static_assert(sizeof(EnvHdr) % 16 == 0, "EnvHdr must keep 16-byte alignment");
 struct DevCfg {
     int E, N, R, P, B, L, M, Mp_log2, K, T, period, expiry;
     int craft_units, craft_distinct, craft_mode, allow_noop, taxes_enabled, skill_init;
+    int recipP;  // ceil(2^16 / P): k / P == (k * recipP) >> 16 for k < 2RP <= 512
     int A, base_craft, base_buy, base_sell, n_levels, n_groups, D_pop, D_gov, D_gov_pad;
     int N4, Npad, n_metrics, n_warps, shrow_len, stage_obs;
     int prices[EJ_MAX_PRICES];
@@ -267,6 +269,65 @@ __device__ __forceinline__ float warp_pick(const float (&x)[EPL], int rank) {
     return __shfl_sync(FULL, v, rank & 31);
 }
 
+// Order statistics r0 <= r1 <= r0 + 1 of the N non-negative values a warp holds (pads = +inf),
+// by walking from a pivot: the previous step's lower median.  With c_lt = #{x < p} and
+// c_le = #{x <= p}, p is the statistic of rank r exactly when c_lt <= r < c_le; otherwise the
+// pivot moves to the next distinct value below (above).  Medians drift by 1-2 distinct values
+// per step on the paper-shaped workloads, so this costs ~100 instructions
+// where the sorting network costs ~450.  Exact for any pivot; gives up (returns false, caller
+// sorts) after WALK_MAX moves or if a value has its sign bit set (keys would not be monotone).
+constexpr int WALK_MAX = 8;
+template <int EPL>
+__device__ __forceinline__ bool walk_select(const float (&x)[EPL], int lane, int N, int r0, int r1, uint32_t* pivot, float& lo,
+                                            float& hi) {
+    uint32_t key[EPL];
+    uint32_t any = 0;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) { key[q] = __float_as_uint(x[q]); any |= key[q]; }
+    if (__reduce_or_sync(FULL, any) & 0x80000000u) return false;
+    uint32_t p = *pivot;
+    int a = 0, b = 0;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) { a += key[q] < p; b += key[q] <= p; }
+    int c_lt = __reduce_add_sync(FULL, a), c_le = __reduce_add_sync(FULL, b);
+    int moves = 0;
+    while (r0 < c_lt) {  // the statistic is below the pivot
+        if (++moves > WALK_MAX) return false;
+        uint32_t mx = 0;
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) mx = max(mx, key[q] < p ? key[q] : 0u);
+        p = __reduce_max_sync(FULL, mx);
+        a = 0;
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) a += key[q] < p;
+        c_le = c_lt;
+        c_lt = __reduce_add_sync(FULL, a);
+    }
+    while (r0 >= c_le) {  // above the pivot
+        if (++moves > WALK_MAX) return false;
+        uint32_t mn = 0xFFFFFFFFu;
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) mn = min(mn, key[q] > p ? key[q] : 0xFFFFFFFFu);
+        p = __reduce_min_sync(FULL, mn);
+        b = 0;
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) b += key[q] <= p;
+        c_lt = c_le;
+        c_le = __reduce_add_sync(FULL, b);
+    }
+    uint32_t p1 = p;
+    if (r1 >= c_le) {
+        uint32_t mn = 0xFFFFFFFFu;
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) mn = min(mn, key[q] > p ? key[q] : 0xFFFFFFFFu);
+        p1 = __reduce_min_sync(FULL, mn);
+    }
+    if (lane == 0) *pivot = p;
+    lo = __uint_as_float(p);
+    hi = __uint_as_float(p1);
+    return true;
+}
+
 __device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm& m, int k, double mean, float q_sum, float lo, float hi,
                                            float scale) {
     const float sd = __fsqrt_rn((float)((double)q_sum * c.inv_n));
@@ -355,9 +416,16 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm& m, int k
         lo = (float)vals[0];
         hi = (float)vals[1];
     } else {
-        warp_sort<EPL>(x, lane);
-        lo = warp_pick<EPL>(x, N >= 2 ? (N >> 1) - 1 : 0);
-        hi = warp_pick<EPL>(x, N >> 1);
+        const int r0 = N >= 2 ? (N >> 1) - 1 : 0, r1 = N >> 1;
+        bool found = false;
+        const bool hinted = k == 1 || k == 2;  // labor, income: med_prev holds last step's lower median
+        if (hinted) found = walk_select<EPL>(x, lane, N, r0, r1, &m.hdr->med_prev[k - 1], lo, hi);
+        if (!found) {
+            warp_sort<EPL>(x, lane);
+            lo = warp_pick<EPL>(x, r0);
+            hi = warp_pick<EPL>(x, r1);
+            if (hinted && lane == 0) m.hdr->med_prev[k - 1] = __float_as_uint(lo);
+        }
         if (k == 0 && mode != 2) {
             // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)  =>  gini * prod = gn / N   (G23)
             double g = 0.0;
@@ -400,8 +468,8 @@ __device__ __forceinline__ void write_market_row(const DevCfg& c, const Sm& m, i
     o[3] = __fmul_rn((float)na, c.s_count);
     o[4] = __fmul_rn((float)m.hdr->last_price[r], c.s_price);
 }
-__device__ __forceinline__ void write_timers(const DevCfg& c, const Sm& m, int tq) {
-    m.shrow[5 * c.R + c.B] = __fdiv_rn((float)(tq % c.period), (float)c.period);
+__device__ __forceinline__ void write_timers(const DevCfg& c, const Sm& m, int tq, int tq_in_period) {
+    m.shrow[5 * c.R + c.B] = __fdiv_rn((float)tq_in_period, (float)c.period);
     m.shrow[5 * c.R + c.B + 1] = __fdiv_rn((float)tq, (float)c.T);
 }
 
@@ -456,9 +524,13 @@ __device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, 
     // ---- government statistics: metric k is owned by one warp (floats from warp 0 up, integer
     // metrics from the last warp down) ----
 #pragma unroll 1
-    for (int k = 0; k < c.n_metrics; ++k) {
-        const int w = k < 3 ? k % NW : NW - 1 - ((k - 3) % NW);
-        if (w == warp) metric_stats<EPL>(c, m, k, lane, mode, e, rew, m.hist + (k < 3 ? 0 : (k - 3) % NW) * HB);
+    for (int it = 0; it < 2; ++it) {
+        // it 0: float metrics k = warp, warp + NW, ... < 3; it 1: integer metrics of resources
+        // r = NW-1-warp, + NW, ... < R.  One instance of metric_stats (instruction footprint).
+        const int first = it == 0 ? warp : 3 + (NW - 1 - warp), last = it == 0 ? 3 : c.n_metrics;
+#pragma unroll 1
+        for (int k = first; k < last; k += NW)
+            metric_stats<EPL>(c, m, k, lane, mode, e, rew, m.hist + (NW - 1 - warp) * HB);
     }
     for (int k = tid; k < c.B + 2; k += NPAD) m.govrow[3 * c.n_metrics + k] = m.shrow[5 * R + k];
 
@@ -493,6 +565,7 @@ __device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, 
             else v = __fmul_rn(m.labor[i], c.s_labor);
             dst[idx] = v;
         }
+        __syncthreads();  // the loop reads other agents' state: the next step must not start updating it
     }
 }
 
@@ -539,7 +612,9 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
     }
     // government levels for the period boundary
     int gov_lvl = -1;
-    const bool boundary = c.taxes_enabled && ((t + 1) % c.period == 0);
+    const int tp = m.hdr->t_in_period;
+    const bool period_end = tp + 1 == c.period;
+    const bool boundary = c.taxes_enabled && period_end;
     if (tid < c.B && (boundary || io.gov_out)) {
         if (io.gov_actions) {
             gov_lvl = io.gov_actions[(size_t)e * c.B + tid];
@@ -602,7 +677,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
         } else if (a < c.base_sell + R * P) {  // market order
             side_c = a >= c.base_sell;
             const int k = a - (side_c ? c.base_sell : c.base_buy);
-            r_c = k / P;
+            r_c = (k * c.recipP) >> 16;
             const int pidx = k - r_c * P;
             price_c = c.prices[pidx];
             bool ok = __popc(mymask) < c.M;
@@ -728,7 +803,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
     // One thread per level.  Trades of a resource: q = max_p min(#bids >= p, #asks <= p); the
     // q best bids and q best asks are popped from the queue heads, then the expired heads.
     for (int l = tid; l < nl; l += NPAD) {
-        const int book = l / P, pidx = l - book * P, r = book >> 1, side = book & 1;
+        const int book = (l * c.recipP) >> 16, pidx = l - book * P, r = book >> 1, side = book & 1;
         const int price = c.prices[pidx];
         const int lb = (r * 2) * P, la = lb + P;
         int totB = 0;
@@ -824,7 +899,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
         if (cr > 0) { m.coin[tid] = __fadd_rn(m.coin[tid], (float)cr); m.credit[tid] = 0; }
     }
     if (tid >= NPAD - R) write_market_row(c, m, NPAD - 1 - tid, cnt_nxt);
-    if (tid == 0) write_timers(c, m, t + 1);
+    if (tid == 0) write_timers(c, m, t + 1, period_end ? 0 : tp + 1);
 
     // ---------------- P4 tax at period end (G17-G20) ----------------
     if (boundary) {
@@ -864,6 +939,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
     __syncthreads();  // #5 state final
     if (tid == 0) {
         m.hdr->t = t + 1;
+        m.hdr->t_in_period = period_end ? 0 : tp + 1;
         if (boundary) m.misc[0] = 0ull;
         if (io.done) io.done[e] = (uint8_t)(t + 1 == c.T);
     }
@@ -884,7 +960,7 @@ __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const Ste
     if (t >= c.T) {  // G28: finished env
         if (tid < c.R) write_market_row(c, m, tid, m.cnt + (t & 1) * c.n_levels);
         if (tid < c.B) m.shrow[5 * c.R + tid] = m.hdr->rates[tid];
-        if (tid == NPAD - 1) write_timers(c, m, t);
+        if (tid == NPAD - 1) write_timers(c, m, t, m.hdr->t_in_period);
         __syncthreads();
         mode = 1;
     } else {
@@ -899,7 +975,7 @@ __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const Ste
 }
 
 template <int NPAD>
-__global__ void __launch_bounds__(NPAD) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
+__global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const StepIO io) {
     extern __shared__ __align__(16) uint8_t smem[];
     const int e = blockIdx.x, tid = threadIdx.x;
@@ -914,20 +990,30 @@ __global__ void __launch_bounds__(NPAD) ej_step_kernel(const __grid_constant__ D
         for (int i = tid; i < c.A; i += NPAD) m.cdf[i] = io.cdf[i];
     __syncthreads();
     const size_t EN = (size_t)c.E * c.N, EB = (size_t)c.E * c.B;
-    StepPtrs p;
+    StepPtrs p;  // running pointers: ring slot `slot` of every output
     p.actions = io.actions;
     p.gov_actions = io.gov_actions;
+    p.obs = io.obs;
+    p.rew = io.rew;
+    p.done = io.done;
+    p.actions_out = io.actions_out;
+    p.gov_out = io.gov_out;
     int slot = 0;
+#pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
-        p.obs = io.obs ? io.obs + (size_t)slot * c.obs_floats : nullptr;
-        p.rew = io.rew ? io.rew + (size_t)slot * (EN + c.E) : nullptr;
-        p.done = io.done ? io.done + (size_t)slot * c.E : nullptr;
-        p.actions_out = io.actions_out ? io.actions_out + slot * EN : nullptr;
-        p.gov_out = io.gov_out ? io.gov_out + slot * EB : nullptr;
         env_step<NPAD>(c, m, tid, e, p, s == 0);
         if (p.actions) p.actions += EN;
         if (p.gov_actions) p.gov_actions += EB;
-        slot = (slot + 1 == io.ring_depth) ? 0 : slot + 1;
+        if (++slot == io.ring_depth) {
+            slot = 0;
+            p.obs = io.obs; p.rew = io.rew; p.done = io.done; p.actions_out = io.actions_out; p.gov_out = io.gov_out;
+        } else {
+            if (p.obs) p.obs += c.obs_floats;
+            if (p.rew) p.rew += EN + c.E;
+            if (p.done) p.done += c.E;
+            if (p.actions_out) p.actions_out += EN;
+            if (p.gov_out) p.gov_out += EB;
+        }
     }
     __syncthreads();
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)smem)[i];
@@ -946,7 +1032,7 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     const int t = m.hdr->t;
     if (tid < c.R) write_market_row(c, m, tid, m.cnt + (t & 1) * c.n_levels);
     if (tid < c.B) m.shrow[5 * c.R + tid] = m.hdr->rates[tid];
-    if (tid == NPAD - 1) write_timers(c, m, t);
+    if (tid == NPAD - 1) write_timers(c, m, t, m.hdr->t_in_period);
     __syncthreads();
     outputs<NPAD>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
