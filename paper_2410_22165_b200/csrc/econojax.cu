@@ -60,59 +60,6 @@ int cuda_fail(ej_env* h, cudaError_t e, const char* where) {
         if (_e != cudaSuccess) return cuda_fail(h, _e, where);   \
     } while (0)
 
-void build_layout(DevCfg& c) {
-    const int N4 = c.N4, R = c.R, nl = c.n_levels;
-    int o = (int)sizeof(EnvHdr);
-    auto take = [&](int bytes) { const int at = o; o = align16(o + bytes); return at; };
-    c.o_coin = take(N4 * 4);
-    c.o_labor = take(N4 * 4);
-    c.o_income = take(N4 * 4);
-    c.o_SC = take(N4 * 4);
-    c.o_esc_coin = take(N4 * 4);
-    c.o_mask = take(N4 * 4);
-    c.o_cf = take(N4 * 8);
-    c.o_SG = take(R * N4 * 4);
-    c.o_inv = take(R * N4 * 4);
-    c.o_esc_res = take(R * N4 * 4);
-    c.o_head = take(nl * 2);
-    c.o_tail = take(nl * 2);
-    c.o_cnt = take(2 * nl * 4);
-    c.o_pool = take((c.N << c.Mp_log2) * 4);
-    c.blob_bytes = o;
-    // scratch (zeroed at kernel start)
-    c.o_key = take(N4 * 4);
-    c.o_cslot = take(N4 * 4);
-    c.o_credit = take(N4 * 4);
-    c.o_sale = take(N4 * 4);
-    c.o_mb = take(R * N4 * 4);
-    c.o_ma = take(R * N4 * 4);
-    if (c.K) {  // book-cap path: compaction buckets
-        c.o_cinfo = take(N4 * 4);
-        c.o_bucket = take(N4 * 8);
-        c.o_sorted = take(N4 * 4);
-        c.o_gcnt = take(c.n_groups * 4);
-        c.o_goff = take(c.n_groups * 4);
-        c.o_anext = c.o_ahead = c.o_cinfo;  // unused
-    } else {  // arrival stacks
-        c.o_anext = take(N4 * 4);
-        c.o_ahead = take(nl * 4);
-        c.o_cinfo = c.o_bucket = c.o_sorted = c.o_gcnt = c.o_goff = c.o_anext;  // unused
-    }
-    c.o_resq = take(EJ_MAX_RESOURCES * 4);
-    c.o_hist = take((R < c.n_warps ? R : c.n_warps) * HB * 4);
-    c.o_shrow = take(c.shrow_len * 4);
-    c.o_govrow = take(c.D_gov_pad * 4);
-    c.o_misc = take(16);
-    c.o_cdf = take(c.A * 4);
-    c.o_stage = o;  // staging tile of the population observation rows (not zeroed)
-    c.stage_obs = 0;
-    if ((c.N * c.D_pop) % 4 == 0 && o + c.N * c.D_pop * 4 <= 100 * 1024) {
-        c.stage_obs = 1;
-        take(c.N * c.D_pop * 4);
-    }
-    c.smem_bytes = o;
-}
-
 template <typename F>
 int for_block_size(int Npad, F&& f) {
     switch (Npad) {
@@ -123,6 +70,66 @@ int for_block_size(int Npad, F&& f) {
         case 512: return f(std::integral_constant<int, 512>());
         default: return f(std::integral_constant<int, 1024>());
     }
+}
+
+// Shared-memory layout: the NP-only sections come from Lay<NP> (compile-time constants shared
+// with the kernels); the R-, P-, M-dependent sections are placed here.
+void build_layout(DevCfg& c) {
+    const int NP = c.Npad, R = c.R, nl = c.n_levels;
+    for_block_size(NP, [&](auto mt) {
+        using L = Lay<decltype(mt)::value>;
+        c.o_key = L::key; c.o_cslot = L::cslot; c.o_anext = L::anext; c.o_cinfo = L::anext; c.o_credit = L::credit;
+        c.o_sale = L::sale; c.o_resq = L::resq; c.o_shrow = L::shrow; c.o_govrow = L::govrow; c.o_misc = L::misc;
+        c.o_blob = L::blob;
+        c.o_coin = L::coin; c.o_labor = L::labor; c.o_income = L::income; c.o_SC = L::SC; c.o_esc_coin = L::esc_coin;
+        c.o_mask = L::mask; c.o_cf = L::cf; c.o_inv = L::inv;
+        return 0;
+    });
+    int o = c.o_inv;  // blob-relative
+    auto take = [&](int bytes) { const int at = o; o = align16(o + bytes); return at; };
+    take(R * NP * 4);
+    c.o_esc_res = take(R * NP * 4);
+    c.o_SG = take(R * NP * 4);
+    c.o_head = take(nl * 2);
+    c.o_tail = take(nl * 2);
+    c.o_cnt = take(2 * nl * 4);
+    c.o_pool = take((c.N << c.Mp_log2) * 4);
+    c.blob_bytes = o;
+    // runtime scratch (absolute offsets; zeroed at kernel start up to the staging tile)
+    o = c.o_blob + c.blob_bytes;
+    c.o_scratch1 = o;
+    c.o_ahead = take(nl * 4);
+    c.o_cdf = take(c.A * 4);
+    if (c.K) {  // book-cap path: compaction buckets
+        c.o_bucket = take(NP * 8);
+        c.o_sorted = take(NP * 4);
+        c.o_gcnt = take(c.n_groups * 4);
+        c.o_goff = take(c.n_groups * 4);
+    } else {
+        c.o_bucket = c.o_sorted = c.o_gcnt = c.o_goff = c.o_ahead;  // unused
+    }
+    // histograms of the integer-metric medians: alias the arrival scratch (key | cslot | anext,
+    // dead once the trades are settled) when they fit
+    const int hist_bytes = (R < c.n_warps ? R : c.n_warps) * HB * 4;
+    c.o_hist = hist_bytes <= 3 * NP * 4 ? c.o_key : take(hist_bytes);
+    // staging tile of the population observation rows (not zeroed); the matched-order lists
+    // mb | ma alias its head (written after the previous step's bulk store has been read,
+    // consumed before the rows are staged)
+    c.o_stage = o;
+    c.stage_obs = 0;
+    const int lists = 2 * R * NP * 4;
+    if ((c.N * c.D_pop) % 4 == 0 && c.N * c.D_pop * 4 >= lists && o + c.N * c.D_pop * 4 <= 100 * 1024) {
+        c.stage_obs = 1;
+        c.stage_alias_bytes = lists;
+        c.o_mb = o;
+        c.o_ma = o + R * NP * 4;
+        take(c.N * c.D_pop * 4);
+    } else {
+        c.o_mb = take(R * NP * 4);
+        c.o_ma = take(R * NP * 4);
+        c.o_stage = o;
+    }
+    c.smem_bytes = o;
 }
 
 int launch_step(ej_env* h, const StepIO& io) {
@@ -215,9 +222,9 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     c.D_pop = 6 + 8 * R + c.B;
     c.D_gov = 3 * (3 + R) + c.B + 2;
     c.D_gov_pad = (c.D_gov + 3) & ~3;
-    c.N4 = (N + 3) & ~3;
     c.Npad = 32;
     while (c.Npad < N) c.Npad <<= 1;
+    c.N4 = c.Npad;  // stride of the per-agent arrays
     c.n_metrics = 3 + R;
     c.n_warps = c.Npad / 32;
     c.shrow_len = 5 * R + c.B + 2;

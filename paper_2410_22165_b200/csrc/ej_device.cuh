@@ -51,6 +51,7 @@ struct DevCfg {
     int recipP;  // ceil(2^16 / P): k / P == (k * recipP) >> 16 for k < 2RP <= 512
     int A, base_craft, base_buy, base_sell, n_levels, n_groups, D_pop, D_gov, D_gov_pad;
     int N4, Npad, n_metrics, n_warps, shrow_len, stage_obs;
+    int stage_alias_bytes;  // head of the staging tile that the matched-order lists overwrite every step
     int prices[EJ_MAX_PRICES];
     float thresholds[EJ_MAX_BRACKETS];
     float rate_table[EJ_MAX_RATE_LEVELS];
@@ -62,6 +63,7 @@ struct DevCfg {
     // blob section offsets (bytes from the blob base)
     int o_coin, o_labor, o_income, o_SC, o_esc_coin, o_mask, o_cf, o_SG, o_inv, o_esc_res;
     int o_head, o_tail, o_cnt, o_pool, blob_bytes;
+    int o_blob, o_scratch1;  // absolute: blob start (= Lay<Npad>::blob), first byte after the blob
     // scratch section offsets (bytes from the shared-memory base; all after the blob)
     int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma, o_bucket, o_sorted;
     int o_gcnt, o_goff, o_resq, o_hist, o_shrow, o_govrow, o_misc, o_cdf, o_stage;
@@ -81,70 +83,85 @@ struct StepIO {
     int n_steps, ring_depth;
 };
 
-struct Sm {
-    EnvHdr* hdr;
-    float *coin, *labor, *income, *SC;
-    int* esc_coin;
-    uint32_t* mask;
-    double* cf;
-    float* SG;
-    int *inv, *esc_res;
-    uint16_t *head, *tail;
-    int* cnt;  // [2][n_levels]: buffer (t & 1) is current
-    uint32_t* pool;
-    uint32_t* key;
-    int* cinfo;
-    uint32_t *cslot, *anext, *ahead;
-    int *credit, *sale;
-    uint32_t *mb, *ma;
-    unsigned long long* bucket;
-    uint32_t* sorted;
-    int *gcnt, *goff, *resq, *hist;
-    float *shrow, *govrow;
-    unsigned long long* misc;  // [0] tax pool in 2^-20 coin
-    uint32_t* cdf;
-    float* stage;
+// Shared-memory layout of one economy.  Everything whose size depends only on the CTA size NP
+// sits at a COMPILE-TIME offset, with per-agent arrays strided by NP: an access is then one
+// LDS/STS [tid*4 + immediate] instead of a rematerialised base pointer (the first version kept
+// ~30 generic pointers in a struct; rebuilding them cost ~10 % of all executed instructions).
+//   [fixed scratch][blob: header | per-agent scalars | inv | esc_res | SG | levels | pool][scratch]
+// Offsets of the R-, P- and M-dependent sections are runtime values in DevCfg (relative to the
+// blob for blob sections, absolute otherwise).  The host reads the same constants (econojax.cu).
+template <int NP>
+struct Lay {
+    // fixed scratch (absolute byte offsets)
+    static constexpr int key = 0;                 // arrival tie keys (Philox x2), u32 [NP]
+    static constexpr int cslot = key + NP * 4;    // pool slot of this step's candidate order
+    static constexpr int anext = cslot + NP * 4;  // arrival stacks: next candidate (K == 0); cinfo (K > 0)
+    static constexpr int credit = anext + NP * 4; // coin credited this step, i32
+    static constexpr int sale = credit + NP * 4;  // sale proceeds this step, i32
+    static constexpr int resq = sale + NP * 4;    // trades per resource, i32 [16]
+    static constexpr int shrow = resq + EJ_MAX_RESOURCES * 4;  // shared tail of the population rows
+    static constexpr int shrow_cap = 5 * EJ_MAX_RESOURCES + EJ_MAX_BRACKETS + 4;
+    static constexpr int govrow = shrow + shrow_cap * 4;
+    static constexpr int govrow_cap = 80;  // >= ceil4(3 (3 + 16) + 16 + 2)
+    static constexpr int misc = govrow + govrow_cap * 4;       // u64 [2]: tax pool
+    static constexpr int blob = misc + 16;
+    // blob sections (byte offsets relative to the blob)
+    static constexpr int coin = (int)sizeof(EnvHdr);
+    static constexpr int labor = coin + NP * 4;
+    static constexpr int income = labor + NP * 4;
+    static constexpr int SC = income + NP * 4;
+    static constexpr int esc_coin = SC + NP * 4;
+    static constexpr int mask = esc_coin + NP * 4;
+    static constexpr int cf = mask + NP * 4;      // cached coin utility, f64 [NP]
+    static constexpr int inv = cf + NP * 8;       // i32 [R][NP]; esc_res and SG follow (runtime offsets)
+    static_assert(blob % 16 == 0 && inv % 16 == 0, "16-byte alignment");
 };
 
-__device__ __forceinline__ Sm carve(const DevCfg& c, uint8_t* s) {
-    Sm m;
-    m.hdr = (EnvHdr*)s;
-    m.coin = (float*)(s + c.o_coin);
-    m.labor = (float*)(s + c.o_labor);
-    m.income = (float*)(s + c.o_income);
-    m.SC = (float*)(s + c.o_SC);
-    m.esc_coin = (int*)(s + c.o_esc_coin);
-    m.mask = (uint32_t*)(s + c.o_mask);
-    m.cf = (double*)(s + c.o_cf);
-    m.SG = (float*)(s + c.o_SG);
-    m.inv = (int*)(s + c.o_inv);
-    m.esc_res = (int*)(s + c.o_esc_res);
-    m.head = (uint16_t*)(s + c.o_head);
-    m.tail = (uint16_t*)(s + c.o_tail);
-    m.cnt = (int*)(s + c.o_cnt);
-    m.pool = (uint32_t*)(s + c.o_pool);
-    m.key = (uint32_t*)(s + c.o_key);
-    m.cinfo = (int*)(s + c.o_cinfo);
-    m.cslot = (uint32_t*)(s + c.o_cslot);
-    m.anext = (uint32_t*)(s + c.o_anext);
-    m.ahead = (uint32_t*)(s + c.o_ahead);
-    m.credit = (int*)(s + c.o_credit);
-    m.sale = (int*)(s + c.o_sale);
-    m.mb = (uint32_t*)(s + c.o_mb);
-    m.ma = (uint32_t*)(s + c.o_ma);
-    m.bucket = (unsigned long long*)(s + c.o_bucket);
-    m.sorted = (uint32_t*)(s + c.o_sorted);
-    m.gcnt = (int*)(s + c.o_gcnt);
-    m.goff = (int*)(s + c.o_goff);
-    m.resq = (int*)(s + c.o_resq);
-    m.hist = (int*)(s + c.o_hist);
-    m.shrow = (float*)(s + c.o_shrow);
-    m.govrow = (float*)(s + c.o_govrow);
-    m.misc = (unsigned long long*)(s + c.o_misc);
-    m.cdf = (uint32_t*)(s + c.o_cdf);
-    m.stage = (float*)(s + c.o_stage);
-    return m;
-}
+template <int NP>
+struct Sm {
+    using L = Lay<NP>;
+    const DevCfg& c;
+    template <class T>
+    __device__ __forceinline__ static T* at(int off) {
+        extern __shared__ __align__(16) uint8_t ej_smem[];
+        return reinterpret_cast<T*>(ej_smem + off);
+    }
+    __device__ __forceinline__ EnvHdr* hdr() const { return at<EnvHdr>(L::blob); }
+    __device__ __forceinline__ float* coin() const { return at<float>(L::blob + L::coin); }
+    __device__ __forceinline__ float* labor() const { return at<float>(L::blob + L::labor); }
+    __device__ __forceinline__ float* income() const { return at<float>(L::blob + L::income); }
+    __device__ __forceinline__ float* SC() const { return at<float>(L::blob + L::SC); }
+    __device__ __forceinline__ int* esc_coin() const { return at<int>(L::blob + L::esc_coin); }
+    __device__ __forceinline__ uint32_t* mask() const { return at<uint32_t>(L::blob + L::mask); }
+    __device__ __forceinline__ double* cf() const { return at<double>(L::blob + L::cf); }
+    __device__ __forceinline__ int* inv() const { return at<int>(L::blob + L::inv); }
+    __device__ __forceinline__ int* esc_res() const { return at<int>(L::blob + c.o_esc_res); }
+    __device__ __forceinline__ float* SG() const { return at<float>(L::blob + c.o_SG); }
+    __device__ __forceinline__ uint16_t* head() const { return at<uint16_t>(L::blob + c.o_head); }
+    __device__ __forceinline__ uint16_t* tail() const { return at<uint16_t>(L::blob + c.o_tail); }
+    __device__ __forceinline__ int* cnt() const { return at<int>(L::blob + c.o_cnt); }  // [2][n_levels]: buffer (t & 1) is current
+    __device__ __forceinline__ uint32_t* pool() const { return at<uint32_t>(L::blob + c.o_pool); }
+    __device__ __forceinline__ uint32_t* key() const { return at<uint32_t>(L::key); }
+    __device__ __forceinline__ uint32_t* cslot() const { return at<uint32_t>(L::cslot); }
+    __device__ __forceinline__ uint32_t* anext() const { return at<uint32_t>(L::anext); }
+    __device__ __forceinline__ int* cinfo() const { return at<int>(L::anext); }
+    __device__ __forceinline__ int* credit() const { return at<int>(L::credit); }
+    __device__ __forceinline__ int* sale() const { return at<int>(L::sale); }
+    __device__ __forceinline__ int* resq() const { return at<int>(L::resq); }
+    __device__ __forceinline__ float* shrow() const { return at<float>(L::shrow); }
+    __device__ __forceinline__ float* govrow() const { return at<float>(L::govrow); }
+    __device__ __forceinline__ unsigned long long* misc() const { return at<unsigned long long>(L::misc); }  // [0] tax pool in 2^-20 coin
+    __device__ __forceinline__ uint32_t* ahead() const { return at<uint32_t>(c.o_ahead); }
+    __device__ __forceinline__ uint32_t* mb() const { return at<uint32_t>(c.o_mb); }
+    __device__ __forceinline__ uint32_t* ma() const { return at<uint32_t>(c.o_ma); }
+    __device__ __forceinline__ unsigned long long* bucket() const { return at<unsigned long long>(c.o_bucket); }
+    __device__ __forceinline__ uint32_t* sorted() const { return at<uint32_t>(c.o_sorted); }
+    __device__ __forceinline__ int* gcnt() const { return at<int>(c.o_gcnt); }
+    __device__ __forceinline__ int* goff() const { return at<int>(c.o_goff); }
+    __device__ __forceinline__ int* hist() const { return at<int>(c.o_hist); }
+    __device__ __forceinline__ uint32_t* cdf() const { return at<uint32_t>(c.o_cdf); }
+    __device__ __forceinline__ float* stage() const { return at<float>(c.o_stage); }
+};
 
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), G30.
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
@@ -328,13 +345,14 @@ __device__ __forceinline__ bool walk_select(const float (&x)[EPL], int lane, int
     return true;
 }
 
-__device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm& m, int k, double mean, float q_sum, float lo, float hi,
+template <int NP>
+__device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm<NP>& m, int k, double mean, float q_sum, float lo, float hi,
                                            float scale) {
     const float sd = __fsqrt_rn((float)((double)q_sum * c.inv_n));
     const float med = (c.N & 1) ? hi : __fmul_rn(0.5f, __fadd_rn(lo, hi));
-    m.govrow[3 * k + 0] = (float)(mean * (double)scale);
-    m.govrow[3 * k + 1] = __fmul_rn(sd, scale);
-    m.govrow[3 * k + 2] = __fmul_rn(med, scale);
+    m.govrow()[3 * k + 0] = (float)(mean * (double)scale);
+    m.govrow()[3 * k + 1] = __fmul_rn(sd, scale);
+    m.govrow()[3 * k + 2] = __fmul_rn(med, scale);
 }
 
 // One warp computes mean, std, median (Fig.1, G26) of metric k (0 coin, 1 labor,
@@ -346,12 +364,12 @@ __device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm& m, int k, 
 // without unrolling): the unrolled network is most of the kernel's instruction footprint.
 //   mode 0 = step, 1 = finished env (reward 0), 2 = observe only
 template <int EPL>
-__device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm& m, int k, int lane, int mode, int e, float* rew,
+__device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<32 * EPL>& m, int k, int lane, int mode, int e, float* rew,
                                              int* hist) {
     const int N = c.N;
     const bool is_int = k >= 3;
-    const float* farr = k == 0 ? m.coin : k == 1 ? m.labor : m.income;
-    const int* iarr = m.inv + (is_int ? k - 3 : 0) * c.N4;
+    const float* farr = k == 0 ? m.coin() : k == 1 ? m.labor() : m.income();
+    const int* iarr = m.inv() + (is_int ? k - 3 : 0) * (32 * EPL);
     float x[EPL];
     double s = 0.0;
     int si = 0, mx = 0;
@@ -419,12 +437,12 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm& m, int k
         const int r0 = N >= 2 ? (N >> 1) - 1 : 0, r1 = N >> 1;
         bool found = false;
         const bool hinted = k == 1 || k == 2;  // labor, income: med_prev holds last step's lower median
-        if (hinted) found = walk_select<EPL>(x, lane, N, r0, r1, &m.hdr->med_prev[k - 1], lo, hi);
+        if (hinted) found = walk_select<EPL>(x, lane, N, r0, r1, &m.hdr()->med_prev[k - 1], lo, hi);
         if (!found) {
             warp_sort<EPL>(x, lane);
             lo = warp_pick<EPL>(x, r0);
             hi = warp_pick<EPL>(x, r1);
-            if (hinted && lane == 0) m.hdr->med_prev[k - 1] = __float_as_uint(lo);
+            if (hinted && lane == 0) m.hdr()->med_prev[k - 1] = __float_as_uint(lo);
         }
         if (k == 0 && mode != 2) {
             // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)  =>  gini * prod = gn / N   (G23)
@@ -440,8 +458,8 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm& m, int k
                 // prod = 0 or N = 1 (then gn = 0 as well)
                 const double ug = s - (double)c.omega * (g * c.inv_n);
                 if (mode == 0) {
-                    if (rew) rew[(size_t)e * (N + 1) + N] = (float)(ug - m.hdr->u_g_prev);
-                    m.hdr->u_g_prev = ug;
+                    if (rew) rew[(size_t)e * (N + 1) + N] = (float)(ug - m.hdr()->u_g_prev);
+                    m.hdr()->u_g_prev = ug;
                 } else if (rew) {
                     rew[(size_t)e * (N + 1) + N] = 0.0f;
                 }
@@ -452,7 +470,8 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm& m, int k
 }
 
 // Shared tail of the population rows: market statistics of the post-step books.
-__device__ __forceinline__ void write_market_row(const DevCfg& c, const Sm& m, int r, const int* cnt) {
+template <int NP>
+__device__ __forceinline__ void write_market_row(const DevCfg& c, const Sm<NP>& m, int r, const int* cnt) {
     int best_bid = 0, best_ask = 0, nb = 0, na = 0;
     for (int p = 0; p < c.P; ++p) {
         const int cb = cnt[(r * 2 + 0) * c.P + p], ca = cnt[(r * 2 + 1) * c.P + p];
@@ -461,40 +480,42 @@ __device__ __forceinline__ void write_market_row(const DevCfg& c, const Sm& m, i
         if (cb > 0) best_bid = c.prices[p];
         if (ca > 0 && best_ask == 0) best_ask = c.prices[p];
     }
-    float* o = m.shrow + r * 5;
+    float* o = m.shrow() + r * 5;
     o[0] = __fmul_rn((float)best_bid, c.s_price);
     o[1] = __fmul_rn((float)best_ask, c.s_price);
     o[2] = __fmul_rn((float)nb, c.s_count);
     o[3] = __fmul_rn((float)na, c.s_count);
-    o[4] = __fmul_rn((float)m.hdr->last_price[r], c.s_price);
+    o[4] = __fmul_rn((float)m.hdr()->last_price[r], c.s_price);
 }
-__device__ __forceinline__ void write_timers(const DevCfg& c, const Sm& m, int tq, int tq_in_period) {
-    m.shrow[5 * c.R + c.B] = __fdiv_rn((float)tq_in_period, (float)c.period);
-    m.shrow[5 * c.R + c.B + 1] = __fdiv_rn((float)tq, (float)c.T);
+template <int NP>
+__device__ __forceinline__ void write_timers(const DevCfg& c, const Sm<NP>& m, int tq, int tq_in_period) {
+    m.shrow()[5 * c.R + c.B] = __fdiv_rn((float)tq_in_period, (float)c.period);
+    m.shrow()[5 * c.R + c.B + 1] = __fdiv_rn((float)tq, (float)c.T);
 }
 
 // Rewards, government statistics and both observation blocks of the state in shared memory.
-// Called after a block barrier that made the state (and m.shrow) final.
+// Called after a block barrier that made the state (and m.shrow()) final.
 //   mode     0 = step, 1 = finished env (rewards 0), 2 = observe only
 //   rows     0 = rewrite only the columns that change every step, 1 = also the tax rates,
 //            2 = every column (first step of a launch: skills)
 template <int NPAD>
-__device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
+__device__ void outputs(const DevCfg& c, const Sm<NPAD>& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
                         double cf_pre, float* obs, float* rew) {
     constexpr int NW = NPAD / 32, EPL = NPAD / 32;
-    const int N = c.N, R = c.R, N4 = c.N4;
+    const int N = c.N, R = c.R;
+    constexpr int N4 = NPAD;  // stride of the per-agent arrays
     const bool act = tid < N;
     const int lane = tid & 31, warp = tid >> 5;
     const bool staged = c.stage_obs && obs;
 
     if (act) {
-        const float coin = m.coin[tid], labor = m.labor[tid];
+        const float coin = m.coin()[tid], labor = m.labor()[tid];
         // ---- population reward: u(post) - u(pre), u = coin term - labor (Eq.1-2) ----
         if (mode == 0) {
             double cf_post = cf_pre;
             if (__float_as_uint(coin) != __float_as_uint(coin_pre)) {
                 cf_post = coin_utility(coin, c.ua, c.inv_ua);
-                m.cf[tid] = cf_post;
+                m.cf()[tid] = cf_post;
             }
             if (rew) rew[(size_t)e * (N + 1) + tid] = (float)((cf_post - (double)labor) - (cf_pre - (double)labor_pre));
         } else if (mode == 1 && rew) {
@@ -502,21 +523,23 @@ __device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, 
         }
         // ---- this agent's observation row (G25) in the staging tile ----
         if (staged) {
-            float* o = m.stage + tid * c.D_pop;
+            float* o = m.stage() + tid * c.D_pop;
             o[0] = __fmul_rn(coin, c.s_coin);
-            for (int r = 0; r < R; ++r) o[1 + r] = __fmul_rn((float)m.inv[r * N4 + tid], c.s_count);
-            o[R + 1] = __fmul_rn((float)m.esc_coin[tid], c.s_coin);
-            for (int r = 0; r < R; ++r) o[R + 2 + r] = __fmul_rn((float)m.esc_res[r * N4 + tid], c.s_count);
+            for (int r = 0; r < R; ++r) o[1 + r] = __fmul_rn((float)m.inv()[r * N4 + tid], c.s_count);
+            o[R + 1] = __fmul_rn((float)m.esc_coin()[tid], c.s_coin);
+            for (int r = 0; r < R; ++r) o[R + 2 + r] = __fmul_rn((float)m.esc_res()[r * N4 + tid], c.s_count);
             o[3 * R + 3] = __fmul_rn(labor, c.s_labor);
             float* tl = o + 3 * R + 4;
-            for (int k = 0; k < 5 * R; ++k) tl[k] = m.shrow[k];
-            tl[5 * R + c.B] = m.shrow[5 * R + c.B];
-            tl[5 * R + c.B + 1] = m.shrow[5 * R + c.B + 1];
-            if (rows >= 1)
-                for (int b = 0; b < c.B; ++b) tl[5 * R + b] = m.shrow[5 * R + b];
-            if (rows >= 2) {
-                for (int r = 0; r < R; ++r) o[2 * R + 2 + r] = m.SG[r * N4 + tid];
-                o[3 * R + 2] = m.SC[tid];
+            for (int k = 0; k < 5 * R; ++k) tl[k] = m.shrow()[k];
+            tl[5 * R + c.B] = m.shrow()[5 * R + c.B];
+            tl[5 * R + c.B + 1] = m.shrow()[5 * R + c.B + 1];
+            // rows whose bytes the matched-order lists reuse are rewritten in full every step
+            const int rows_eff = (tid * c.D_pop * 4 < c.stage_alias_bytes) ? 2 : rows;
+            if (rows_eff >= 1)
+                for (int b = 0; b < c.B; ++b) tl[5 * R + b] = m.shrow()[5 * R + b];
+            if (rows_eff >= 2) {
+                for (int r = 0; r < R; ++r) o[2 * R + 2 + r] = m.SG()[r * N4 + tid];
+                o[3 * R + 2] = m.SC()[tid];
             }
         }
     }
@@ -530,9 +553,9 @@ __device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, 
         const int first = it == 0 ? warp : 3 + (NW - 1 - warp), last = it == 0 ? 3 : c.n_metrics;
 #pragma unroll 1
         for (int k = first; k < last; k += NW)
-            metric_stats<EPL>(c, m, k, lane, mode, e, rew, m.hist + (NW - 1 - warp) * HB);
+            metric_stats<EPL>(c, m, k, lane, mode, e, rew, m.hist() + (NW - 1 - warp) * HB);
     }
-    for (int k = tid; k < c.B + 2; k += NPAD) m.govrow[3 * c.n_metrics + k] = m.shrow[5 * R + k];
+    for (int k = tid; k < c.B + 2; k += NPAD) m.govrow()[3 * c.n_metrics + k] = m.shrow()[5 * R + k];
 
     if (obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
@@ -540,11 +563,11 @@ __device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, 
     if (obs && tid == 0) {  // bulk stores: the env's contiguous [N][D_pop] tile and its government row
         if (staged) {
             float* dst = obs + (size_t)e * N * c.D_pop;
-            const uint32_t src = (uint32_t)__cvta_generic_to_shared(m.stage);
+            const uint32_t src = (uint32_t)__cvta_generic_to_shared(m.stage());
             asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(N * c.D_pop * 4) : "memory");
         }
         float* gdst = obs + c.gov_obs_offset + (size_t)e * c.D_gov_pad;
-        const uint32_t gsrc = (uint32_t)__cvta_generic_to_shared(m.govrow);
+        const uint32_t gsrc = (uint32_t)__cvta_generic_to_shared(m.govrow());
         asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(gsrc), "r"(c.D_gov_pad * 4) : "memory");
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     }
@@ -555,14 +578,14 @@ __device__ void outputs(const DevCfg& c, const Sm& m, int tid, int e, int mode, 
         for (int idx = tid; idx < total; idx += NPAD) {
             const int i = idx / D, k = idx - i * D;
             float v;
-            if (k >= priv) v = m.shrow[k - priv];
-            else if (k == 0) v = __fmul_rn(m.coin[i], c.s_coin);
-            else if (k <= R) v = __fmul_rn((float)m.inv[(k - 1) * N4 + i], c.s_count);
-            else if (k == R + 1) v = __fmul_rn((float)m.esc_coin[i], c.s_coin);
-            else if (k <= 2 * R + 1) v = __fmul_rn((float)m.esc_res[(k - R - 2) * N4 + i], c.s_count);
-            else if (k <= 3 * R + 1) v = m.SG[(k - 2 * R - 2) * N4 + i];
-            else if (k == 3 * R + 2) v = m.SC[i];
-            else v = __fmul_rn(m.labor[i], c.s_labor);
+            if (k >= priv) v = m.shrow()[k - priv];
+            else if (k == 0) v = __fmul_rn(m.coin()[i], c.s_coin);
+            else if (k <= R) v = __fmul_rn((float)m.inv()[(k - 1) * N4 + i], c.s_count);
+            else if (k == R + 1) v = __fmul_rn((float)m.esc_coin()[i], c.s_coin);
+            else if (k <= 2 * R + 1) v = __fmul_rn((float)m.esc_res()[(k - R - 2) * N4 + i], c.s_count);
+            else if (k <= 3 * R + 1) v = m.SG()[(k - 2 * R - 2) * N4 + i];
+            else if (k == 3 * R + 2) v = m.SC()[i];
+            else v = __fmul_rn(m.labor()[i], c.s_labor);
             dst[idx] = v;
         }
         __syncthreads();  // the loop reads other agents' state: the next step must not start updating it
@@ -583,13 +606,14 @@ struct StepPtrs {
 // expire -> tax); returns the pre-step values the rewards need.  `first` = first step of this
 // launch (full observation rows).
 template <int NPAD>
-__device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid, int e, const StepPtrs& io, bool first, int t,
+__device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NPAD>& m, int tid, int e, const StepPtrs& io, bool first, int t,
                                           float& coin_pre, float& labor_pre, double& cf_pre, int& rows) {
-    const int N = c.N, R = c.R, P = c.P, N4 = c.N4, nl = c.n_levels;
+    const int N = c.N, R = c.R, P = c.P, nl = c.n_levels;
+    constexpr int N4 = NPAD;  // stride of the per-agent arrays
     const bool act = tid < N;
     const uint32_t gid = c.env_id_base + (uint32_t)e;
-    int* cnt_cur = m.cnt + (t & 1) * nl;
-    int* cnt_nxt = m.cnt + ((t & 1) ^ 1) * nl;
+    int* cnt_cur = m.cnt() + (t & 1) * nl;
+    int* cnt_nxt = m.cnt() + ((t & 1) ^ 1) * nl;
 
     // ---------------- P1 actions (one action per agent per step) ----------------
     uint32_t x0 = 0, x1 = 0, x2 = 0, x3 = 0;
@@ -602,17 +626,17 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
             int lo = 0, hi = c.A - 1;
             while (lo < hi) {
                 const int mid = (lo + hi) >> 1;
-                if (x0 < m.cdf[mid]) hi = mid;
+                if (x0 < m.cdf()[mid]) hi = mid;
                 else lo = mid + 1;
             }
             a = lo;
         }
         if (io.actions_out) io.actions_out[(size_t)e * N + tid] = a;
-        m.key[tid] = x2;
+        m.key()[tid] = x2;
     }
     // government levels for the period boundary
     int gov_lvl = -1;
-    const int tp = m.hdr->t_in_period;
+    const int tp = m.hdr()->t_in_period;
     const bool period_end = tp + 1 == c.period;
     const bool boundary = c.taxes_enabled && period_end;
     if (tid < c.B && (boundary || io.gov_out)) {
@@ -630,27 +654,27 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
     int lvl = -1, grp = 0, pos = 0, price_c = 0, r_c = 0, side_c = 0;
     uint32_t slot = 0, mymask = 0, old_tail = NIL;
     if (act) {
-        coin_pre = m.coin[tid];
-        labor_pre = m.labor[tid];
-        cf_pre = m.cf[tid];
-        mymask = m.mask[tid];
+        coin_pre = m.coin()[tid];
+        labor_pre = m.labor()[tid];
+        cf_pre = m.cf()[tid];
+        mymask = m.mask()[tid];
         bool invalid = false;
         if (a < 0 || a >= c.A) {
             invalid = true;  // G2
         } else if (a < R) {  // gather: floor(SG + rho), rho = u * 1.1 (G8)
             const float rho = __fmul_rn(u01(x1), 1.1f);
-            const float s = __fadd_rn(m.SG[a * N4 + tid], rho);
-            m.inv[a * N4 + tid] += (int)floorf(s);
-            m.labor[tid] = __fadd_rn(labor_pre, c.labor_gather);
+            const float s = __fadd_rn(m.SG()[a * N4 + tid], rho);
+            m.inv()[a * N4 + tid] += (int)floorf(s);
+            m.labor()[tid] = __fadd_rn(labor_pre, c.labor_gather);
         } else if (a < c.base_buy) {  // craft
             bool ok;
             if (c.craft_mode == EJ_CRAFT_PER_RESOURCE) {
                 const int r = a - R;
-                ok = m.inv[r * N4 + tid] >= c.craft_units;
-                if (ok) m.inv[r * N4 + tid] -= c.craft_units;
+                ok = m.inv()[r * N4 + tid] >= c.craft_units;
+                if (ok) m.inv()[r * N4 + tid] -= c.craft_units;
             } else {
                 int enough = 0;
-                for (int r = 0; r < R; ++r) enough += m.inv[r * N4 + tid] >= c.craft_units;
+                for (int r = 0; r < R; ++r) enough += m.inv()[r * N4 + tid] >= c.craft_units;
                 ok = enough >= c.craft_distinct;
                 if (ok) {  // the R_d most-held resources, ties to the lowest index (G7)
                     uint32_t used = 0;
@@ -658,19 +682,19 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
                         int best = -1, bestv = 0;
                         for (int r = 0; r < R; ++r) {
                             if ((used >> r) & 1u) continue;
-                            const int v = m.inv[r * N4 + tid];
+                            const int v = m.inv()[r * N4 + tid];
                             if (best < 0 || v > bestv) { best = r; bestv = v; }
                         }
                         used |= 1u << best;
-                        m.inv[best * N4 + tid] = bestv - c.craft_units;
+                        m.inv()[best * N4 + tid] = bestv - c.craft_units;
                     }
                 }
             }
             if (ok) {
-                const float pay = __fmul_rn(m.SC[tid], c.craft_scale);
-                m.coin[tid] = __fadd_rn(coin_pre, pay);
-                m.income[tid] = __fadd_rn(m.income[tid], pay);
-                m.labor[tid] = __fadd_rn(labor_pre, c.labor_craft);
+                const float pay = __fmul_rn(m.SC()[tid], c.craft_scale);
+                m.coin()[tid] = __fadd_rn(coin_pre, pay);
+                m.income()[tid] = __fadd_rn(m.income()[tid], pay);
+                m.labor()[tid] = __fadd_rn(labor_pre, c.labor_craft);
             } else {
                 invalid = true;
             }
@@ -682,24 +706,24 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
             price_c = c.prices[pidx];
             bool ok = __popc(mymask) < c.M;
             if (side_c == 0) ok = ok && (coin_pre >= (float)price_c);
-            else ok = ok && (m.inv[r_c * N4 + tid] >= 1);
+            else ok = ok && (m.inv()[r_c * N4 + tid] >= 1);
             if (ok) {
                 lvl = (r_c * 2 + side_c) * P + pidx;
                 slot = ((uint32_t)tid << c.Mp_log2) + (uint32_t)(__ffs(~mymask) - 1);
-                m.cslot[tid] = slot;
-                old_tail = m.tail[lvl];  // read before anyone links (tails change after barrier #1)
+                m.cslot()[tid] = slot;
+                old_tail = m.tail()[lvl];  // read before anyone links (tails change after barrier #1)
                 if (c.K) {
                     grp = r_c * 2 + side_c;
-                    pos = atomicAdd(&m.gcnt[grp], 1);
-                    m.cinfo[tid] = lvl;
+                    pos = atomicAdd(&m.gcnt()[grp], 1);
+                    m.cinfo()[tid] = lvl;
                 } else {  // push on the level's arrival stack
-                    m.anext[tid] = atomicExch(&m.ahead[lvl], (uint32_t)tid);
+                    m.anext()[tid] = atomicExch(&m.ahead()[lvl], (uint32_t)tid);
                 }
             } else {
                 invalid = true;
             }
         }  // else NO-OP
-        if (invalid) atomicAdd(&m.hdr->n_invalid, 1);
+        if (invalid) atomicAdd(&m.hdr()->n_invalid, 1);
     }
     __syncthreads();  // #1 arrivals registered
 
@@ -713,17 +737,17 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
         if (lvl >= 0) {
             int succ = -1;
             uint32_t sk = 0;
-            uint32_t j = m.ahead[lvl];
+            uint32_t j = m.ahead()[lvl];
             while (j != NIL) {
                 if ((int)j != tid) {
-                    const uint32_t kj = m.key[j];
+                    const uint32_t kj = m.key()[j];
                     const bool later = (kj > x2) || (kj == x2 && (int)j > tid);
                     if (!later) ++lrank;
                     else if (succ < 0 || kj < sk || (kj == sk && (int)j < succ)) { succ = (int)j; sk = kj; }
                 }
-                j = m.anext[j];
+                j = m.anext()[j];
             }
-            if (succ >= 0) nxt = m.cslot[succ];
+            if (succ >= 0) nxt = m.cslot()[succ];
             accepted = true;
         }
     } else {
@@ -732,29 +756,29 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
             int carry = 0;
             for (int base = 0; base < c.n_groups; base += 32) {
                 const int g = base + tid;
-                const int v = g < c.n_groups ? m.gcnt[g] : 0;
+                const int v = g < c.n_groups ? m.gcnt()[g] : 0;
                 int incl = v;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) {
                     const int y = __shfl_up_sync(FULL, incl, o);
                     if (tid >= o) incl += y;
                 }
-                if (g < c.n_groups) m.goff[g] = carry + incl - v;
+                if (g < c.n_groups) m.goff()[g] = carry + incl - v;
                 carry += __shfl_sync(FULL, incl, 31);
             }
         }
         __syncthreads();
         const unsigned long long mine = ((unsigned long long)x2 << 32) | (unsigned long long)tid;
-        if (lvl >= 0) m.bucket[m.goff[grp] + pos] = mine;
+        if (lvl >= 0) m.bucket()[m.goff()[grp] + pos] = mine;
         __syncthreads();
         int before = 0, gbase = 0, gn = 0;
         if (lvl >= 0) {
-            gbase = m.goff[grp];
-            gn = m.gcnt[grp];
+            gbase = m.goff()[grp];
+            gn = m.gcnt()[grp];
             int brank = 0;
             for (int k = 0; k < gn; ++k) {
-                const unsigned long long o = m.bucket[gbase + k];
-                const int lj = m.cinfo[(int)(o & 0xFFFFFFFFu)];
+                const unsigned long long o = m.bucket()[gbase + k];
+                const int lj = m.cinfo()[(int)(o & 0xFFFFFFFFu)];
                 const bool earlier = o < mine, same = lj == lvl;
                 brank += earlier;
                 lrank += same && earlier;
@@ -763,38 +787,38 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
             int n_rest = 0;
             for (int p = 0; p < P; ++p) n_rest += cnt_cur[grp * P + p];
             accepted = n_rest + brank < c.K;
-            m.sorted[gbase + before] = (uint32_t)tid | (accepted ? 0x10000u : 0u);
+            m.sorted()[gbase + before] = (uint32_t)tid | (accepted ? 0x10000u : 0u);
         }
         __syncthreads();
         if (lvl >= 0 && accepted && before + 1 < gn) {
-            const uint32_t s = m.sorted[gbase + before + 1];
+            const uint32_t s = m.sorted()[gbase + before + 1];
             const int j = (int)(s & 0xFFFFu);
-            if ((s & 0x10000u) && m.cinfo[j] == lvl) nxt = m.cslot[j];
+            if ((s & 0x10000u) && m.cinfo()[j] == lvl) nxt = m.cslot()[j];
         }
-        for (int g = tid; g < c.n_groups; g += NPAD) m.gcnt[g] = 0;  // ready for the next step
+        for (int g = tid; g < c.n_groups; g += NPAD) m.gcnt()[g] = 0;  // ready for the next step
     }
 
     if (lvl >= 0) {
         if (accepted) {
-            m.pool[slot] = nxt | (((uint32_t)t & 0xFFFFu) << 16);
+            m.pool()[slot] = nxt | (((uint32_t)t & 0xFFFFu) << 16);
             if (lrank == 0) {
-                if (old_tail != NIL) m.pool[old_tail] = (m.pool[old_tail] & 0xFFFF0000u) | slot;
-                else m.head[lvl] = (uint16_t)slot;
+                if (old_tail != NIL) m.pool()[old_tail] = (m.pool()[old_tail] & 0xFFFF0000u) | slot;
+                else m.head()[lvl] = (uint16_t)slot;
             }
-            if (nxt == NIL) m.tail[lvl] = (uint16_t)slot;
+            if (nxt == NIL) m.tail()[lvl] = (uint16_t)slot;
             atomicAdd(&cnt_cur[lvl], 1);
-            m.mask[tid] = mymask | (1u << (slot & ((1u << c.Mp_log2) - 1u)));
+            m.mask()[tid] = mymask | (1u << (slot & ((1u << c.Mp_log2) - 1u)));
             if (side_c == 0) {  // escrow
-                m.coin[tid] = __fsub_rn(coin_pre, (float)price_c);
-                m.esc_coin[tid] += price_c;
+                m.coin()[tid] = __fsub_rn(coin_pre, (float)price_c);
+                m.esc_coin()[tid] += price_c;
             } else {
-                m.inv[r_c * N4 + tid] -= 1;
-                m.esc_res[r_c * N4 + tid] += 1;
+                m.inv()[r_c * N4 + tid] -= 1;
+                m.esc_res()[r_c * N4 + tid] += 1;
             }
-            m.labor[tid] = __fadd_rn(labor_pre, c.labor_trade);
-            atomicAdd(&m.hdr->n_placed, 1);
+            m.labor()[tid] = __fadd_rn(labor_pre, c.labor_trade);
+            atomicAdd(&m.hdr()->n_placed, 1);
         } else {
-            atomicAdd(&m.hdr->n_invalid, 1);
+            atomicAdd(&m.hdr()->n_invalid, 1);
         }
     }
     __syncthreads();  // #2 books hold this step's arrivals
@@ -820,41 +844,41 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
         const int better = side ? alt_me : bgt_me;  // orders ahead of this level on its side
         int n = cnt_cur[l];
         const int tk = max(0, min(n, q - better));
-        uint32_t h = m.head[l];
+        uint32_t h = m.head()[l];
         if (tk > 0) {
-            uint32_t* dst = (side ? m.ma : m.mb) + r * N4 + better;
+            uint32_t* dst = (side ? m.ma() : m.mb()) + r * N4 + better;
             for (int k = 0; k < tk; ++k) {
                 dst[k] = h | ((uint32_t)pidx << 16);
-                h = m.pool[h] & 0xFFFFu;
+                h = m.pool()[h] & 0xFFFFu;
             }
             n -= tk;
         }
         int nexp = 0;
         while (h != NIL) {
-            const uint32_t pe = m.pool[h];
+            const uint32_t pe = m.pool()[h];
             const uint32_t age = ((uint32_t)t - (pe >> 16)) & 0xFFFFu;
             if ((int)age < c.expiry) break;
             const int owner = (int)(h >> c.Mp_log2);
             if (side == 0) {
-                atomicSub(&m.esc_coin[owner], price);
-                atomicAdd(&m.credit[owner], price);
+                atomicSub(&m.esc_coin()[owner], price);
+                atomicAdd(&m.credit()[owner], price);
             } else {
-                atomicSub(&m.esc_res[r * N4 + owner], 1);
-                atomicAdd(&m.inv[r * N4 + owner], 1);
+                atomicSub(&m.esc_res()[r * N4 + owner], 1);
+                atomicAdd(&m.inv()[r * N4 + owner], 1);
             }
-            atomicAnd(&m.mask[owner], ~(1u << (h & ((1u << c.Mp_log2) - 1u))));
+            atomicAnd(&m.mask()[owner], ~(1u << (h & ((1u << c.Mp_log2) - 1u))));
             ++nexp;
             --n;
             h = pe & 0xFFFFu;
         }
         if (tk > 0 || nexp > 0) {
-            m.head[l] = (uint16_t)h;
-            if (h == NIL) m.tail[l] = (uint16_t)NIL;
-            if (nexp) atomicAdd(&m.hdr->n_expired, nexp);
+            m.head()[l] = (uint16_t)h;
+            if (h == NIL) m.tail()[l] = (uint16_t)NIL;
+            if (nexp) atomicAdd(&m.hdr()->n_expired, nexp);
         }
         cnt_nxt[l] = n;
-        if (c.K == 0) m.ahead[l] = NIL;
-        if (side == 0 && pidx == 0) m.resq[r] = q;
+        if (c.K == 0) m.ahead()[l] = NIL;
+        if (side == 0 && pidx == 0) m.resq()[r] = q;
     }
     __syncthreads();  // #3 matched lists complete
 
@@ -862,41 +886,41 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
     {
         int total = 0;
         for (int r = 0; r < R; ++r) {
-            const int q = m.resq[r];
+            const int q = m.resq()[r];
             total += q;
             if (tid < q) {
-                const uint32_t eb = m.mb[r * N4 + tid], ea = m.ma[r * N4 + tid];
+                const uint32_t eb = m.mb()[r * N4 + tid], ea = m.ma()[r * N4 + tid];
                 const uint32_t sb = eb & 0xFFFFu, sa = ea & 0xFFFFu;
                 const int pb = c.prices[eb >> 16], pa = c.prices[ea >> 16];
                 const int ob = (int)(sb >> c.Mp_log2), oa = (int)(sa >> c.Mp_log2);
-                const uint32_t age_b = ((uint32_t)t - (m.pool[sb] >> 16)) & 0xFFFFu;
-                const uint32_t age_a = ((uint32_t)t - (m.pool[sa] >> 16)) & 0xFFFFu;
+                const uint32_t age_b = ((uint32_t)t - (m.pool()[sb] >> 16)) & 0xFFFFu;
+                const uint32_t age_a = ((uint32_t)t - (m.pool()[sa] >> 16)) & 0xFFFFu;
                 bool bid_later;
                 if (age_b != age_a) bid_later = age_b < age_a;
-                else if (m.key[ob] != m.key[oa]) bid_later = m.key[ob] > m.key[oa];
+                else if (m.key()[ob] != m.key()[oa]) bid_later = m.key()[ob] > m.key()[oa];
                 else bid_later = ob > oa;
                 const int pi = bid_later ? pb : pa;
                 const uint32_t bitmask = (1u << c.Mp_log2) - 1u;
-                atomicSub(&m.esc_coin[ob], pb);
-                if (pb - pi) atomicAdd(&m.credit[ob], pb - pi);  // refund of the escrowed excess
-                atomicAdd(&m.inv[r * N4 + ob], 1);
-                atomicAnd(&m.mask[ob], ~(1u << (sb & bitmask)));
-                atomicSub(&m.esc_res[r * N4 + oa], 1);
-                atomicAdd(&m.credit[oa], pi);
-                atomicAdd(&m.sale[oa], pi);
-                atomicAnd(&m.mask[oa], ~(1u << (sa & bitmask)));
-                if (tid == q - 1) m.hdr->last_price[r] = pi;
+                atomicSub(&m.esc_coin()[ob], pb);
+                if (pb - pi) atomicAdd(&m.credit()[ob], pb - pi);  // refund of the escrowed excess
+                atomicAdd(&m.inv()[r * N4 + ob], 1);
+                atomicAnd(&m.mask()[ob], ~(1u << (sb & bitmask)));
+                atomicSub(&m.esc_res()[r * N4 + oa], 1);
+                atomicAdd(&m.credit()[oa], pi);
+                atomicAdd(&m.sale()[oa], pi);
+                atomicAnd(&m.mask()[oa], ~(1u << (sa & bitmask)));
+                if (tid == q - 1) m.hdr()->last_price[r] = pi;
             }
         }
-        if (tid == 0) m.hdr->n_trades += total;
+        if (tid == 0) m.hdr()->n_trades += total;
     }
     __syncthreads();  // #4 credits complete
 
     // income from sales (G16), coin credit once per agent
     if (act) {
-        const int sl = m.sale[tid], cr = m.credit[tid];
-        if (sl > 0) { m.income[tid] = __fadd_rn(m.income[tid], (float)sl); m.sale[tid] = 0; }
-        if (cr > 0) { m.coin[tid] = __fadd_rn(m.coin[tid], (float)cr); m.credit[tid] = 0; }
+        const int sl = m.sale()[tid], cr = m.credit()[tid];
+        if (sl > 0) { m.income()[tid] = __fadd_rn(m.income()[tid], (float)sl); m.sale()[tid] = 0; }
+        if (cr > 0) { m.coin()[tid] = __fadd_rn(m.coin()[tid], (float)cr); m.credit()[tid] = 0; }
     }
     if (tid >= NPAD - R) write_market_row(c, m, NPAD - 1 - tid, cnt_nxt);
     if (tid == 0) write_timers(c, m, t + 1, period_end ? 0 : tp + 1);
@@ -905,42 +929,42 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
     if (boundary) {
         long long fx = 0;
         if (act) {
-            const float income = m.income[tid];
+            const float income = m.income()[tid];
             float tax = 0.0f, lo = 0.0f;
             for (int b = 0; b < c.B; ++b) {
                 const float hi = (b < c.B - 1) ? c.thresholds[b] : INFINITY;
                 const float top = (income < hi) ? income : hi;
                 float por = __fsub_rn(top, lo);
                 if (por < 0.0f) por = 0.0f;
-                tax = __fadd_rn(tax, __fmul_rn(m.hdr->rates[b], por));
+                tax = __fadd_rn(tax, __fmul_rn(m.hdr()->rates[b], por));
                 lo = hi;
             }
-            const float coin = m.coin[tid];
+            const float coin = m.coin()[tid];
             if (tax > coin) tax = coin;  // G17
-            m.coin[tid] = __fsub_rn(coin, tax);
+            m.coin()[tid] = __fsub_rn(coin, tax);
             fx = __double2ll_rn((double)tax * 1048576.0);  // G19
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) fx += __shfl_xor_sync(FULL, fx, o);
-        if ((tid & 31) == 0 && fx != 0) atomicAdd(&m.misc[0], (unsigned long long)fx);
+        if ((tid & 31) == 0 && fx != 0) atomicAdd(&m.misc()[0], (unsigned long long)fx);
         __syncthreads();
         if (act) {
-            const float pool = __double2float_rn((double)(long long)m.misc[0] * (1.0 / 1048576.0));
+            const float pool = __double2float_rn((double)(long long)m.misc()[0] * (1.0 / 1048576.0));
             const float share = __fdiv_rn(pool, (float)N);  // P:195 "(1/n)"
-            m.coin[tid] = __fadd_rn(m.coin[tid], share);
-            m.income[tid] = 0.0f;
+            m.coin()[tid] = __fadd_rn(m.coin()[tid], share);
+            m.income()[tid] = 0.0f;
         }
         if (tid < c.B) {  // rates of the upcoming period
-            if (gov_lvl < 0 || gov_lvl >= c.L) atomicAdd(&m.hdr->n_bad_gov, 1);
-            else m.hdr->rates[tid] = c.rate_table[gov_lvl];
+            if (gov_lvl < 0 || gov_lvl >= c.L) atomicAdd(&m.hdr()->n_bad_gov, 1);
+            else m.hdr()->rates[tid] = c.rate_table[gov_lvl];
         }
     }
-    if (tid < c.B && (boundary || first)) m.shrow[5 * R + tid] = m.hdr->rates[tid];
+    if (tid < c.B && (boundary || first)) m.shrow()[5 * R + tid] = m.hdr()->rates[tid];
     __syncthreads();  // #5 state final
     if (tid == 0) {
-        m.hdr->t = t + 1;
-        m.hdr->t_in_period = period_end ? 0 : tp + 1;
-        if (boundary) m.misc[0] = 0ull;
+        m.hdr()->t = t + 1;
+        m.hdr()->t_in_period = period_end ? 0 : tp + 1;
+        if (boundary) m.misc()[0] = 0ull;
         if (io.done) io.done[e] = (uint8_t)(t + 1 == c.T);
     }
 
@@ -950,17 +974,17 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm& m, int tid,
 // One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
 // observations.  outputs() has this single call site (instruction footprint).
 template <int NPAD>
-__device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const StepPtrs& io, bool first) {
-    const int t = m.hdr->t;
+__device__ void env_step(const DevCfg& c, const Sm<NPAD>& m, int tid, int e, const StepPtrs& io, bool first) {
+    const int t = m.hdr()->t;
     // the previous step's bulk stores must have read the staging tile before it is rewritten
     if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     float coin_pre = 0.f, labor_pre = 0.f;
     double cf_pre = 0.0;
     int mode = 0, rows = 2;
     if (t >= c.T) {  // G28: finished env
-        if (tid < c.R) write_market_row(c, m, tid, m.cnt + (t & 1) * c.n_levels);
-        if (tid < c.B) m.shrow[5 * c.R + tid] = m.hdr->rates[tid];
-        if (tid == NPAD - 1) write_timers(c, m, t, m.hdr->t_in_period);
+        if (tid < c.R) write_market_row(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
+        if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
+        if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
         __syncthreads();
         mode = 1;
     } else {
@@ -977,17 +1001,19 @@ __device__ void env_step(const DevCfg& c, const Sm& m, int tid, int e, const Ste
 template <int NPAD>
 __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const StepIO io) {
-    extern __shared__ __align__(16) uint8_t smem[];
+    extern __shared__ __align__(16) uint8_t ej_smem[];
+    uint8_t* const sblob = ej_smem + Lay<NPAD>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
-    const Sm m = carve(c, smem);
+    const Sm<NPAD> m{c};
     uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
-    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)smem)[i] = blob[i];
-    for (int i = tid; i < (c.o_stage - c.blob_bytes) / 4; i += NPAD) ((uint32_t*)(smem + c.blob_bytes))[i] = 0u;
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
+    for (int i = tid; i < Lay<NPAD>::blob / 16; i += NPAD) ((uint4*)ej_smem)[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (int i = tid; i < (c.o_stage - c.o_scratch1) / 16; i += NPAD) ((uint4*)(ej_smem + c.o_scratch1))[i] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
     if (c.K == 0)
-        for (int l = tid; l < c.n_levels; l += NPAD) m.ahead[l] = NIL;
+        for (int l = tid; l < c.n_levels; l += NPAD) m.ahead()[l] = NIL;
     if (!io.actions)
-        for (int i = tid; i < c.A; i += NPAD) m.cdf[i] = io.cdf[i];
+        for (int i = tid; i < c.A; i += NPAD) m.cdf()[i] = io.cdf[i];
     __syncthreads();
     const size_t EN = (size_t)c.E * c.N, EB = (size_t)c.E * c.B;
     StepPtrs p;  // running pointers: ring slot `slot` of every output
@@ -1016,23 +1042,24 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
         }
     }
     __syncthreads();
-    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)smem)[i];
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)sblob)[i];
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 template <int NPAD>
 __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant__ DevCfg c, const uint8_t* __restrict__ state,
                                                           float* obs) {
-    extern __shared__ __align__(16) uint8_t smem[];
+    extern __shared__ __align__(16) uint8_t ej_smem[];
+    uint8_t* const sblob = ej_smem + Lay<NPAD>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
-    const Sm m = carve(c, smem);
+    const Sm<NPAD> m{c};
     const uint4* blob = (const uint4*)(state + (size_t)e * c.blob_bytes);
-    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)smem)[i] = blob[i];
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
     __syncthreads();
-    const int t = m.hdr->t;
-    if (tid < c.R) write_market_row(c, m, tid, m.cnt + (t & 1) * c.n_levels);
-    if (tid < c.B) m.shrow[5 * c.R + tid] = m.hdr->rates[tid];
-    if (tid == NPAD - 1) write_timers(c, m, t, m.hdr->t_in_period);
+    const int t = m.hdr()->t;
+    if (tid < c.R) write_market_row(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
+    if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
+    if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
     __syncthreads();
     outputs<NPAD>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
@@ -1041,15 +1068,16 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
 // Reset (G29, G30): one CTA per env builds the blob in shared memory and stores it.
 template <int NPAD>
 __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state) {
-    extern __shared__ __align__(16) uint8_t smem[];
+    extern __shared__ __align__(16) uint8_t ej_smem[];
+    uint8_t* const sblob = ej_smem + Lay<NPAD>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
-    const Sm m = carve(c, smem);
-    for (int i = tid; i < c.blob_bytes / 4; i += NPAD) ((uint32_t*)smem)[i] = 0u;
+    const Sm<NPAD> m{c};
+    for (int i = tid; i < c.blob_bytes / 4; i += NPAD) ((uint32_t*)sblob)[i] = 0u;
     __syncthreads();
     const uint32_t gid = c.env_id_base + (uint32_t)e;
     if (tid < c.N) {
-        m.coin[tid] = c.starting_coin;
-        m.cf[tid] = coin_utility(c.starting_coin, c.ua, c.inv_ua);
+        m.coin()[tid] = c.starting_coin;
+        m.cf()[tid] = coin_utility(c.starting_coin, c.ua, c.inv_ua);
         uint32_t x[4] = {0, 0, 0, 0};
         for (int d = 0; d <= c.R; ++d) {  // skill draw d: Philox stream 16, "t" field d/4, word d%4
             if ((d & 3) == 0) philox4x32_10(gid, (uint32_t)tid, (uint32_t)(d >> 2), 16u, c.seed_lo, c.seed_hi, x[0], x[1], x[2], x[3]);
@@ -1062,19 +1090,19 @@ __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ 
                 if (v < c.clip_lo) v = c.clip_lo;
                 if (v > c.clip_hi) v = c.clip_hi;
             }
-            if (d < c.R) m.SG[d * c.N4 + tid] = v;
-            else m.SC[tid] = v;
+            if (d < c.R) m.SG()[d * NPAD + tid] = v;
+            else m.SC()[tid] = v;
         }
     }
-    for (int l = tid; l < c.n_levels; l += NPAD) { m.head[l] = (uint16_t)NIL; m.tail[l] = (uint16_t)NIL; }
+    for (int l = tid; l < c.n_levels; l += NPAD) { m.head()[l] = (uint16_t)NIL; m.tail()[l] = (uint16_t)NIL; }
     if (tid == 0) {  // all coins equal: gini = 0, prod = N * coin (exact)
         const double prod = (double)c.N * (double)c.starting_coin;
         const double eq = (double)c.omega * (1.0 - 0.0) + (1.0 - (double)c.omega);
-        m.hdr->u_g_prev = eq * prod;
+        m.hdr()->u_g_prev = eq * prod;
     }
     __syncthreads();
     uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
-    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)smem)[i];
+    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)sblob)[i];
 }
 
 }  // namespace
