@@ -330,7 +330,10 @@ def main():
     if os.path.exists(traffic_path):
         try:
             with open(traffic_path) as f:
-                line["roofline"]["traffic"] = json.load(f).get(name)
+                tr = json.load(f).get(name)
+            if tr:  # ncu-measured DRAM bytes per env-step x env-steps per launch (per launch, like `achieved`)
+                line["roofline"]["traffic"] = tr["bytes_per_env_step"] * E * K / max(1, launches)
+                line["roofline"]["traffic_source"] = tr["source"]
         except Exception:
             pass
     if world == 1 and not args.no_cpu_baseline:
