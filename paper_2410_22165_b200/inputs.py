@@ -153,3 +153,35 @@ def action_stream(cfg: dict, steps: int, seed: int | None = None, E: int | None 
     B = len(p["thresholds"]) + 1
     gov = rng.integers(0, len(p["rate_table"]), size=(steps, E, B), dtype=np.int32)
     return acts, gov
+
+
+def _to_bf16_bits(x: np.ndarray) -> np.ndarray:
+    """Round float32 to bfloat16 (nearest even), returned as uint16 bit patterns."""
+    b = np.ascontiguousarray(x, np.float32).view(np.uint32).astype(np.uint64)
+    return ((b + 0x7FFF + ((b >> 16) & 1)) >> 16).astype(np.uint16)
+
+
+def policy_dims(cfg: dict) -> dict:
+    """Input/output widths of the two policy MLPs of a config."""
+    p = cfg["params"]
+    R, P, B, L = cfg["R"], len(p["prices"]), len(p["thresholds"]) + 1, len(p["rate_table"])
+    return dict(D_pop=6 + 8 * R + B, D_gov=3 * (3 + R) + B + 2, A=num_actions(R, P, p["craft_mode"], p["allow_noop"]),
+                gov_out=B * L, B=B, L=L)
+
+
+def policy_weights(cfg: dict, seed: int = 0, hidden: int = 128, std: float = 0.02, bias_std: float = 0.0):
+    """Random-init policy networks of BASELINE.json configs[4]: obs -> 128 -> 128 -> logits, weights
+    ~ N(0, std) rounded to bf16 (returned as uint16 bit patterns, [out][in] row-major), biases 0
+    (or N(0, bias_std) for tests of the bias path).  Returns (pop_net, gov_net) dicts."""
+    d = policy_dims(cfg)
+    rng = np.random.Generator(np.random.Philox(key=seed + 77))
+
+    def net(n_in, n_out):
+        out = {}
+        for name, (o, i) in (("w1", (hidden, n_in)), ("w2", (hidden, hidden)), ("w3", (n_out, hidden))):
+            out[name] = _to_bf16_bits((rng.standard_normal((o, i)) * std).astype(np.float32))
+        for name, o in (("b1", hidden), ("b2", hidden), ("b3", n_out)):
+            out[name] = (rng.standard_normal(o) * bias_std).astype(np.float32)
+        return out
+
+    return net(d["D_pop"], d["A"]), net(d["D_gov"], d["gov_out"])
