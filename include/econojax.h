@@ -114,7 +114,25 @@ typedef struct ej_rollout_io {
     uint8_t* done_ring;               /* [ring_depth][E] */
     int32_t* actions_ring;            /* [ring_depth][E][N] actions actually applied */
     int32_t* gov_actions_ring;        /* [ring_depth][E][B] */
+    float* pop_logits_ring;           /* policy mode only: [ring_depth][E*N][A] logits the actions were sampled from */
+    float* gov_logits_ring;           /* policy mode only: [ring_depth][E][B*L] */
 } ej_rollout_io;
+
+/* One tanh MLP  in_dim -> 128 -> 128 -> out_dim  (Table 2; BASELINE.json
+ * configs[4]).  HOST pointers, read during ej_set_policy only: bf16 bit patterns in the
+ * row-major [out_features][in_features] layout of a linear layer, fp32 biases. */
+typedef struct ej_mlp {
+    uint32_t struct_size;             /* = sizeof(ej_mlp) */
+    int32_t in_dim;                   /* D_pop (population) or D_gov (government) */
+    int32_t hidden;                   /* must be 128 */
+    int32_t out_dim;                  /* A (population) or B*L (government: B heads of L levels), <= 256 */
+    const uint16_t* w1;               /* [128][in_dim] */
+    const uint16_t* w2;               /* [128][128] */
+    const uint16_t* w3;               /* [out_dim][128] */
+    const float* b1;                  /* [128] */
+    const float* b2;                  /* [128] */
+    const float* b3;                  /* [out_dim] */
+} ej_mlp;
 
 /* Validate, allocate library-owned device state for E envs on the current CUDA device.
  * Errors: EJ_ERR_PARAM (field named), EJ_ERR_NOMEM, EJ_ERR_CUDA.  *out is NULL on failure;
@@ -165,6 +183,23 @@ int ej_set_action_cdf(ej_env* h, const uint32_t* cdf, int32_t A);
  * dump").  Both synchronise the stream.  Cold path: used by tests and checkpointing. */
 int ej_get_state(ej_env* h, int32_t env_begin, int32_t env_count, int32_t* words, size_t n_words);
 int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t* words, size_t n_words);
+
+/* a12 (G33): install (or, with two NULLs, remove) the shared population policy and the
+ * government policy.  While installed, ej_rollout draws its actions from them whenever
+ * io->actions_in / gov_actions_in is NULL: logits = W3 tanh(W2 tanh(W1 bf16(obs) + b1) + b2) + b3
+ * with bf16 operands, fp32 accumulation on the tensor cores and activations re-rounded to
+ * bf16; action = first a with u * S < sum_{j<=a} exp(l_j - max l), u = (x >> 8) * 2^-24 from the
+ * Philox word the CDF generator would have used (population: stream 0 word 0; government
+ * head b: stream 1 + b/4, word b%4).  Errors: EJ_ERR_PARAM (dims), EJ_ERR_NOMEM, EJ_ERR_CUDA. */
+int ej_set_policy(ej_env* h, const ej_mlp* pop, const ej_mlp* gov);
+
+/* Sample actions for the current clock of every env from the installed policies.
+ *  obs              device, obs_floats floats: observation of the current state (ej_observe / last ej_step)
+ *  actions_out      device [E][N] int32
+ *  gov_actions_out  device [E][B] int32
+ *  pop_logits_out   device [E*N][A] float or NULL;  gov_logits_out  device [E][B*L] float or NULL */
+int ej_policy_act(ej_env* h, const float* obs, int32_t* actions_out, int32_t* gov_actions_out, float* pop_logits_out,
+                  float* gov_logits_out);
 
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 int64_t ej_launch_count(const ej_env* h);

@@ -56,12 +56,21 @@ class EjRolloutIO(C.Structure):
         ("actions_in", C.c_void_p), ("gov_actions_in", C.c_void_p),
         ("obs_ring", C.c_void_p), ("rew_ring", C.c_void_p), ("done_ring", C.c_void_p),
         ("actions_ring", C.c_void_p), ("gov_actions_ring", C.c_void_p),
+        ("pop_logits_ring", C.c_void_p), ("gov_logits_ring", C.c_void_p),
+    ]
+
+
+class EjMlp(C.Structure):
+    _fields_ = [
+        ("struct_size", C.c_uint32), ("in_dim", C.c_int32), ("hidden", C.c_int32), ("out_dim", C.c_int32),
+        ("w1", C.c_void_p), ("w2", C.c_void_p), ("w3", C.c_void_p),
+        ("b1", C.c_void_p), ("b2", C.c_void_p), ("b3", C.c_void_p),
     ]
 
 
 EXPORTS = ("ej_create", "ej_destroy", "ej_set_stream", "ej_layout", "ej_last_error", "ej_reset", "ej_observe",
            "ej_step", "ej_step_host", "ej_rollout", "ej_set_action_cdf", "ej_get_state", "ej_set_state",
-           "ej_launch_count")
+           "ej_launch_count", "ej_set_policy", "ej_policy_act")
 
 _lib = None
 
@@ -89,6 +98,8 @@ def lib():
         L.ej_get_state.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_size_t]
         L.ej_set_state.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_size_t]
         L.ej_launch_count.argtypes = [vp]; L.ej_launch_count.restype = C.c_int64
+        L.ej_set_policy.argtypes = [vp, C.POINTER(EjMlp), C.POINTER(EjMlp)]
+        L.ej_policy_act.argtypes = [vp, vp, vp, vp, vp, vp]
         for name in EXPORTS:
             if name not in ("ej_last_error", "ej_launch_count"):
                 getattr(L, name).restype = C.c_int
@@ -191,6 +202,33 @@ def ej_set_state(h, env_begin: int, env_count: int, words: int, n_words: int):
     _check(h, lib().ej_set_state(h, env_begin, env_count, words, n_words))
 
 
+def ej_set_policy(h, pop: EjMlp | None, gov: EjMlp | None):
+    _check(h, lib().ej_set_policy(h, C.byref(pop) if pop is not None else None, C.byref(gov) if gov is not None else None))
+
+
+def ej_policy_act(h, obs: int, actions_out: int, gov_actions_out: int, pop_logits_out: int | None, gov_logits_out: int | None):
+    _check(h, lib().ej_policy_act(h, obs, actions_out, gov_actions_out, pop_logits_out, gov_logits_out))
+
+
+def make_mlp(net: dict) -> EjMlp:
+    """ej_mlp over host arrays: net = {"w1","w2","w3": uint16 bf16 bits [out][in]; "b1","b2","b3": float32}.
+    The arrays must stay alive until ej_set_policy returns (the struct keeps them referenced)."""
+    m = EjMlp()
+    m.struct_size = C.sizeof(EjMlp)
+    keep = []
+    for k in ("w1", "w2", "w3"):
+        a = np.ascontiguousarray(net[k], np.uint16)
+        keep.append(a)
+        setattr(m, k, a.ctypes.data)
+    for k in ("b1", "b2", "b3"):
+        a = np.ascontiguousarray(net[k], np.float32)
+        keep.append(a)
+        setattr(m, k, a.ctypes.data)
+    m.in_dim, m.hidden, m.out_dim = keep[0].shape[1], keep[0].shape[0], keep[2].shape[0]
+    m._keep = keep
+    return m
+
+
 def ej_launch_count(h) -> int:
     return int(lib().ej_launch_count(h))
 
@@ -274,14 +312,28 @@ class Env:
                      None if obs is None else obs.ctypes.data, None if rew is None else rew.ctypes.data,
                      None if done is None else done.ctypes.data)
 
+    def set_policy(self, pop_net: dict | None, gov_net: dict | None):
+        if pop_net is None and gov_net is None:
+            ej_set_policy(self.h, None, None)
+        else:
+            ej_set_policy(self.h, make_mlp(pop_net), make_mlp(gov_net))
+
+    def policy_act(self, obs, actions=None, gov_actions=None, pop_logits=None, gov_logits=None):
+        t = self.torch
+        actions = t.zeros((self.E, self.N), dtype=t.int32, device=self.device) if actions is None else actions
+        gov_actions = t.zeros((self.E, self.B), dtype=t.int32, device=self.device) if gov_actions is None else gov_actions
+        ej_policy_act(self.h, obs.data_ptr(), actions.data_ptr(), gov_actions.data_ptr(), _dp(pop_logits), _dp(gov_logits))
+        return actions, gov_actions
+
     def rollout(self, T, ring_depth=1, actions_in=None, gov_actions_in=None, obs_ring=None, rew_ring=None,
-                done_ring=None, actions_ring=None, gov_actions_ring=None):
+                done_ring=None, actions_ring=None, gov_actions_ring=None, pop_logits_ring=None, gov_logits_ring=None):
         io = EjRolloutIO()
         io.struct_size = C.sizeof(EjRolloutIO)
         io.ring_depth = ring_depth
         io.actions_in, io.gov_actions_in = _dp(actions_in), _dp(gov_actions_in)
         io.obs_ring, io.rew_ring, io.done_ring = _dp(obs_ring), _dp(rew_ring), _dp(done_ring)
         io.actions_ring, io.gov_actions_ring = _dp(actions_ring), _dp(gov_actions_ring)
+        io.pop_logits_ring, io.gov_logits_ring = _dp(pop_logits_ring), _dp(gov_logits_ring)
         ej_rollout(self.h, T, io)
 
     def set_action_cdf(self, cdf: np.ndarray):

@@ -13,6 +13,7 @@
 #include <vector>
 
 #include "ej_device.cuh"
+#include "ej_policy.cuh"
 
 namespace {
 
@@ -38,6 +39,13 @@ struct ej_env {
     int32_t *d_act = nullptr, *d_gov = nullptr;
     float *d_obs = nullptr, *d_rew = nullptr;
     uint8_t* d_done = nullptr;
+    // a12: installed policies and the buffers the policy-driven rollout chains through
+    bool has_policy = false;
+    PolicyNet pop_net{}, gov_net{};
+    uint8_t *d_pop_blob = nullptr, *d_gov_blob = nullptr;
+    float* d_pobs = nullptr;
+    int32_t *d_pact = nullptr, *d_pgov = nullptr;
+    int n_sms = 148;
 };
 
 namespace {
@@ -162,6 +170,129 @@ size_t state_words(const DevCfg& c) {
 int32_t f2w(float f) { int32_t w; memcpy(&w, &f, 4); return w; }
 float w2f(int32_t w) { float f; memcpy(&f, &w, 4); return f; }
 
+// ---- a12: policy networks ----
+int policy_smem_bytes(const PolicyNet& n) {
+    const int a_cols = n.K1p > PH ? n.K1p : PH;
+    return PTILE * a_cols * 2 + n.blob_bytes;
+}
+
+// Repack a row-major [rows][cols] bf16 matrix into the canonical K-major no-swizzle UMMA layout
+// with rows_p x cols_p extent (zero padded): element (r, k) at (r%8)*16 + (r/8)*cols_p*16 + (k/8)*128 + (k%8)*2.
+void pack_operand(const uint16_t* w, int rows, int cols, int rows_p, int cols_p, uint8_t* dst) {
+    memset(dst, 0, (size_t)rows_p * cols_p * 2);
+    for (int r = 0; r < rows; ++r)
+        for (int k = 0; k < cols; ++k) {
+            const size_t off = (size_t)(r & 7) * 16 + (size_t)(r >> 3) * cols_p * 16 + (size_t)(k >> 3) * 128 + (size_t)(k & 7) * 2;
+            memcpy(dst + off, &w[(size_t)r * cols + k], 2);
+        }
+}
+
+int build_net(ej_env* h, const ej_mlp* m, const char* which, int in_dim, int n_heads, int head, PolicyNet& net, uint8_t** d_blob) {
+    if (m->struct_size != sizeof(ej_mlp)) return fail(h, EJ_ERR_PARAM, "bad field: %s.struct_size", which);
+    if (m->hidden != PH) return fail(h, EJ_ERR_PARAM, "bad field: %s.hidden (must be 128)", which);
+    if (m->in_dim != in_dim) return fail(h, EJ_ERR_PARAM, "bad field: %s.in_dim", which);
+    if (m->out_dim != n_heads * head || m->out_dim > 256) return fail(h, EJ_ERR_PARAM, "bad field: %s.out_dim", which);
+    if (!m->w1 || !m->w2 || !m->w3 || !m->b1 || !m->b2 || !m->b3) return fail(h, EJ_ERR_PARAM, "bad field: %s weights", which);
+    net.D_in = in_dim;
+    net.K1p = (in_dim + 15) & ~15;
+    net.n_out = m->out_dim;
+    net.Op = (m->out_dim + 15) & ~15;
+    net.n_heads = n_heads;
+    net.head = head;
+    net.w1_bytes = PH * net.K1p * 2;
+    net.w2_bytes = PH * PH * 2;
+    net.w3_bytes = net.Op * PH * 2;
+    const int bias_bytes = align16((PH + PH + net.Op) * 4);
+    net.blob_bytes = net.w1_bytes + net.w2_bytes + net.w3_bytes + bias_bytes;
+    net.recipK1p = (uint32_t)((0x100000000ull + net.K1p - 1) / net.K1p);
+    if (policy_smem_bytes(net) > 200 * 1024) return fail(h, EJ_ERR_PARAM, "bad field: %s (network does not fit in shared memory)", which);
+    std::vector<uint8_t> blob(net.blob_bytes, 0);
+    pack_operand(m->w1, PH, in_dim, PH, net.K1p, blob.data());
+    pack_operand(m->w2, PH, PH, PH, PH, blob.data() + net.w1_bytes);
+    pack_operand(m->w3, m->out_dim, PH, net.Op, PH, blob.data() + net.w1_bytes + net.w2_bytes);
+    float* b = (float*)(blob.data() + net.w1_bytes + net.w2_bytes + net.w3_bytes);
+    memcpy(b, m->b1, PH * 4);
+    memcpy(b + PH, m->b2, PH * 4);
+    memcpy(b + 2 * PH, m->b3, (size_t)m->out_dim * 4);
+    if (*d_blob) { cudaFree(*d_blob); *d_blob = nullptr; }
+    if (cudaMalloc(d_blob, blob.size()) != cudaSuccess) { cudaGetLastError(); return fail(h, EJ_ERR_NOMEM, "%s", "policy allocation failed"); }
+    EJ_CUDA(h, cudaMemcpy(*d_blob, blob.data(), blob.size(), cudaMemcpyHostToDevice), "policy upload");
+    net.blob = *d_blob;
+    return EJ_OK;
+}
+
+int launch_policy(ej_env* h, const PolicyNet& net, const float* obs, int row_stride, int rows, int rows_per_env, int fixed_agent,
+                  uint32_t stream_base, int32_t* actions, float* logits) {
+    const DevCfg& c = h->c;
+    PolicyArgs a;
+    memset(&a, 0, sizeof(a));
+    a.net = net;
+    a.obs = obs; a.row_stride = row_stride; a.rows = rows; a.rows_per_env = rows_per_env; a.fixed_agent = fixed_agent;
+    a.state = h->d_state; a.blob_stride = c.blob_bytes;
+    a.env_id_base = c.env_id_base; a.seed_lo = c.seed_lo; a.seed_hi = c.seed_hi; a.stream_base = stream_base;
+    a.actions = actions; a.logits = logits;
+    const int a_cols = net.K1p > PH ? net.K1p : PH;
+    a.smem_A = 0;
+    a.smem_W1 = PTILE * a_cols * 2;
+    a.smem_W2 = a.smem_W1 + net.w1_bytes;
+    a.smem_W3 = a.smem_W2 + net.w2_bytes;
+    a.smem_bias = a.smem_W3 + net.w3_bytes;
+    const int tiles = (rows + PTILE - 1) / PTILE;
+    const int grid = tiles < 2 * h->n_sms ? tiles : 2 * h->n_sms;
+    ej_policy_kernel<<<grid, PTILE, policy_smem_bytes(net), h->stream>>>(a);
+    h->launches++;
+    EJ_CUDA(h, cudaGetLastError(), "ej_policy_kernel launch");
+    return EJ_OK;
+}
+
+int launch_step(ej_env* h, const StepIO& io);
+
+// ej_rollout in policy mode: per step, policy kernels (population, government) on the current
+// observation, then one step of the env kernel.  Observations and actions chain through the
+// caller's rings when given, else through library-owned buffers.
+int rollout_with_policy(ej_env* h, int T, const ej_rollout_io* rio, const StepIO& base) {
+    const DevCfg& c = h->c;
+    const size_t EN = (size_t)c.E * c.N, EB = (size_t)c.E * c.B;
+    const int depth = base.ring_depth;
+    float* pl_ring = rio ? rio->pop_logits_ring : nullptr;
+    float* gl_ring = rio ? rio->gov_logits_ring : nullptr;
+    // observation of the current state
+    int rc = for_block_size(c.Npad, [&](auto mt) {
+        constexpr int MT = decltype(mt)::value;
+        ej_observe_kernel<MT><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, h->d_pobs);
+        h->launches++;
+        EJ_CUDA(h, cudaGetLastError(), "ej_observe_kernel launch");
+        return EJ_OK;
+    });
+    if (rc != EJ_OK) return rc;
+    const float* cur_obs = h->d_pobs;
+    for (int s = 0; s < T; ++s) {
+        const int slot = s % depth;
+        int32_t* act = base.actions_out ? base.actions_out + slot * EN : h->d_pact;
+        int32_t* gov = base.gov_out ? base.gov_out + slot * EB : h->d_pgov;
+        rc = launch_policy(h, h->pop_net, cur_obs, c.D_pop, c.E * c.N, c.N, -1, 0u, act, pl_ring ? pl_ring + (size_t)slot * EN * c.A : nullptr);
+        if (rc != EJ_OK) return rc;
+        if (base.gov_actions) {
+            gov = const_cast<int32_t*>(base.gov_actions + (size_t)s * EB);
+        } else {
+            rc = launch_policy(h, h->gov_net, cur_obs + c.gov_obs_offset, c.D_gov_pad, c.E, 1, c.N, 1u, gov,
+                               gl_ring ? gl_ring + (size_t)slot * c.E * c.B * c.L : nullptr);
+            if (rc != EJ_OK) return rc;
+        }
+        StepIO io;
+        memset(&io, 0, sizeof(io));
+        io.cdf = base.cdf; io.n_steps = 1; io.ring_depth = 1;
+        io.actions = act; io.gov_actions = gov;
+        io.obs = base.obs ? base.obs + (size_t)slot * c.obs_floats : h->d_pobs;
+        io.rew = base.rew ? base.rew + (size_t)slot * (EN + c.E) : nullptr;
+        io.done = base.done ? base.done + (size_t)slot * c.E : nullptr;
+        rc = launch_step(h, io);
+        if (rc != EJ_OK) return rc;
+        cur_obs = io.obs;
+    }
+    return EJ_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -273,6 +404,7 @@ int ej_destroy(ej_env* h) {
     cudaStreamSynchronize(h->stream);
     cudaFree(h->d_state); cudaFree(h->d_cdf);
     cudaFree(h->d_act); cudaFree(h->d_gov); cudaFree(h->d_obs); cudaFree(h->d_rew); cudaFree(h->d_done);
+    cudaFree(h->d_pop_blob); cudaFree(h->d_gov_blob); cudaFree(h->d_pobs); cudaFree(h->d_pact); cudaFree(h->d_pgov);
     delete h;
     return EJ_OK;
 }
@@ -382,7 +514,46 @@ int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* rio) {
         io.obs = rio->obs_ring; io.rew = rio->rew_ring; io.done = rio->done_ring;
         io.actions_out = rio->actions_ring; io.gov_out = rio->gov_actions_ring;
     }
+    if (h->has_policy && !io.actions) return rollout_with_policy(h, T, rio, io);
     return launch_step(h, io);
+}
+
+int ej_set_policy(ej_env* h, const ej_mlp* pop, const ej_mlp* gov) {
+    if (!h) return EJ_ERR_PARAM;
+    const DevCfg& c = h->c;
+    if (!pop && !gov) { h->has_policy = false; return EJ_OK; }
+    if (!pop || !gov) return fail(h, EJ_ERR_PARAM, "bad field: %s", "pop / gov (both or neither)");
+    EJ_CUDA(h, cudaStreamSynchronize(h->stream), "set_policy sync");
+    h->has_policy = false;
+    int rc = build_net(h, pop, "pop", c.D_pop, 1, c.A, h->pop_net, &h->d_pop_blob);
+    if (rc != EJ_OK) return rc;
+    rc = build_net(h, gov, "gov", c.D_gov, c.B, c.L, h->gov_net, &h->d_gov_blob);
+    if (rc != EJ_OK) return rc;
+    const int smem = policy_smem_bytes(h->pop_net) > policy_smem_bytes(h->gov_net) ? policy_smem_bytes(h->pop_net) : policy_smem_bytes(h->gov_net);
+    EJ_CUDA(h, cudaFuncSetAttribute(ej_policy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem), "smem attr (policy)");
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&h->n_sms, cudaDevAttrMultiProcessorCount, dev);
+    if (!h->d_pobs) {
+        cudaError_t ce = cudaMalloc(&h->d_pobs, (size_t)c.obs_floats * 4);
+        if (ce == cudaSuccess) ce = cudaMalloc(&h->d_pact, (size_t)c.E * c.N * 4);
+        if (ce == cudaSuccess) ce = cudaMalloc(&h->d_pgov, (size_t)c.E * c.B * 4);
+        if (ce != cudaSuccess) { cudaGetLastError(); return fail(h, EJ_ERR_NOMEM, "%s", "policy buffers allocation failed"); }
+    }
+    h->has_policy = true;
+    return EJ_OK;
+}
+
+int ej_policy_act(ej_env* h, const float* obs, int32_t* actions_out, int32_t* gov_actions_out, float* pop_logits_out,
+                  float* gov_logits_out) {
+    if (!h) return EJ_ERR_PARAM;
+    if (!h->has_policy) return fail(h, EJ_ERR_STATE, "%s", "ej_policy_act before ej_set_policy");
+    if (!h->was_reset) return fail(h, EJ_ERR_STATE, "%s", "ej_policy_act before ej_reset / ej_set_state");
+    if (!obs || !actions_out || !gov_actions_out) return fail(h, EJ_ERR_PARAM, "bad field: %s", "obs / actions_out / gov_actions_out");
+    const DevCfg& c = h->c;
+    int rc = launch_policy(h, h->pop_net, obs, c.D_pop, c.E * c.N, c.N, -1, 0u, actions_out, pop_logits_out);
+    if (rc != EJ_OK) return rc;
+    return launch_policy(h, h->gov_net, obs + c.gov_obs_offset, c.D_gov_pad, c.E, 1, c.N, 1u, gov_actions_out, gov_logits_out);
 }
 
 int ej_set_action_cdf(ej_env* h, const uint32_t* cdf, int32_t A) {
