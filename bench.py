@@ -36,7 +36,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-from paper_2410_22165_b200 import inputs  # noqa: E402
+from paper_2410_22165_b200 import inputs, sharding  # noqa: E402
 
 METRIC = "agent_steps_per_sec"
 UNIT = "agent-steps/s"
@@ -201,9 +201,12 @@ def main():
 
     E, N, R, T = cfg["E"], cfg["N"], cfg["R"], cfg["T"]
     # envs are independent and keyed by global id: rank r owns global envs [r*E, (r+1)*E) (weak scaling)
-    params = dict(cfg["params"], env_id_base=rank * E)
+    params = dict(cfg["params"], env_id_base=sharding.shard_env_base(rank, world, E))
     env = binding.Env(E, N, R, params, device=str(dev))
     env.set_action_cdf(inputs.action_cdf(cfg))
+    use_policy = cfg["action_mix"] == "policy"
+    if use_policy:  # configs[4]: actions come from the on-GPU policy MLPs (a12)
+        env.set_policy(*inputs.policy_weights(cfg, seed=cfg["seed"]))
     B, K, W = env.B, args.steps, args.warmup
     depth = max(1, min(args.ring, K))
     chunk = min(K, 128)  # action streams are supplied per chunk of <= 128 steps (resident in HBM)
@@ -227,8 +230,8 @@ def main():
                 env.reset(cfg["seed"])
                 run_steps.t = t_now = 0
             m = min(n - done_steps, chunk, T - t_now)
-            env.rollout(m, ring_depth=depth, actions_in=acts, gov_actions_in=gov, obs_ring=obs_ring, rew_ring=rew_ring,
-                        done_ring=done_ring)
+            env.rollout(m, ring_depth=depth, actions_in=None if use_policy else acts, gov_actions_in=None if use_policy else gov,
+                        obs_ring=obs_ring, rew_ring=rew_ring, done_ring=done_ring)
             run_steps.t += m
             done_steps += m
 
@@ -248,11 +251,8 @@ def main():
     launches = env.launch_count() - l0
     ms = ev0.elapsed_time(ev1)
     clocks = sampler.stop()
-    if world > 1:
-        tmax = torch.tensor([ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-        ms = float(tmax.item())
-    value = world * E * N * K / (ms * 1e-3)
+    ms = sharding.max_over_ranks(ms, dist, dev)
+    value = sharding.total_units(E * N * K, world) / (ms * 1e-3)
 
     # ---- per-launch ej_step path, device-resident inputs (reported beside the rollout) ----
     step_ms = None
@@ -292,10 +292,7 @@ def main():
         e1.record()
         barrier()
         e_ms = e0.elapsed_time(e1)
-        if world > 1:
-            tm = torch.tensor([e_ms], device=dev, dtype=torch.float64)
-            dist.all_reduce(tm, op=dist.ReduceOp.MAX)
-            e_ms = float(tm.item())
+        e_ms = sharding.max_over_ranks(e_ms, dist, dev)
         e2e = {"value": world * E * N * Ke / (e_ms * 1e-3), "unit": UNIT,
                "h2d_bytes_per_step": int(4 * E * N + 4 * E * B),
                "d2h_bytes_per_step": int(4 * env.obs_floats + 4 * E * (N + 1) + E),
@@ -312,7 +309,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": ms / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f32", "data": "synthetic",
-        "config": {"workload": workload_desc(name, cfg, E), "E_per_gpu": E, "api": "ej_rollout (persistent kernel)",
+        "config": {"workload": workload_desc(name, cfg, E), "E_per_gpu": E, "api": "ej_rollout (policy kernels + step kernel per step)" if use_policy else "ej_rollout (persistent kernel)",
                    "l2": "outputs go to a ring of %d steps x %.1f MB (> 126 MB L2); action streams %d steps x %.1f MB" % (
                        depth, bytes_env_step * E / 1e6, chunk, 4e-6 * E * (N + B))},
         "env_steps_per_sec": world * E * K / (ms * 1e-3),

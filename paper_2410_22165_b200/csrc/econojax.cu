@@ -171,9 +171,22 @@ int32_t f2w(float f) { int32_t w; memcpy(&w, &f, 4); return w; }
 float w2f(int32_t w) { float f; memcpy(&f, &w, 4); return f; }
 
 // ---- a12: policy networks ----
-int policy_smem_bytes(const PolicyNet& n) {
+int align128(int x) { return (x + 127) & ~127; }
+
+// Dynamic shared memory of ej_policy_kernel: weights once, then per group an A tile and the fp32 staging tile.
+int policy_group_bytes(const PolicyNet& n, int row_stride) {
     const int a_cols = n.K1p > PH ? n.K1p : PH;
-    return PTILE * a_cols * 2 + n.blob_bytes;
+    return align128(PTILE * a_cols * 2 + align16(PTILE * row_stride * 4));
+}
+int policy_tmem_cols(const PolicyNet& n) { return n.Op > 128 ? 256 : 128; }
+int policy_groups(const PolicyNet& n, int row_stride) {
+    int g = P_TMEM_ALLOC / policy_tmem_cols(n);
+    const int fit = (227 * 1024 - align128(n.blob_bytes)) / policy_group_bytes(n, row_stride);
+    if (g > fit) g = fit;
+    return g > PGROUPS ? PGROUPS : g;
+}
+int policy_smem_bytes(const PolicyNet& n, int row_stride) {
+    return align128(n.blob_bytes) + policy_groups(n, row_stride) * policy_group_bytes(n, row_stride);
 }
 
 // Repack a row-major [rows][cols] bf16 matrix into the canonical K-major no-swizzle UMMA layout
@@ -205,7 +218,7 @@ int build_net(ej_env* h, const ej_mlp* m, const char* which, int in_dim, int n_h
     const int bias_bytes = align16((PH + PH + net.Op) * 4);
     net.blob_bytes = net.w1_bytes + net.w2_bytes + net.w3_bytes + bias_bytes;
     net.recipK1p = (uint32_t)((0x100000000ull + net.K1p - 1) / net.K1p);
-    if (policy_smem_bytes(net) > 200 * 1024) return fail(h, EJ_ERR_PARAM, "bad field: %s (network does not fit in shared memory)", which);
+    if (policy_groups(net, in_dim + 3) < 1) return fail(h, EJ_ERR_PARAM, "bad field: %s (network does not fit in shared memory)", which);
     std::vector<uint8_t> blob(net.blob_bytes, 0);
     pack_operand(m->w1, PH, in_dim, PH, net.K1p, blob.data());
     pack_operand(m->w2, PH, PH, PH, PH, blob.data() + net.w1_bytes);
@@ -221,10 +234,9 @@ int build_net(ej_env* h, const ej_mlp* m, const char* which, int in_dim, int n_h
     return EJ_OK;
 }
 
-int launch_policy(ej_env* h, const PolicyNet& net, const float* obs, int row_stride, int rows, int rows_per_env, int fixed_agent,
-                  uint32_t stream_base, int32_t* actions, float* logits) {
+void fill_job(ej_env* h, PolicyArgs& a, const PolicyNet& net, const float* obs, int row_stride, int rows, int rows_per_env,
+              int fixed_agent, uint32_t stream_base, int32_t* actions, float* logits) {
     const DevCfg& c = h->c;
-    PolicyArgs a;
     memset(&a, 0, sizeof(a));
     a.net = net;
     a.obs = obs; a.row_stride = row_stride; a.rows = rows; a.rows_per_env = rows_per_env; a.fixed_agent = fixed_agent;
@@ -232,14 +244,39 @@ int launch_policy(ej_env* h, const PolicyNet& net, const float* obs, int row_str
     a.env_id_base = c.env_id_base; a.seed_lo = c.seed_lo; a.seed_hi = c.seed_hi; a.stream_base = stream_base;
     a.actions = actions; a.logits = logits;
     const int a_cols = net.K1p > PH ? net.K1p : PH;
-    a.smem_A = 0;
-    a.smem_W1 = PTILE * a_cols * 2;
+    a.smem_W1 = 0;
     a.smem_W2 = a.smem_W1 + net.w1_bytes;
     a.smem_W3 = a.smem_W2 + net.w2_bytes;
     a.smem_bias = a.smem_W3 + net.w3_bytes;
-    const int tiles = (rows + PTILE - 1) / PTILE;
-    const int grid = tiles < 2 * h->n_sms ? tiles : 2 * h->n_sms;
-    ej_policy_kernel<<<grid, PTILE, policy_smem_bytes(net), h->stream>>>(a);
+    a.smem_group = align128(net.blob_bytes);
+    a.group_bytes = policy_group_bytes(net, row_stride);
+    a.stage_off = PTILE * a_cols * 2;
+    a.groups = policy_groups(net, row_stride);
+    a.tmem_cols = policy_tmem_cols(net);
+}
+
+int ctas_for(const PolicyArgs& a, int cap) {
+    const int tiles = (a.rows + PTILE - 1) / PTILE;
+    const int want = (tiles + a.groups - 1) / a.groups;
+    return want < cap ? want : cap;
+}
+
+// Population and (optionally) government policy in ONE launch: the government's few tiles get
+// their own CTAs next to the population's, so they cost no extra launch and no extra latency.
+int launch_policy(ej_env* h, const float* obs, int32_t* actions, int32_t* gov_actions, float* pop_logits, float* gov_logits) {
+    const DevCfg& c = h->c;
+    PolicyLaunch pl;
+    memset(&pl, 0, sizeof(pl));
+    fill_job(h, pl.job[0], h->pop_net, obs, c.D_pop, c.E * c.N, c.N, -1, 0u, actions, pop_logits);
+    int smem = policy_smem_bytes(h->pop_net, c.D_pop), gov_ctas = 0;
+    if (gov_actions) {
+        fill_job(h, pl.job[1], h->gov_net, obs + c.gov_obs_offset, c.D_gov_pad, c.E, 1, c.N, 1u, gov_actions, gov_logits);
+        gov_ctas = ctas_for(pl.job[1], h->n_sms / 8 > 0 ? h->n_sms / 8 : 1);
+        const int sg = policy_smem_bytes(h->gov_net, c.D_gov_pad);
+        if (sg > smem) smem = sg;
+    }
+    pl.split = ctas_for(pl.job[0], h->n_sms - gov_ctas);
+    ej_policy_kernel<<<pl.split + gov_ctas, PGROUPS * PTILE, smem, h->stream>>>(pl);
     h->launches++;
     EJ_CUDA(h, cudaGetLastError(), "ej_policy_kernel launch");
     return EJ_OK;
@@ -270,15 +307,11 @@ int rollout_with_policy(ej_env* h, int T, const ej_rollout_io* rio, const StepIO
         const int slot = s % depth;
         int32_t* act = base.actions_out ? base.actions_out + slot * EN : h->d_pact;
         int32_t* gov = base.gov_out ? base.gov_out + slot * EB : h->d_pgov;
-        rc = launch_policy(h, h->pop_net, cur_obs, c.D_pop, c.E * c.N, c.N, -1, 0u, act, pl_ring ? pl_ring + (size_t)slot * EN * c.A : nullptr);
+        const bool gov_supplied = base.gov_actions != nullptr;
+        rc = launch_policy(h, cur_obs, act, gov_supplied ? nullptr : gov, pl_ring ? pl_ring + (size_t)slot * EN * c.A : nullptr,
+                           gl_ring ? gl_ring + (size_t)slot * c.E * c.B * c.L : nullptr);
         if (rc != EJ_OK) return rc;
-        if (base.gov_actions) {
-            gov = const_cast<int32_t*>(base.gov_actions + (size_t)s * EB);
-        } else {
-            rc = launch_policy(h, h->gov_net, cur_obs + c.gov_obs_offset, c.D_gov_pad, c.E, 1, c.N, 1u, gov,
-                               gl_ring ? gl_ring + (size_t)slot * c.E * c.B * c.L : nullptr);
-            if (rc != EJ_OK) return rc;
-        }
+        if (gov_supplied) gov = const_cast<int32_t*>(base.gov_actions + (size_t)s * EB);
         StepIO io;
         memset(&io, 0, sizeof(io));
         io.cdf = base.cdf; io.n_steps = 1; io.ring_depth = 1;
@@ -529,7 +562,8 @@ int ej_set_policy(ej_env* h, const ej_mlp* pop, const ej_mlp* gov) {
     if (rc != EJ_OK) return rc;
     rc = build_net(h, gov, "gov", c.D_gov, c.B, c.L, h->gov_net, &h->d_gov_blob);
     if (rc != EJ_OK) return rc;
-    const int smem = policy_smem_bytes(h->pop_net) > policy_smem_bytes(h->gov_net) ? policy_smem_bytes(h->pop_net) : policy_smem_bytes(h->gov_net);
+    const int sp = policy_smem_bytes(h->pop_net, c.D_pop), sg = policy_smem_bytes(h->gov_net, c.D_gov_pad);
+    const int smem = sp > sg ? sp : sg;
     EJ_CUDA(h, cudaFuncSetAttribute(ej_policy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem), "smem attr (policy)");
     int dev = 0;
     cudaGetDevice(&dev);
@@ -551,9 +585,8 @@ int ej_policy_act(ej_env* h, const float* obs, int32_t* actions_out, int32_t* go
     if (!h->was_reset) return fail(h, EJ_ERR_STATE, "%s", "ej_policy_act before ej_reset / ej_set_state");
     if (!obs || !actions_out || !gov_actions_out) return fail(h, EJ_ERR_PARAM, "bad field: %s", "obs / actions_out / gov_actions_out");
     const DevCfg& c = h->c;
-    int rc = launch_policy(h, h->pop_net, obs, c.D_pop, c.E * c.N, c.N, -1, 0u, actions_out, pop_logits_out);
-    if (rc != EJ_OK) return rc;
-    return launch_policy(h, h->gov_net, obs + c.gov_obs_offset, c.D_gov_pad, c.E, 1, c.N, 1u, gov_actions_out, gov_logits_out);
+    (void)c;
+    return launch_policy(h, obs, actions_out, gov_actions_out, pop_logits_out, gov_logits_out);
 }
 
 int ej_set_action_cdf(ej_env* h, const uint32_t* cdf, int32_t A) {

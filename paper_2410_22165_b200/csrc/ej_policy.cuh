@@ -9,8 +9,10 @@
 // same layout between layers.  Each layer is a chain of tcgen05.mma (M=128, N=128|Op, K=16)
 // issued by one thread, accumulating in TMEM; completion comes back through tcgen05.commit on
 // an mbarrier; the epilogue reads its row with tcgen05.ld, adds the bias, applies tanh, rounds
-// to bf16 and writes the next layer's A operand.  Two CTAs per SM overlap one CTA's epilogue
-// with the other's MMAs.
+// to bf16 and writes the next layer's A operand.  One CTA per SM holds the weights once and runs
+// TWO such 128-thread groups on alternating tiles (own A tile, own half of TMEM, own named
+// barrier), so one group's epilogue overlaps the other's MMAs; the fp32 observation tile of the
+// group's next tile is prefetched by a 1-D TMA bulk copy (cp.async.bulk) while it computes.
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -20,7 +22,8 @@ namespace {
 
 constexpr int PH = 128;        // hidden width (B:configs[4]: 128 -> 128)
 constexpr int PTILE = 128;     // rows per tile = UMMA M
-constexpr int P_TMEM_COLS = 256;
+constexpr int P_TMEM_ALLOC = 512;  // whole TMEM of the SM (one CTA per SM); group g uses columns [g * tmem_cols, ...)
+constexpr int PGROUPS = 3;         // 128-thread groups per CTA (a job may use fewer)
 
 struct PolicyNet {
     const uint8_t* blob;   // device: W1 | W2 | W3 (canonical bf16) | b1 | b2 | b3 (f32)
@@ -44,7 +47,16 @@ struct PolicyArgs {
     uint32_t stream_base;    // Philox stream of head 0 (population 0, government 1); head h uses word h % 4 of stream + h / 4
     int32_t* actions;        // [rows][n_heads]
     float* logits;           // [rows][n_out] or null
-    int smem_A, smem_W1, smem_W2, smem_W3, smem_bias;  // byte offsets in dynamic shared memory
+    int smem_W1, smem_W2, smem_W3, smem_bias;  // byte offsets in dynamic shared memory (shared by both groups)
+    int smem_group, group_bytes, stage_off;     // group g: A tile at smem_group + g * group_bytes, fp32 staging at + stage_off
+    int groups, tmem_cols;   // active groups of this job (<= PGROUPS) and TMEM columns per group (128 or 256)
+};
+
+// One launch runs up to two jobs side by side: CTAs [0, split) work on job 0 (population),
+// CTAs [split, gridDim.x) on job 1 (government), each with its own weights in shared memory.
+struct PolicyLaunch {
+    PolicyArgs job[2];
+    int split;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -93,6 +105,19 @@ __device__ __forceinline__ void tmem_ld8(uint32_t taddr, float (&v)[8]) {
     for (int j = 0; j < 8; ++j) v[j] = __uint_as_float(r[j]);
 }
 
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float (&v)[16]) {
+    uint32_t r[16];
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+          "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+#pragma unroll
+    for (int j = 0; j < 16; ++j) v[j] = __uint_as_float(r[j]);
+}
+
 __device__ __forceinline__ float tanh_fast(float x) {
     float y;
     asm("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x));
@@ -117,95 +142,161 @@ __device__ __forceinline__ void issue_layer(uint32_t a_addr, uint32_t w_addr, in
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" ::"r"(bar) : "memory");
 }
 
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];\n"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+          "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
+          "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
+          "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+}
+
 // Hidden-layer epilogue: this thread's accumulator row -> +bias -> tanh -> bf16 -> A operand (kp = 128).
 __device__ __forceinline__ void hidden_epilogue(uint32_t taddr_row, const float* bias, uint8_t* A, int row) {
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-#pragma unroll 4
-    for (int c = 0; c < PH; c += 8) {
-        float v[8];
-        tmem_ld8(taddr_row + c, v);
-        uint32_t w[4];
+#pragma unroll 1
+    for (int c = 0; c < PH; c += 32) {
+        uint32_t r[32];
+        tmem_ld32(taddr_row + c, r);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const float a0 = tanh_fast(v[2 * j] + bias[c + 2 * j]), a1 = tanh_fast(v[2 * j + 1] + bias[c + 2 * j + 1]);
-            const __nv_bfloat162 h = __floats2bfloat162_rn(a0, a1);
-            w[j] = *reinterpret_cast<const uint32_t*>(&h);
+        for (int g = 0; g < 4; ++g) {
+            uint32_t w[4];
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k = g * 8 + 2 * j;
+                const float a0 = tanh_fast(__uint_as_float(r[k]) + bias[c + k]), a1 = tanh_fast(__uint_as_float(r[k + 1]) + bias[c + k + 1]);
+                const __nv_bfloat162 h = __floats2bfloat162_rn(a0, a1);
+                w[j] = *reinterpret_cast<const uint32_t*>(&h);
+            }
+            *reinterpret_cast<uint4*>(A + op_off(row, c + g * 8, PH)) = make_uint4(w[0], w[1], w[2], w[3]);
         }
-        *reinterpret_cast<uint4*>(A + op_off(row, c, PH)) = make_uint4(w[0], w[1], w[2], w[3]);
     }
 }
 
-__global__ void __launch_bounds__(PTILE, 2) ej_policy_kernel(const __grid_constant__ PolicyArgs a) {
+__device__ __forceinline__ void group_sync(int grp) { asm volatile("bar.sync %0, %1;\n" ::"r"(grp + 1), "r"(PTILE) : "memory"); }
+
+// 1-D TMA bulk copy global -> shared, completion on an mbarrier (bytes and both addresses multiples of 16).
+__device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;\n" ::"r"(bar), "r"(bytes) : "memory");
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];\n" ::"r"(dst), "l"(src), "r"(bytes),
+                 "r"(bar)
+                 : "memory");
+}
+
+__global__ void __launch_bounds__(PGROUPS* PTILE, 1) ej_policy_kernel(const __grid_constant__ PolicyLaunch pl) {
+    const bool second = (int)blockIdx.x >= pl.split;
+    const PolicyArgs& a = second ? pl.job[1] : pl.job[0];
+    const int bid = second ? (int)blockIdx.x - pl.split : (int)blockIdx.x, nblk = second ? (int)gridDim.x - pl.split : pl.split;
     extern __shared__ __align__(128) uint8_t psm[];
-    __shared__ __align__(8) unsigned long long mbar;
+    __shared__ __align__(8) unsigned long long mbar_mma[PGROUPS], mbar_tma[PGROUPS];
     __shared__ uint32_t tmem_slot;
-    const int tid = threadIdx.x, warp = tid >> 5;
+    const int tid = threadIdx.x, warp = tid >> 5, grp = tid >> 7, gtid = tid & (PTILE - 1);
     const PolicyNet& n = a.net;
-    uint8_t* A = psm + a.smem_A;
+    uint8_t* A = psm + a.smem_group + grp * a.group_bytes;
+    const float* stage = reinterpret_cast<const float*>(A + a.stage_off);
     const float* b1 = reinterpret_cast<const float*>(psm + a.smem_bias);
     const float* b2 = b1 + PH;
     const float* b3 = b2 + PH;
 
-    // ---- one-time setup: weights to shared memory, mbarrier, TMEM ----
+    // ---- one-time setup: weights to shared memory (once per SM), mbarriers, TMEM ----
     {
         const uint4* src = reinterpret_cast<const uint4*>(n.blob);
         uint4* dst = reinterpret_cast<uint4*>(psm + a.smem_W1);  // W1 | W2 | W3 | biases are contiguous in both
-        for (int i = tid; i < n.blob_bytes / 16; i += PTILE) dst[i] = src[i];
+        for (int i = tid; i < n.blob_bytes / 16; i += PGROUPS * PTILE) dst[i] = src[i];
     }
-    const uint32_t bar = smem_u32(&mbar);
     if (tid == 0) {
-        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(bar) : "memory");
+        for (int g = 0; g < PGROUPS; ++g) {
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(&mbar_mma[g])) : "memory");
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(&mbar_tma[g])) : "memory");
+        }
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
     }
     if (warp == 0) {
-        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_slot)), "r"(P_TMEM_COLS) : "memory");
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_slot)), "r"(P_TMEM_ALLOC) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
     }
     asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // weights were written by the generic proxy
     asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-    const uint32_t tmem = tmem_slot;
-    const uint32_t taddr_row = tmem + ((uint32_t)(warp * 32) << 16);  // this warp's 32 lanes
-    const uint32_t a_addr = smem_u32(A), w1_addr = smem_u32(psm + a.smem_W1), w2_addr = smem_u32(psm + a.smem_W2),
-                   w3_addr = smem_u32(psm + a.smem_W3);
-    uint32_t phase = 0;
+    const uint32_t tmem_base = tmem_slot;
+    const uint32_t tmem = tmem_base + (uint32_t)(grp * a.tmem_cols);           // this group's columns
+    const uint32_t taddr_row = tmem + ((uint32_t)((warp & 3) * 32) << 16);     // this warp's 32 lanes
+    const uint32_t bar = smem_u32(&mbar_mma[grp]), tbar = smem_u32(&mbar_tma[grp]);
+    const uint32_t a_addr = smem_u32(A), stage_addr = smem_u32(stage), w1_addr = smem_u32(psm + a.smem_W1),
+                   w2_addr = smem_u32(psm + a.smem_W2), w3_addr = smem_u32(psm + a.smem_W3);
+    uint32_t phase = 0, tphase = 0;
 
     const int n_tiles = (a.rows + PTILE - 1) / PTILE;
-    for (int tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const int row0 = tile * PTILE;
-        // ---- observation tile -> bf16 A operand (K1p columns, zero padded) ----
-        for (int idx = tid; idx < PTILE * n.K1p; idx += PTILE) {
-            const int r = (int)__umulhi((uint32_t)idx, n.recipK1p), k = idx - r * n.K1p;
-            float v = 0.0f;
-            if (k < n.D_in && row0 + r < a.rows) v = a.obs[(size_t)(row0 + r) * a.row_stride + k];
-            *reinterpret_cast<__nv_bfloat16*>(A + op_off(r, k, n.K1p)) = __float2bfloat16_rn(v);
+    const int tile_step = nblk * a.groups;
+    // a tile's rows are contiguous in global memory; TMA needs 16-byte multiples
+    auto tile_rows = [&](int tile) { const int left = a.rows - tile * PTILE; return left < PTILE ? left : PTILE; };
+    auto tile_bytes = [&](int tile) { return (uint32_t)(tile_rows(tile) * a.row_stride * 4); };
+    auto tile_src = [&](int tile) { return a.obs + (size_t)tile * PTILE * a.row_stride; };
+    auto tma_ok = [&](int tile) { return ((reinterpret_cast<uintptr_t>(tile_src(tile)) | tile_bytes(tile)) & 15u) == 0; };
+    int tile = grp < a.groups ? bid * a.groups + grp : n_tiles;  // surplus groups idle
+    if (tile < n_tiles && gtid == 0 && tma_ok(tile)) tma_load_1d(stage_addr, tile_src(tile), tile_bytes(tile), tbar);
+
+    for (; tile < n_tiles; tile += tile_step) {
+        const int row0 = tile * PTILE, nrows = tile_rows(tile);
+        // ---- observation tile (fp32, staged) -> bf16 A operand (K1p columns, zero padded) ----
+        if (tma_ok(tile)) {
+            mbar_wait(tbar, tphase);
+            tphase ^= 1;
+        } else {  // unaligned tile: plain coalesced copy by the group
+            float* st = const_cast<float*>(stage);
+            const float* src = tile_src(tile);
+            for (int i = gtid; i < nrows * a.row_stride; i += PTILE) st[i] = src[i];
+            group_sync(grp);
+        }
+        {
+            const float* my = stage + gtid * a.row_stride;
+            for (int kc = 0; kc < n.K1p / 8; ++kc) {
+                uint32_t w[4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int k = kc * 8 + 2 * j;
+                    const float v0 = (gtid < nrows && k < n.D_in) ? my[k] : 0.0f;
+                    const float v1 = (gtid < nrows && k + 1 < n.D_in) ? my[k + 1] : 0.0f;
+                    const __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
+                    w[j] = *reinterpret_cast<const uint32_t*>(&h);
+                }
+                *reinterpret_cast<uint4*>(A + op_off(gtid, kc * 8, n.K1p)) = make_uint4(w[0], w[1], w[2], w[3]);
+            }
         }
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        __syncthreads();
-        if (tid == 0) issue_layer(a_addr, w1_addr, n.K1p, PH, tmem, bar);
+        group_sync(grp);
+        if (gtid == 0) {
+            issue_layer(a_addr, w1_addr, n.K1p, PH, tmem, bar);
+            const int next = tile + tile_step;  // the staging buffer is free: prefetch the group's next tile
+            if (next < n_tiles && tma_ok(next)) tma_load_1d(stage_addr, tile_src(next), tile_bytes(next), tbar);
+        }
         mbar_wait(bar, phase);
         phase ^= 1;
-        hidden_epilogue(taddr_row, b1, A, tid);
+        hidden_epilogue(taddr_row, b1, A, gtid);
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        __syncthreads();
-        if (tid == 0) issue_layer(a_addr, w2_addr, PH, PH, tmem, bar);
+        group_sync(grp);
+        if (gtid == 0) issue_layer(a_addr, w2_addr, PH, PH, tmem, bar);
         mbar_wait(bar, phase);
         phase ^= 1;
-        hidden_epilogue(taddr_row, b2, A, tid);
+        hidden_epilogue(taddr_row, b2, A, gtid);
         asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
         asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        __syncthreads();
-        if (tid == 0) issue_layer(a_addr, w3_addr, PH, n.Op, tmem, bar);
+        group_sync(grp);
+        if (gtid == 0) issue_layer(a_addr, w3_addr, PH, n.Op, tmem, bar);
         mbar_wait(bar, phase);
         phase ^= 1;
         asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
 
         // ---- logits -> softmax -> inverse-CDF sample per head (G33) ----
-        const int row = row0 + tid;
-        const bool live = row < a.rows;
+        const int row = row0 + gtid;
+        const bool live = gtid < nrows;
         const int env = live ? row / a.rows_per_env : 0;
         const int agent = a.fixed_agent >= 0 ? a.fixed_agent : row - env * a.rows_per_env;
         const int t = live ? *reinterpret_cast<const int*>(a.state + (size_t)env * a.blob_stride) : 0;
@@ -217,32 +308,41 @@ __global__ void __launch_bounds__(PTILE, 2) ej_policy_kernel(const __grid_consta
             const uint32_t xw = (h & 3) == 0 ? x[0] : (h & 3) == 1 ? x[1] : (h & 3) == 2 ? x[2] : x[3];
             const float u = u01(xw);
             const int lo = h * n.head, hi = lo + n.head;
-            // pass 1: running maximum and sum of exp (online softmax), fp32
-            float mx = -INFINITY, s = 0.0f;
-            for (int c = lo & ~7; c < hi; c += 8) {
-                float v[8];
-                tmem_ld8(taddr_row + c, v);
+            // three sweeps over this thread's TMEM row, each a chain of independent operations:
+            // maximum; sum of exp(l - max); first index whose cumulative weight exceeds u * sum
+            float mx = -INFINITY;
+            for (int c = lo & ~15; c < hi; c += 16) {
+                float v[16];
+                tmem_ld16(taddr_row + c, v);
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < 16; ++j) {
                     const int col = c + j;
                     if (col >= lo && col < hi) {
                         const float l = v[j] + b3[col];
                         if (a.logits && live) a.logits[(size_t)row * n.n_out + col] = l;
-                        if (l > mx) { s = s * __expf(mx - l) + 1.0f; mx = l; }
-                        else s += __expf(l - mx);
+                        mx = fmaxf(mx, l);
                     }
                 }
             }
-            // pass 2: first index whose cumulative weight exceeds u * s (last index otherwise)
+            float s = 0.0f;
+            for (int c = lo & ~15; c < hi; c += 16) {
+                float v[16];
+                tmem_ld16(taddr_row + c, v);
+#pragma unroll
+                for (int j = 0; j < 16; ++j) {
+                    const int col = c + j;
+                    if (col >= lo && col < hi) s += __expf(v[j] + b3[col] - mx);
+                }
+            }
             const float target = u * s;
             float cum = 0.0f;
             int pick = n.head - 1;
             bool found = false;
-            for (int c = lo & ~7; c < hi; c += 8) {
-                float v[8];
-                tmem_ld8(taddr_row + c, v);
+            for (int c = lo & ~15; c < hi; c += 16) {
+                float v[16];
+                tmem_ld16(taddr_row + c, v);
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < 16; ++j) {
                     const int col = c + j;
                     if (col >= lo && col < hi) {
                         cum += __expf(v[j] + b3[col] - mx);
@@ -254,10 +354,12 @@ __global__ void __launch_bounds__(PTILE, 2) ej_policy_kernel(const __grid_consta
         }
         // the next tile's MMAs overwrite these TMEM columns and the A tile
         asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        __syncthreads();
+        group_sync(grp);
     }
 
-    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem), "r"(P_TMEM_COLS) : "memory");
+    asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+    __syncthreads();
+    if (warp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(tmem_base), "r"(P_TMEM_ALLOC) : "memory");
 }
 
 }  // namespace

@@ -111,7 +111,7 @@ def test_policy_rollout_teacher_forced():
     g.rollout(T, ring_depth=T, obs_ring=obs_ring, rew_ring=rew_ring, done_ring=done_ring, actions_ring=act_ring,
               gov_actions_ring=gov_ring, pop_logits_ring=pl_ring, gov_logits_ring=gl_ring)
     torch.cuda.synchronize()
-    assert g.launch_count() - l0 == 1 + 3 * T   # observe + (pop policy, gov policy, step) per step
+    assert g.launch_count() - l0 == 1 + 2 * T   # observe + (policy kernel, step kernel) per step
     pop_obs, gov_obs = g.split_obs(obs_ring)
     pop_obs, gov_obs = pop_obs.cpu().numpy(), gov_obs.cpu().numpy()
     rew, done = rew_ring.cpu().numpy(), done_ring.cpu().numpy()
