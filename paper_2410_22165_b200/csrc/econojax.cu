@@ -218,6 +218,11 @@ int build_net(ej_env* h, const ej_mlp* m, const char* which, int in_dim, int n_h
     const int bias_bytes = align16((PH + PH + net.Op) * 4);
     net.blob_bytes = net.w1_bytes + net.w2_bytes + net.w3_bytes + bias_bytes;
     net.recipK1p = (uint32_t)((0x100000000ull + net.K1p - 1) / net.K1p);
+    net.nch = 0;
+    for (int hh = 0; hh < n_heads; ++hh) {
+        const int span = ((hh * head + head - 1) >> 4) - ((hh * head) >> 4) + 1;
+        if (span > net.nch) net.nch = span;
+    }
     if (policy_groups(net, in_dim + 3) < 1) return fail(h, EJ_ERR_PARAM, "bad field: %s (network does not fit in shared memory)", which);
     std::vector<uint8_t> blob(net.blob_bytes, 0);
     pack_operand(m->w1, PH, in_dim, PH, net.K1p, blob.data());

@@ -32,6 +32,7 @@ struct PolicyNet {
     int n_heads, head;     // categorical heads of `head` logits each (n_out = n_heads * head)
     int w1_bytes, w2_bytes, w3_bytes, blob_bytes;
     uint32_t recipK1p;     // ceil(2^32 / K1p)
+    int nch;               // 16-column chunks a head's logits span at most (register-resident sampler if <= 5)
 };
 
 struct PolicyArgs {
@@ -177,6 +178,128 @@ __device__ __forceinline__ void hidden_epilogue(uint32_t taddr_row, const float*
     }
 }
 
+template <int OFF, int LEN>
+__device__ __forceinline__ void tmem_ld16_async(uint32_t taddr, float (&r)[LEN]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];\n"
+        : "=f"(r[OFF + 0]), "=f"(r[OFF + 1]), "=f"(r[OFF + 2]), "=f"(r[OFF + 3]), "=f"(r[OFF + 4]), "=f"(r[OFF + 5]), "=f"(r[OFF + 6]),
+          "=f"(r[OFF + 7]), "=f"(r[OFF + 8]), "=f"(r[OFF + 9]), "=f"(r[OFF + 10]), "=f"(r[OFF + 11]), "=f"(r[OFF + 12]),
+          "=f"(r[OFF + 13]), "=f"(r[OFF + 14]), "=f"(r[OFF + 15])
+        : "r"(taddr)
+        : "memory");
+}
+
+template <int CH, int NCH>
+__device__ __forceinline__ void load_window(uint32_t taddr, int c0, int op, float (&l)[NCH * 16]) {
+    if constexpr (CH < NCH) {
+        if (c0 + 16 * CH < op) tmem_ld16_async<16 * CH>(taddr + c0 + 16 * CH, l);
+        else {
+#pragma unroll
+            for (int j = 0; j < 16; ++j) l[16 * CH + j] = 0.0f;
+        }
+        load_window<CH + 1, NCH>(taddr, c0, op, l);
+    }
+}
+
+// One categorical head whose logits span at most NCH 16-column chunks: the whole window is read
+// into registers once; maximum, exponentials, their sum and the cumulative search all run on
+// registers (masked columns carry -inf, whose exponential is 0).  Returns the sampled index.
+template <int NCH>
+__device__ __forceinline__ int sample_head(uint32_t taddr_row, const float* b3, int lo, int hi, int op, float u, float* logits_row) {
+    const int c0 = lo & ~15;
+    float l[NCH * 16];
+    load_window<0, NCH>(taddr_row, c0, op, l);
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+    float mx = -INFINITY;
+#pragma unroll
+    for (int ch = 0; ch < NCH; ++ch) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int col = c0 + 16 * ch + 4 * q;
+            float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (col < op) b = *reinterpret_cast<const float4*>(b3 + col);
+            const float bb[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int k = 16 * ch + 4 * q + j;
+                const bool in = (col + j >= lo) && (col + j < hi);
+                l[k] = in ? l[k] + bb[j] : -INFINITY;
+                mx = fmaxf(mx, l[k]);
+            }
+        }
+    }
+    if (logits_row) {
+#pragma unroll
+        for (int k = 0; k < NCH * 16; ++k)
+            if (c0 + k >= lo && c0 + k < hi) logits_row[c0 + k] = l[k];
+    }
+    const float mneg = -mx * 1.4426950408889634f;
+    float s = 0.0f;
+#pragma unroll
+    for (int k = 0; k < NCH * 16; ++k) {
+        l[k] = exp2f(__fmaf_rn(l[k], 1.4426950408889634f, mneg));  // exp(l - max); 0 for masked columns
+        s += l[k];
+    }
+    const float target = u * s;
+    float cum = 0.0f;
+    int below = 0;  // number of leading window slots whose cumulative weight is <= target
+#pragma unroll
+    for (int k = 0; k < NCH * 16; ++k) {
+        cum += l[k];
+        below += (cum <= target) ? 1 : 0;
+    }
+    int pick = c0 + below - lo;  // cum is non-decreasing: `below` slots precede the first index with target < cum
+    const int last = hi - lo - 1;
+    pick = pick < 0 ? 0 : pick;
+    return pick > last ? last : pick;
+}
+
+// Fallback for heads wider than 80 logits: three sweeps over the TMEM row (maximum; sum of
+// exp(l - max); first index whose cumulative weight exceeds u * sum).
+__device__ __forceinline__ int sample_head_sweeps(uint32_t taddr_row, const float* b3, int lo, int hi, float u, float* logits_row) {
+    float mx = -INFINITY;
+    for (int c = lo & ~15; c < hi; c += 16) {
+        float v[16];
+        tmem_ld16(taddr_row + c, v);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int col = c + j;
+            if (col >= lo && col < hi) {
+                const float l = v[j] + b3[col];
+                if (logits_row) logits_row[col] = l;
+                mx = fmaxf(mx, l);
+            }
+        }
+    }
+    float s = 0.0f;
+    for (int c = lo & ~15; c < hi; c += 16) {
+        float v[16];
+        tmem_ld16(taddr_row + c, v);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int col = c + j;
+            if (col >= lo && col < hi) s += __expf(v[j] + b3[col] - mx);
+        }
+    }
+    const float target = u * s;
+    float cum = 0.0f;
+    int pick = hi - lo - 1;
+    bool found = false;
+    for (int c = lo & ~15; c < hi; c += 16) {
+        float v[16];
+        tmem_ld16(taddr_row + c, v);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int col = c + j;
+            if (col >= lo && col < hi) {
+                cum += __expf(v[j] + b3[col] - mx);
+                if (!found && target < cum) { pick = col - lo; found = true; }
+            }
+        }
+    }
+    return pick;
+}
+
 __device__ __forceinline__ void group_sync(int grp) { asm volatile("bar.sync %0, %1;\n" ::"r"(grp + 1), "r"(PTILE) : "memory"); }
 
 // 1-D TMA bulk copy global -> shared, completion on an mbarrier (bytes and both addresses multiples of 16).
@@ -308,47 +431,15 @@ __global__ void __launch_bounds__(PGROUPS* PTILE, 1) ej_policy_kernel(const __gr
             const uint32_t xw = (h & 3) == 0 ? x[0] : (h & 3) == 1 ? x[1] : (h & 3) == 2 ? x[2] : x[3];
             const float u = u01(xw);
             const int lo = h * n.head, hi = lo + n.head;
-            // three sweeps over this thread's TMEM row, each a chain of independent operations:
-            // maximum; sum of exp(l - max); first index whose cumulative weight exceeds u * sum
-            float mx = -INFINITY;
-            for (int c = lo & ~15; c < hi; c += 16) {
-                float v[16];
-                tmem_ld16(taddr_row + c, v);
-#pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const int col = c + j;
-                    if (col >= lo && col < hi) {
-                        const float l = v[j] + b3[col];
-                        if (a.logits && live) a.logits[(size_t)row * n.n_out + col] = l;
-                        mx = fmaxf(mx, l);
-                    }
-                }
-            }
-            float s = 0.0f;
-            for (int c = lo & ~15; c < hi; c += 16) {
-                float v[16];
-                tmem_ld16(taddr_row + c, v);
-#pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const int col = c + j;
-                    if (col >= lo && col < hi) s += __expf(v[j] + b3[col] - mx);
-                }
-            }
-            const float target = u * s;
-            float cum = 0.0f;
-            int pick = n.head - 1;
-            bool found = false;
-            for (int c = lo & ~15; c < hi; c += 16) {
-                float v[16];
-                tmem_ld16(taddr_row + c, v);
-#pragma unroll
-                for (int j = 0; j < 16; ++j) {
-                    const int col = c + j;
-                    if (col >= lo && col < hi) {
-                        cum += __expf(v[j] + b3[col] - mx);
-                        if (!found && target < cum) { pick = col - lo; found = true; }
-                    }
-                }
+            float* lrow = (a.logits && live) ? a.logits + (size_t)row * n.n_out : nullptr;
+            int pick;
+            switch (n.nch) {
+                case 1: pick = sample_head<1>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                case 2: pick = sample_head<2>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                case 3: pick = sample_head<3>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                case 4: pick = sample_head<4>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                case 5: pick = sample_head<5>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                default: pick = sample_head_sweeps(taddr_row, b3, lo, hi, u, lrow); break;
             }
             if (live) a.actions[(size_t)row * n.n_heads + h] = pick;
         }
