@@ -68,24 +68,35 @@ int cuda_fail(ej_env* h, cudaError_t e, const char* where) {
         if (_e != cudaSuccess) return cuda_fail(h, _e, where);   \
     } while (0)
 
+// Kernel variants: CTA size NPAD (a power of two >= N) and stride NS of the per-agent arrays:
+// NPAD itself, or the tighter 13/16 NPAD when N fits (N = 100: 104 instead of 128, which is what
+// brings the headline shape from 7 to 8 resident CTAs per SM).
+constexpr int tight_stride(int npad) { return npad >= 64 ? npad / 16 * 13 : npad; }
+
+template <int NPAD, typename F>
+int for_stride(int ns, F&& f) {
+    if (ns == NPAD) return f(std::integral_constant<int, NPAD>(), std::integral_constant<int, NPAD>());
+    return f(std::integral_constant<int, NPAD>(), std::integral_constant<int, tight_stride(NPAD)>());
+}
+
 template <typename F>
-int for_block_size(int Npad, F&& f) {
+int for_variant(int Npad, int ns, F&& f) {
     switch (Npad) {
-        case 32: return f(std::integral_constant<int, 32>());
-        case 64: return f(std::integral_constant<int, 64>());
-        case 128: return f(std::integral_constant<int, 128>());
-        case 256: return f(std::integral_constant<int, 256>());
-        case 512: return f(std::integral_constant<int, 512>());
-        default: return f(std::integral_constant<int, 1024>());
+        case 32: return for_stride<32>(ns, f);
+        case 64: return for_stride<64>(ns, f);
+        case 128: return for_stride<128>(ns, f);
+        case 256: return for_stride<256>(ns, f);
+        case 512: return for_stride<512>(ns, f);
+        default: return for_stride<1024>(ns, f);
     }
 }
 
 // Shared-memory layout: the NP-only sections come from Lay<NP> (compile-time constants shared
 // with the kernels); the R-, P-, M-dependent sections are placed here.
 void build_layout(DevCfg& c) {
-    const int NP = c.Npad, R = c.R, nl = c.n_levels;
-    for_block_size(NP, [&](auto mt) {
-        using L = Lay<decltype(mt)::value>;
+    const int NP = c.N4, R = c.R, nl = c.n_levels;  // NP: stride of the per-agent arrays
+    for_variant(c.Npad, NP, [&](auto, auto ns) {
+        using L = Lay<decltype(ns)::value>;
         c.o_key = L::key; c.o_cslot = L::cslot; c.o_anext = L::anext; c.o_cinfo = L::anext; c.o_credit = L::credit;
         c.o_sale = L::sale; c.o_resq = L::resq; c.o_shrow = L::shrow; c.o_govrow = L::govrow; c.o_misc = L::misc;
         c.o_blob = L::blob;
@@ -142,9 +153,9 @@ void build_layout(DevCfg& c) {
 
 int launch_step(ej_env* h, const StepIO& io) {
     const DevCfg& c = h->c;
-    return for_block_size(c.Npad, [&](auto mt) {
-        constexpr int MT = decltype(mt)::value;
-        ej_step_kernel<MT><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, io);
+    return for_variant(c.Npad, c.N4, [&](auto mt, auto ns) {
+        constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
+        ej_step_kernel<MT, NS><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, io);
         h->launches++;
         EJ_CUDA(h, cudaGetLastError(), "ej_step_kernel launch");
         return EJ_OK;
@@ -153,11 +164,11 @@ int launch_step(ej_env* h, const StepIO& io) {
 
 int set_smem_attr(ej_env* h) {
     const DevCfg& c = h->c;
-    return for_block_size(c.Npad, [&](auto mt) {
-        constexpr int MT = decltype(mt)::value;
-        EJ_CUDA(h, cudaFuncSetAttribute(ej_step_kernel<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step)");
-        EJ_CUDA(h, cudaFuncSetAttribute(ej_observe_kernel<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (observe)");
-        EJ_CUDA(h, cudaFuncSetAttribute(ej_reset_kernel<MT>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (reset)");
+    return for_variant(c.Npad, c.N4, [&](auto mt, auto ns) {
+        constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
+        EJ_CUDA(h, cudaFuncSetAttribute(ej_step_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step)");
+        EJ_CUDA(h, cudaFuncSetAttribute(ej_observe_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (observe)");
+        EJ_CUDA(h, cudaFuncSetAttribute(ej_reset_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (reset)");
         return EJ_OK;
     });
 }
@@ -299,9 +310,9 @@ int rollout_with_policy(ej_env* h, int T, const ej_rollout_io* rio, const StepIO
     float* pl_ring = rio ? rio->pop_logits_ring : nullptr;
     float* gl_ring = rio ? rio->gov_logits_ring : nullptr;
     // observation of the current state
-    int rc = for_block_size(c.Npad, [&](auto mt) {
-        constexpr int MT = decltype(mt)::value;
-        ej_observe_kernel<MT><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, h->d_pobs);
+    int rc = for_variant(c.Npad, c.N4, [&](auto mt, auto ns) {
+        constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
+        ej_observe_kernel<MT, NS><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, h->d_pobs);
         h->launches++;
         EJ_CUDA(h, cudaGetLastError(), "ej_observe_kernel launch");
         return EJ_OK;
@@ -393,7 +404,7 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     c.D_gov_pad = (c.D_gov + 3) & ~3;
     c.Npad = 32;
     while (c.Npad < N) c.Npad <<= 1;
-    c.N4 = c.Npad;  // stride of the per-agent arrays
+    c.N4 = (N <= tight_stride(c.Npad)) ? tight_stride(c.Npad) : c.Npad;  // stride of the per-agent arrays
     c.n_metrics = 3 + R;
     c.n_warps = c.Npad / 32;
     c.shrow_len = 5 * R + c.B + 2;
@@ -475,9 +486,9 @@ int ej_reset(ej_env* h, uint64_t seed) {
     DevCfg& c = h->c;
     c.seed_lo = (uint32_t)(seed & 0xFFFFFFFFull);
     c.seed_hi = (uint32_t)(seed >> 32);
-    int rc = for_block_size(c.Npad, [&](auto mt) {
-        constexpr int MT = decltype(mt)::value;
-        ej_reset_kernel<MT><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state);
+    int rc = for_variant(c.Npad, c.N4, [&](auto mt, auto ns) {
+        constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
+        ej_reset_kernel<MT, NS><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state);
         h->launches++;
         EJ_CUDA(h, cudaGetLastError(), "ej_reset_kernel launch");
         return EJ_OK;
@@ -490,9 +501,9 @@ int ej_observe(ej_env* h, float* obs_out) {
     if (!h || !obs_out) return h ? fail(h, EJ_ERR_PARAM, "bad field: %s", "obs_out") : EJ_ERR_PARAM;
     if (!h->was_reset) return fail(h, EJ_ERR_STATE, "%s", "ej_observe before ej_reset / ej_set_state");
     const DevCfg& c = h->c;
-    return for_block_size(c.Npad, [&](auto mt) {
-        constexpr int MT = decltype(mt)::value;
-        ej_observe_kernel<MT><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, obs_out);
+    return for_variant(c.Npad, c.N4, [&](auto mt, auto ns) {
+        constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
+        ej_observe_kernel<MT, NS><<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, obs_out);
         h->launches++;
         EJ_CUDA(h, cudaGetLastError(), "ej_observe_kernel launch");
         return EJ_OK;

@@ -363,13 +363,13 @@ __device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm<NP>& m, int
 // the register sorting network.  ONE instance of this code per kernel (the caller loops over k
 // without unrolling): the unrolled network is most of the kernel's instruction footprint.
 //   mode 0 = step, 1 = finished env (reward 0), 2 = observe only
-template <int EPL>
-__device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<32 * EPL>& m, int k, int lane, int mode, int e, float* rew,
+template <int EPL, int NS>
+__device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, int k, int lane, int mode, int e, float* rew,
                                              int* hist) {
     const int N = c.N;
     const bool is_int = k >= 3;
     const float* farr = k == 0 ? m.coin() : k == 1 ? m.labor() : m.income();
-    const int* iarr = m.inv() + (is_int ? k - 3 : 0) * (32 * EPL);
+    const int* iarr = m.inv() + (is_int ? k - 3 : 0) * NS;
     float x[EPL];
     double s = 0.0;
     int si = 0, mx = 0;
@@ -498,12 +498,12 @@ __device__ __forceinline__ void write_timers(const DevCfg& c, const Sm<NP>& m, i
 //   mode     0 = step, 1 = finished env (rewards 0), 2 = observe only
 //   rows     0 = rewrite only the columns that change every step, 1 = also the tax rates,
 //            2 = every column (first step of a launch: skills)
-template <int NPAD>
-__device__ void outputs(const DevCfg& c, const Sm<NPAD>& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
+template <int NPAD, int NS>
+__device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
                         double cf_pre, float* obs, float* rew) {
     constexpr int NW = NPAD / 32, EPL = NPAD / 32;
     const int N = c.N, R = c.R;
-    constexpr int N4 = NPAD;  // stride of the per-agent arrays
+    constexpr int N4 = NS;  // stride of the per-agent arrays
     const bool act = tid < N;
     const int lane = tid & 31, warp = tid >> 5;
     const bool staged = c.stage_obs && obs;
@@ -553,7 +553,7 @@ __device__ void outputs(const DevCfg& c, const Sm<NPAD>& m, int tid, int e, int 
         const int first = it == 0 ? warp : 3 + (NW - 1 - warp), last = it == 0 ? 3 : c.n_metrics;
 #pragma unroll 1
         for (int k = first; k < last; k += NW)
-            metric_stats<EPL>(c, m, k, lane, mode, e, rew, m.hist() + (NW - 1 - warp) * HB);
+            metric_stats<EPL, NS>(c, m, k, lane, mode, e, rew, m.hist() + (NW - 1 - warp) * HB);
     }
     for (int k = tid; k < c.B + 2; k += NPAD) m.govrow()[3 * c.n_metrics + k] = m.shrow()[5 * R + k];
 
@@ -605,11 +605,11 @@ struct StepPtrs {
 // Phases P1-P4 of one environment step on the state in shared memory (G1: actions -> match ->
 // expire -> tax); returns the pre-step values the rewards need.  `first` = first step of this
 // launch (full observation rows).
-template <int NPAD>
-__device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NPAD>& m, int tid, int e, const StepPtrs& io, bool first, int t,
+template <int NPAD, int NS>
+__device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int tid, int e, const StepPtrs& io, bool first, int t,
                                           float& coin_pre, float& labor_pre, double& cf_pre, int& rows) {
     const int N = c.N, R = c.R, P = c.P, nl = c.n_levels;
-    constexpr int N4 = NPAD;  // stride of the per-agent arrays
+    constexpr int N4 = NS;  // stride of the per-agent arrays
     const bool act = tid < N;
     const uint32_t gid = c.env_id_base + (uint32_t)e;
     int* cnt_cur = m.cnt() + (t & 1) * nl;
@@ -973,8 +973,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NPAD>& m, in
 
 // One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
 // observations.  outputs() has this single call site (instruction footprint).
-template <int NPAD>
-__device__ void env_step(const DevCfg& c, const Sm<NPAD>& m, int tid, int e, const StepPtrs& io, bool first) {
+template <int NPAD, int NS>
+__device__ void env_step(const DevCfg& c, const Sm<NS>& m, int tid, int e, const StepPtrs& io, bool first) {
     const int t = m.hdr()->t;
     // the previous step's bulk stores must have read the staging tile before it is rewritten
     if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
@@ -988,26 +988,26 @@ __device__ void env_step(const DevCfg& c, const Sm<NPAD>& m, int tid, int e, con
         __syncthreads();
         mode = 1;
     } else {
-        step_body<NPAD>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
+        step_body<NPAD, NS>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
     }
     // ---------------- P5 rewards, P6 observations ----------------
-    outputs<NPAD>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs, io.rew);
+    outputs<NPAD, NS>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs, io.rew);
     if (mode == 1) {
         if (tid == 0 && io.done) io.done[e] = 1;
         __syncthreads();  // shrow is rewritten at the very start of the next finished step
     }
 }
 
-template <int NPAD>
+template <int NPAD, int NS>
 __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const StepIO io) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
-    uint8_t* const sblob = ej_smem + Lay<NPAD>::blob;
+    uint8_t* const sblob = ej_smem + Lay<NS>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
-    const Sm<NPAD> m{c};
+    const Sm<NS> m{c};
     uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
-    for (int i = tid; i < Lay<NPAD>::blob / 16; i += NPAD) ((uint4*)ej_smem)[i] = make_uint4(0u, 0u, 0u, 0u);
+    for (int i = tid; i < Lay<NS>::blob / 16; i += NPAD) ((uint4*)ej_smem)[i] = make_uint4(0u, 0u, 0u, 0u);
     for (int i = tid; i < (c.o_stage - c.o_scratch1) / 16; i += NPAD) ((uint4*)(ej_smem + c.o_scratch1))[i] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
     if (c.K == 0)
@@ -1027,7 +1027,7 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
     int slot = 0;
 #pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
-        env_step<NPAD>(c, m, tid, e, p, s == 0);
+        env_step<NPAD, NS>(c, m, tid, e, p, s == 0);
         if (p.actions) p.actions += EN;
         if (p.gov_actions) p.gov_actions += EB;
         if (++slot == io.ring_depth) {
@@ -1046,13 +1046,13 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
-template <int NPAD>
+template <int NPAD, int NS>
 __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant__ DevCfg c, const uint8_t* __restrict__ state,
                                                           float* obs) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
-    uint8_t* const sblob = ej_smem + Lay<NPAD>::blob;
+    uint8_t* const sblob = ej_smem + Lay<NS>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
-    const Sm<NPAD> m{c};
+    const Sm<NS> m{c};
     const uint4* blob = (const uint4*)(state + (size_t)e * c.blob_bytes);
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
     __syncthreads();
@@ -1061,17 +1061,17 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
     if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
     __syncthreads();
-    outputs<NPAD>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
+    outputs<NPAD, NS>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 // Reset (G29, G30): one CTA per env builds the blob in shared memory and stores it.
-template <int NPAD>
+template <int NPAD, int NS>
 __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
-    uint8_t* const sblob = ej_smem + Lay<NPAD>::blob;
+    uint8_t* const sblob = ej_smem + Lay<NS>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
-    const Sm<NPAD> m{c};
+    const Sm<NS> m{c};
     for (int i = tid; i < c.blob_bytes / 4; i += NPAD) ((uint32_t*)sblob)[i] = 0u;
     __syncthreads();
     const uint32_t gid = c.env_id_base + (uint32_t)e;
@@ -1090,7 +1090,7 @@ __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ 
                 if (v < c.clip_lo) v = c.clip_lo;
                 if (v > c.clip_hi) v = c.clip_hi;
             }
-            if (d < c.R) m.SG()[d * NPAD + tid] = v;
+            if (d < c.R) m.SG()[d * NS + tid] = v;
             else m.SC()[tid] = v;
         }
     }
