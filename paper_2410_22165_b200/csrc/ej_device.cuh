@@ -470,11 +470,12 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, i
 }
 
 // Shared tail of the population rows: market statistics of the post-step books.
-template <int NP>
+template <int PT, int NP>
 __device__ __forceinline__ void write_market_row(const DevCfg& c, const Sm<NP>& m, int r, const int* cnt) {
+    const int P = PT > 0 ? PT : c.P;
     int best_bid = 0, best_ask = 0, nb = 0, na = 0;
-    for (int p = 0; p < c.P; ++p) {
-        const int cb = cnt[(r * 2 + 0) * c.P + p], ca = cnt[(r * 2 + 1) * c.P + p];
+    for (int p = 0; p < P; ++p) {
+        const int cb = cnt[(r * 2 + 0) * P + p], ca = cnt[(r * 2 + 1) * P + p];
         nb += cb;
         na += ca;
         if (cb > 0) best_bid = c.prices[p];
@@ -498,11 +499,11 @@ __device__ __forceinline__ void write_timers(const DevCfg& c, const Sm<NP>& m, i
 //   mode     0 = step, 1 = finished env (rewards 0), 2 = observe only
 //   rows     0 = rewrite only the columns that change every step, 1 = also the tax rates,
 //            2 = every column (first step of a launch: skills)
-template <int NPAD, int NS>
+template <int NPAD, int NS, int RT>
 __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
                         double cf_pre, float* obs, float* rew) {
     constexpr int NW = NPAD / 32, EPL = NPAD / 32;
-    const int N = c.N, R = c.R;
+    const int N = c.N, R = RT > 0 ? RT : c.R;  // RT > 0: resource count known at compile time (loops unroll)
     constexpr int N4 = NS;  // stride of the per-agent arrays
     const bool act = tid < N;
     const int lane = tid & 31, warp = tid >> 5;
@@ -605,10 +606,11 @@ struct StepPtrs {
 // Phases P1-P4 of one environment step on the state in shared memory (G1: actions -> match ->
 // expire -> tax); returns the pre-step values the rewards need.  `first` = first step of this
 // launch (full observation rows).
-template <int NPAD, int NS>
+template <int NPAD, int NS, int RT, int PT>
 __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int tid, int e, const StepPtrs& io, bool first, int t,
                                           float& coin_pre, float& labor_pre, double& cf_pre, int& rows) {
-    const int N = c.N, R = c.R, P = c.P, nl = c.n_levels;
+    // RT, PT > 0: resource and price counts known at compile time (shape-specialised variants)
+    const int N = c.N, R = RT > 0 ? RT : c.R, P = PT > 0 ? PT : c.P, nl = (RT > 0 && PT > 0) ? 2 * RT * PT : c.n_levels;
     constexpr int N4 = NS;  // stride of the per-agent arrays
     const bool act = tid < N;
     const uint32_t gid = c.env_id_base + (uint32_t)e;
@@ -701,7 +703,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
         } else if (a < c.base_sell + R * P) {  // market order
             side_c = a >= c.base_sell;
             const int k = a - (side_c ? c.base_sell : c.base_buy);
-            r_c = (k * c.recipP) >> 16;
+            r_c = PT > 0 ? k / (PT > 0 ? PT : 1) : (k * c.recipP) >> 16;
             const int pidx = k - r_c * P;
             price_c = c.prices[pidx];
             bool ok = __popc(mymask) < c.M;
@@ -827,7 +829,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
     // One thread per level.  Trades of a resource: q = max_p min(#bids >= p, #asks <= p); the
     // q best bids and q best asks are popped from the queue heads, then the expired heads.
     for (int l = tid; l < nl; l += NPAD) {
-        const int book = (l * c.recipP) >> 16, pidx = l - book * P, r = book >> 1, side = book & 1;
+        const int book = PT > 0 ? l / (PT > 0 ? PT : 1) : (l * c.recipP) >> 16, pidx = l - book * P, r = book >> 1, side = book & 1;
         const int price = c.prices[pidx];
         const int lb = (r * 2) * P, la = lb + P;
         int totB = 0;
@@ -922,7 +924,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
         if (sl > 0) { m.income()[tid] = __fadd_rn(m.income()[tid], (float)sl); m.sale()[tid] = 0; }
         if (cr > 0) { m.coin()[tid] = __fadd_rn(m.coin()[tid], (float)cr); m.credit()[tid] = 0; }
     }
-    if (tid >= NPAD - R) write_market_row(c, m, NPAD - 1 - tid, cnt_nxt);
+    if (tid >= NPAD - R) write_market_row<PT>(c, m, NPAD - 1 - tid, cnt_nxt);
     if (tid == 0) write_timers(c, m, t + 1, period_end ? 0 : tp + 1);
 
     // ---------------- P4 tax at period end (G17-G20) ----------------
@@ -973,7 +975,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
 
 // One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
 // observations.  outputs() has this single call site (instruction footprint).
-template <int NPAD, int NS>
+template <int NPAD, int NS, int RT, int PT>
 __device__ void env_step(const DevCfg& c, const Sm<NS>& m, int tid, int e, const StepPtrs& io, bool first) {
     const int t = m.hdr()->t;
     // the previous step's bulk stores must have read the staging tile before it is rewritten
@@ -982,23 +984,23 @@ __device__ void env_step(const DevCfg& c, const Sm<NS>& m, int tid, int e, const
     double cf_pre = 0.0;
     int mode = 0, rows = 2;
     if (t >= c.T) {  // G28: finished env
-        if (tid < c.R) write_market_row(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
+        if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
         if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
         if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
         __syncthreads();
         mode = 1;
     } else {
-        step_body<NPAD, NS>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
+        step_body<NPAD, NS, RT, PT>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
     }
     // ---------------- P5 rewards, P6 observations ----------------
-    outputs<NPAD, NS>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs, io.rew);
+    outputs<NPAD, NS, RT>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs, io.rew);
     if (mode == 1) {
         if (tid == 0 && io.done) io.done[e] = 1;
         __syncthreads();  // shrow is rewritten at the very start of the next finished step
     }
 }
 
-template <int NPAD, int NS>
+template <int NPAD, int NS, int RT, int PT>
 __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const StepIO io) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
@@ -1027,7 +1029,7 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
     int slot = 0;
 #pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
-        env_step<NPAD, NS>(c, m, tid, e, p, s == 0);
+        env_step<NPAD, NS, RT, PT>(c, m, tid, e, p, s == 0);
         if (p.actions) p.actions += EN;
         if (p.gov_actions) p.gov_actions += EB;
         if (++slot == io.ring_depth) {
@@ -1057,11 +1059,11 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
     __syncthreads();
     const int t = m.hdr()->t;
-    if (tid < c.R) write_market_row(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
+    if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
     if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
     if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
     __syncthreads();
-    outputs<NPAD, NS>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
+    outputs<NPAD, NS, 0>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 

@@ -133,6 +133,25 @@ def test_paper_price_grid_and_defaults():
         pair.step_and_compare(acts[t], gov[t], "defaults t=%d" % t, check_state=(t % 10 == 0))
 
 
+@pytest.mark.parametrize("N,R,prices", [(100, 4, [3, 6, 9]), (100, 2, [2, 4, 6, 8, 10]), (100, 12, [3, 6, 9]), (60, 5, list(range(1, 11))),
+                                        (1000, 3, [3, 6, 9])])
+def test_shapes_of_generic_and_specialised_kernels(N, R, prices):
+    # the step kernel has shape-specialised variants (R, P compile-time) for BASELINE.json's shapes and a
+    # generic one for everything else: the paper's section-5 shapes (r = 4 and r = 12 with prices {3,6,9}:
+    # 30 and 86 actions) and other odd shapes run the generic kernel, [2..10] at R = 2 a specialised one
+    p = inputs.default_params()
+    p.update(prices=prices, episode_length=60, tax_period=20, thresholds=inputs.THRESHOLDS_7, skill_init=inputs.SKILL_PARETO_CLIP,
+             craft_distinct=2)
+    E = 2 if N == 1000 else 4
+    cfg = dict(E=E, N=N, R=R, T=60, seed=9, action_mix="uniform", params=p)
+    pair = Pair(E, N, R, p, 9)
+    if R in (4, 12) and len(prices) == 3:
+        assert pair.g.A == {4: 30, 12: 86}[R]
+    acts, gov = inputs.action_stream(cfg, 60, seed=9, E=E)
+    for t in range(60):
+        pair.step_and_compare(acts[t], gov[t], "shape N=%d R=%d P=%d t=%d" % (N, R, len(prices), t), check_state=(t % 10 == 0 or t == 59))
+
+
 # ---------------- scripted worked examples, seeded into the GPU through the canonical dump ----------------
 def _scripted(N, R, params, setup, steps):
     """setup(oracle_env) scripts the oracle; its dump is loaded into the GPU env; both then step."""
