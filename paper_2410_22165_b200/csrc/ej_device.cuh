@@ -556,7 +556,7 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
         for (int k = first; k < last; k += NW)
             metric_stats<EPL, NS>(c, m, k, lane, mode, e, rew, m.hist() + (NW - 1 - warp) * HB);
     }
-    for (int k = tid; k < c.B + 2; k += NPAD) m.govrow()[3 * c.n_metrics + k] = m.shrow()[5 * R + k];
+    if (tid < c.B + 2) m.govrow()[3 * c.n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
 
     if (obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
@@ -593,14 +593,19 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
     }
 }
 
+// Inputs and outputs of step `s` of a launch (ring slot `slot`), resolved where they are used:
+// keeping seven running pointers alive in every thread cost ~6 % of the executed instructions.
 struct StepPtrs {
-    const int32_t* actions;
-    const int32_t* gov_actions;
-    float* obs;
-    float* rew;
-    uint8_t* done;
-    int32_t* actions_out;
-    int32_t* gov_out;
+    const StepIO& io;
+    const DevCfg& c;
+    int s, slot;
+    __device__ __forceinline__ const int32_t* actions() const { return io.actions ? io.actions + (size_t)s * c.E * c.N : nullptr; }
+    __device__ __forceinline__ const int32_t* gov_actions() const { return io.gov_actions ? io.gov_actions + (size_t)s * c.E * c.B : nullptr; }
+    __device__ __forceinline__ float* obs() const { return io.obs ? io.obs + (size_t)slot * c.obs_floats : nullptr; }
+    __device__ __forceinline__ float* rew() const { return io.rew ? io.rew + (size_t)slot * c.E * (c.N + 1) : nullptr; }
+    __device__ __forceinline__ uint8_t* done() const { return io.done ? io.done + (size_t)slot * c.E : nullptr; }
+    __device__ __forceinline__ int32_t* actions_out() const { return io.actions_out ? io.actions_out + (size_t)slot * c.E * c.N : nullptr; }
+    __device__ __forceinline__ int32_t* gov_out() const { return io.gov_out ? io.gov_out + (size_t)slot * c.E * c.B : nullptr; }
 };
 
 // Phases P1-P4 of one environment step on the state in shared memory (G1: actions -> match ->
@@ -622,8 +627,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
     int a = -1;
     if (act) {
         philox4x32_10(gid, (uint32_t)tid, (uint32_t)t, 0u, c.seed_lo, c.seed_hi, x0, x1, x2, x3);
-        if (io.actions) {
-            a = io.actions[(size_t)e * N + tid];
+        if (io.io.actions) {
+            a = io.actions()[(size_t)e * N + tid];
         } else {  // smallest a with x0 < cdf[a]; last entry read as 2^32 (G30)
             int lo = 0, hi = c.A - 1;
             while (lo < hi) {
@@ -633,7 +638,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             }
             a = lo;
         }
-        if (io.actions_out) io.actions_out[(size_t)e * N + tid] = a;
+        if (io.io.actions_out) io.actions_out()[(size_t)e * N + tid] = a;
         m.key()[tid] = x2;
     }
     // government levels for the period boundary
@@ -641,16 +646,16 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
     const int tp = m.hdr()->t_in_period;
     const bool period_end = tp + 1 == c.period;
     const bool boundary = c.taxes_enabled && period_end;
-    if (tid < c.B && (boundary || io.gov_out)) {
-        if (io.gov_actions) {
-            gov_lvl = io.gov_actions[(size_t)e * c.B + tid];
+    if (tid < c.B && (boundary || io.io.gov_out)) {
+        if (io.io.gov_actions) {
+            gov_lvl = io.gov_actions()[(size_t)e * c.B + tid];
         } else {
             uint32_t g0, g1, g2, g3;
             philox4x32_10(gid, (uint32_t)N, (uint32_t)t, (uint32_t)(1 + tid / 4), c.seed_lo, c.seed_hi, g0, g1, g2, g3);
             const uint32_t gx = (tid & 3) == 0 ? g0 : (tid & 3) == 1 ? g1 : (tid & 3) == 2 ? g2 : g3;
             gov_lvl = (int)(((unsigned long long)gx * (unsigned long long)c.L) >> 32);
         }
-        if (io.gov_out) io.gov_out[(size_t)e * c.B + tid] = gov_lvl;
+        if (io.io.gov_out) io.gov_out()[(size_t)e * c.B + tid] = gov_lvl;
     }
 
     int lvl = -1, grp = 0, pos = 0, price_c = 0, r_c = 0, side_c = 0;
@@ -967,7 +972,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
         m.hdr()->t = t + 1;
         m.hdr()->t_in_period = period_end ? 0 : tp + 1;
         if (boundary) m.misc()[0] = 0ull;
-        if (io.done) io.done[e] = (uint8_t)(t + 1 == c.T);
+        if (io.io.done) io.done()[e] = (uint8_t)(t + 1 == c.T);
     }
 
     rows = first ? 2 : (boundary ? 1 : 0);
@@ -993,16 +998,16 @@ __device__ void env_step(const DevCfg& c, const Sm<NS>& m, int tid, int e, const
         step_body<NPAD, NS, RT, PT>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
     }
     // ---------------- P5 rewards, P6 observations ----------------
-    outputs<NPAD, NS, RT>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs, io.rew);
+    outputs<NPAD, NS, RT>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs(), io.rew());
     if (mode == 1) {
-        if (tid == 0 && io.done) io.done[e] = 1;
+        if (tid == 0 && io.io.done) io.done()[e] = 1;
         __syncthreads();  // shrow is rewritten at the very start of the next finished step
     }
 }
 
 template <int NPAD, int NS, int RT, int PT>
 __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
-                                                       const StepIO io) {
+                                                       const __grid_constant__ StepIO io) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
     uint8_t* const sblob = ej_smem + Lay<NS>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
@@ -1017,31 +1022,12 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
     if (!io.actions)
         for (int i = tid; i < c.A; i += NPAD) m.cdf()[i] = io.cdf[i];
     __syncthreads();
-    const size_t EN = (size_t)c.E * c.N, EB = (size_t)c.E * c.B;
-    StepPtrs p;  // running pointers: ring slot `slot` of every output
-    p.actions = io.actions;
-    p.gov_actions = io.gov_actions;
-    p.obs = io.obs;
-    p.rew = io.rew;
-    p.done = io.done;
-    p.actions_out = io.actions_out;
-    p.gov_out = io.gov_out;
-    int slot = 0;
+    StepPtrs p{io, c, 0, 0};
 #pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
+        p.s = s;
         env_step<NPAD, NS, RT, PT>(c, m, tid, e, p, s == 0);
-        if (p.actions) p.actions += EN;
-        if (p.gov_actions) p.gov_actions += EB;
-        if (++slot == io.ring_depth) {
-            slot = 0;
-            p.obs = io.obs; p.rew = io.rew; p.done = io.done; p.actions_out = io.actions_out; p.gov_out = io.gov_out;
-        } else {
-            if (p.obs) p.obs += c.obs_floats;
-            if (p.rew) p.rew += EN + c.E;
-            if (p.done) p.done += c.E;
-            if (p.actions_out) p.actions_out += EN;
-            if (p.gov_out) p.gov_out += EB;
-        }
+        p.slot = (p.slot + 1 == io.ring_depth) ? 0 : p.slot + 1;
     }
     __syncthreads();
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)sblob)[i];
