@@ -166,10 +166,12 @@ __device__ __forceinline__ void hidden_epilogue(uint32_t taddr_row, const float*
 #pragma unroll
         for (int g = 0; g < 4; ++g) {
             uint32_t w[4];
+            const float4 bl = *reinterpret_cast<const float4*>(bias + c + g * 8), bh = *reinterpret_cast<const float4*>(bias + c + g * 8 + 4);
+            const float bb[8] = {bl.x, bl.y, bl.z, bl.w, bh.x, bh.y, bh.z, bh.w};
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
                 const int k = g * 8 + 2 * j;
-                const float a0 = tanh_fast(__uint_as_float(r[k]) + bias[c + k]), a1 = tanh_fast(__uint_as_float(r[k + 1]) + bias[c + k + 1]);
+                const float a0 = tanh_fast(__uint_as_float(r[k]) + bb[2 * j]), a1 = tanh_fast(__uint_as_float(r[k + 1]) + bb[2 * j + 1]);
                 const __nv_bfloat162 h = __floats2bfloat162_rn(a0, a1);
                 w[j] = *reinterpret_cast<const uint32_t*>(&h);
             }
