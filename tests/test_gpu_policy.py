@@ -184,3 +184,55 @@ def test_policy_error_paths():
     env.set_policy(None, None)
     with pytest.raises(binding.EjError):
         env.policy_act(obs)
+
+
+def test_full_size_config5_sampled_envs():
+    """BASELINE.json configs[4] at full size (E=2048, N=100, R=3) in the launch configuration bench.py
+    times (policy kernel + step kernel per step, output rings); sampled envs are teacher-forced through
+    1-env oracles keyed by global env id, their logits and samples re-checked."""
+    import torch
+
+    cfg = inputs.configs()["config5_policy"]
+    N, R, E, T, depth = cfg["N"], cfg["R"], cfg["E"], 24, 24
+    ids = [0, 1, 127, 128, 1023, 2046, 2047]
+    pair = Pair(E, N, R, cfg["params"], cfg["seed"], env_ids=ids)
+    g = pair.g
+    pop, gov = inputs.policy_weights(cfg, seed=cfg["seed"])   # the weights bench.py installs
+    g.set_policy(pop, gov)
+    obs_ring, rew_ring, done_ring = g.new_obs(depth), g.new_rew(depth), g.new_done(depth)
+    act_ring = torch.zeros((depth, E, N), dtype=torch.int32, device="cuda")
+    gov_ring = torch.zeros((depth, E, g.B), dtype=torch.int32, device="cuda")
+    pl_ring = torch.zeros((depth, E * N, g.A), dtype=torch.float32, device="cuda")
+    gl_ring = torch.zeros((depth, E, g.B * g.L), dtype=torch.float32, device="cuda")
+    g.rollout(T, ring_depth=depth, obs_ring=obs_ring, rew_ring=rew_ring, done_ring=done_ring, actions_ring=act_ring,
+              gov_actions_ring=gov_ring, pop_logits_ring=pl_ring, gov_logits_ring=gl_ring)
+    torch.cuda.synchronize()
+    pop_obs, gov_obs = g.split_obs(obs_ring)
+    pop_obs, gov_obs = pop_obs[:, ids].cpu().numpy(), gov_obs[:, ids].cpu().numpy()
+    rew, done = rew_ring[:, ids].cpu().numpy(), done_ring[:, ids].cpu().numpy()
+    a_out, g_out = act_ring[:, ids].cpu().numpy(), gov_ring[:, ids].cpu().numpy()
+    pl = pl_ring.reshape(depth, E, N, g.A)[:, ids].cpu().numpy()
+    gl = gl_ring[:, ids].cpu().numpy()
+    outs = [o.observe() for o in pair.o]
+    o_pop, o_gov = np.concatenate([x[0] for x in outs]), np.concatenate([x[1] for x in outs])
+    amb = tot = 0
+    for t in range(T):
+        ol_pop = OP.mlp_logits(pop, o_pop.reshape(len(ids) * N, -1)).reshape(len(ids), N, -1)
+        ol_gov = OP.mlp_logits(gov, o_gov.reshape(len(ids), -1))
+        check_logits(pl[t], ol_pop, "t=%d population logits" % t)
+        check_logits(gl[t], ol_gov, "t=%d government logits" % t)
+        if t % 6 == 0 or t == T - 1:
+            a_, t_ = check_samples(cfg["seed"], ids, N, [t] * len(ids), ol_pop, ol_gov, a_out[t], g_out[t], g.B, g.L, "t=%d" % t)
+            amb, tot = amb + a_, tot + t_
+        o_pop, o_gov, o_rew, o_done = _teacher_step(pair, a_out[t], g_out[t])
+        compare_outputs(g, pop_obs[t], gov_obs[t], rew[t], done[t], o_pop, o_gov, o_rew, o_done, "config5 full size t=%d" % t)
+    compare_state(pair.g_state(), pair.o_state(), "config5 full size final state")
+    assert amb <= max(2, 0.01 * tot)
+    an = act_ring.cpu().numpy()
+    assert an.min() >= 0 and an.max() < g.A
+
+
+def _teacher_step(pair, acts_sel, gov_sel):
+    """Step the 1-env oracles of a sampled-env Pair with already-selected action rows."""
+    outs = [o.step(acts_sel[k:k + 1], gov_sel[k:k + 1]) for k, o in enumerate(pair.o)]
+    return tuple(np.concatenate([x[j] for x in outs]) for j in range(4))
