@@ -96,6 +96,7 @@ def lib():
             L.orc_observe.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
             L.orc_step.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.c_void_p] * 6
             L.orc_draw_actions.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
+            L.orc_action_mask.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
             L.orc_state_words.argtypes = [C.c_void_p]; L.orc_state_words.restype = C.c_size_t
             L.orc_get_state.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
             L.orc_set_agent.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_float, i32p, f32p, C.c_float]
@@ -187,6 +188,13 @@ class OracleEnv:
         gov = np.zeros((n, self.B), np.int32)
         self.L.orc_draw_actions(self.h, env_begin, n, _ptr(cdf), _ptr(actions), _ptr(gov))
         return actions, gov
+
+    def action_mask(self, env_begin=0, env_count=None):
+        """[n][N][A] uint8, 1 = action available in the current state (f1)."""
+        n = self.E - env_begin if env_count is None else env_count
+        m = np.zeros((n, self.N, self.A), np.uint8)
+        self.L.orc_action_mask(self.h, env_begin, n, _ptr(m))
+        return m
 
     def get_state(self, env_begin=0, env_count=None):
         n = self.E - env_begin if env_count is None else env_count

@@ -744,3 +744,49 @@ float orc_get_agent_f(const orc_sim* s, int32_t env, int32_t agent, int32_t what
     const orc_env* v = &s->env[env];
     return what == 0 ? v->coin[agent] : what == 1 ? v->labor[agent] : v->income[agent];
 }
+
+/* f1: action mask ("unavailable actions ... zero probability"; the availability
+ * rules are P:199 "cannot sell a resource it does not have" plus the action preconditions of
+ * P:145-168 and the order cap P:277).  Plain definition, one action at a time:
+ *   gather r            always available
+ *   craft               #{r : inv[r] >= R_kappa} >= R_d  (PER_RESOURCE r: inv[r] >= R_kappa)
+ *   buy (r, price)      coin >= price  and  live orders < M
+ *   sell (r, price)     inv[r] >= 1    and  live orders < M
+ *   no-op               always available
+ * The per-book cap K (G15) depends on the arrival order of the step and is not part of the mask.
+ * Writes A bytes (0 / 1) per agent: mask[env_count][N][A]. */
+void orc_action_mask(const orc_sim* s, int32_t env_begin, int32_t env_count, uint8_t* mask) {
+    const orc_params* p = &s->p;
+    const int32_t N = s->N, R = s->R, P = p->num_prices;
+    const int32_t n_craft = (p->craft_mode == ORC_CRAFT_PER_RESOURCE) ? R : 1;
+    const int32_t base_buy = R + n_craft, base_sell = base_buy + R * P;
+    const int32_t A = orc_num_actions(R, P, p->craft_mode, p->allow_noop);
+    for (int32_t k = 0; k < env_count; ++k) {
+        const orc_env* v = &s->env[env_begin + k];
+        for (int32_t i = 0; i < N; ++i) {
+            uint8_t* m = mask + ((size_t)k * N + i) * A;
+            const int32_t room = v->n_live[i] < p->max_active_orders;
+            for (int32_t a = 0; a < A; ++a) {
+                int32_t ok;
+                if (a < R) {
+                    ok = 1;
+                } else if (a < base_buy) {
+                    if (p->craft_mode == ORC_CRAFT_PER_RESOURCE) {
+                        ok = v->inv[i * R + (a - R)] >= p->craft_units;
+                    } else {
+                        int32_t enough = 0;
+                        for (int32_t r = 0; r < R; ++r) enough += v->inv[i * R + r] >= p->craft_units;
+                        ok = enough >= p->craft_distinct;
+                    }
+                } else if (a < base_sell) {
+                    ok = room && v->coin[i] >= (float)p->prices[(a - base_buy) % P];
+                } else if (a < base_sell + R * P) {
+                    ok = room && v->inv[i * R + (a - base_sell) / P] >= 1;
+                } else {
+                    ok = 1;
+                }
+                m[a] = (uint8_t)ok;
+            }
+        }
+    }
+}
