@@ -152,6 +152,16 @@ int ej_reset(ej_env* h, uint64_t seed);
 /* Observation of the current state (e.g. right after reset) into obs_out (device, obs_floats). */
 int ej_observe(ej_env* h, float* obs_out);
 
+/* f1: action mask of the current state ("unavailable actions" get zero probability;
+ * P:199; action preconditions P:145-168; order cap P:277) into mask_out, device, [E][N][A] bytes,
+ * 1 = available, 4-byte aligned: gather and no-op always; craft iff #{r : inv[r] >= craft_units} >=
+ * craft_distinct (PER_RESOURCE r: inv[r] >= craft_units); buy (r, p) iff coin >= prices[p] and live
+ * orders < max_active_orders; sell (r, p) iff inv[r] >= 1 and live orders < max_active_orders.  With
+ * book_cap == 0 an action is available exactly when submitting it would not bump the env's `invalid`
+ * counter; the per-book cap depends on the step's arrival order and is not part of the mask (G15).
+ * Errors: EJ_ERR_PARAM (NULL / misaligned pointer), EJ_ERR_STATE (before reset), EJ_ERR_CUDA. */
+int ej_action_mask(ej_env* h, uint8_t* mask_out);
+
 /* One step of all E envs (order of effects G1: actions -> match -> expire -> tax -> rewards ->
  * observations -> t++).
  *  actions      device [E][N] int32 action indices (layout ej_layout_info.base_*)

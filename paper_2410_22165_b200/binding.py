@@ -70,7 +70,7 @@ class EjMlp(C.Structure):
 
 EXPORTS = ("ej_create", "ej_destroy", "ej_set_stream", "ej_layout", "ej_last_error", "ej_reset", "ej_observe",
            "ej_step", "ej_step_host", "ej_rollout", "ej_set_action_cdf", "ej_get_state", "ej_set_state",
-           "ej_launch_count", "ej_set_policy", "ej_policy_act")
+           "ej_launch_count", "ej_set_policy", "ej_policy_act", "ej_action_mask")
 
 _lib = None
 
@@ -91,6 +91,7 @@ def lib():
         L.ej_last_error.argtypes = [vp]; L.ej_last_error.restype = C.c_char_p
         L.ej_reset.argtypes = [vp, C.c_uint64]
         L.ej_observe.argtypes = [vp, vp]
+        L.ej_action_mask.argtypes = [vp, vp]
         L.ej_step.argtypes = [vp, vp, vp, vp, vp, vp]
         L.ej_step_host.argtypes = [vp, vp, vp, vp, vp, vp]
         L.ej_rollout.argtypes = [vp, C.c_int32, C.POINTER(EjRolloutIO)]
@@ -176,6 +177,10 @@ def ej_reset(h, seed: int):
 
 def ej_observe(h, obs_out: int):
     _check(h, lib().ej_observe(h, obs_out))
+
+
+def ej_action_mask(h, mask_out: int):
+    _check(h, lib().ej_action_mask(h, mask_out))
 
 
 def ej_step(h, actions: int, gov_actions: int, obs_out: int | None, rew_out: int | None, done_out: int | None):
@@ -294,6 +299,15 @@ class Env:
         obs = self.new_obs() if obs is None else obs
         ej_observe(self.h, obs.data_ptr())
         return obs
+
+    def action_mask(self, mask=None):
+        """f1: [E, N, A] uint8 availability mask of the current state."""
+        t = self.torch
+        if mask is None:
+            mask = t.empty((self.E, self.N, self.A), dtype=t.uint8, device=self.device)
+        assert mask.dtype == t.uint8 and mask.is_cuda and mask.is_contiguous() and mask.numel() == self.E * self.N * self.A
+        ej_action_mask(self.h, mask.data_ptr())
+        return mask
 
     def step(self, actions, gov_actions, obs=None, rew=None, done=None, want_obs=True):
         t = self.torch

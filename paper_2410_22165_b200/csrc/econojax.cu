@@ -530,6 +530,19 @@ int ej_observe(ej_env* h, float* obs_out) {
     });
 }
 
+int ej_action_mask(ej_env* h, uint8_t* mask_out) {
+    if (!h) return EJ_ERR_PARAM;
+    if (!mask_out || ((uintptr_t)mask_out & 3)) return fail(h, EJ_ERR_PARAM, "bad field: %s", "mask_out");
+    if (!h->was_reset) return fail(h, EJ_ERR_STATE, "%s", "ej_action_mask before ej_reset / ej_set_state");
+    const DevCfg& c = h->c;
+    const unsigned long long total = (unsigned long long)c.E * c.N * c.A;
+    const unsigned long long words = (total + 3) / 4;
+    ej_mask_kernel<<<(unsigned)((words + 255) / 256), 256, 0, h->stream>>>(c, h->d_state, mask_out, total);
+    h->launches++;
+    EJ_CUDA(h, cudaGetLastError(), "ej_mask_kernel launch");
+    return EJ_OK;
+}
+
 int ej_step(ej_env* h, const int32_t* actions, const int32_t* gov_actions, float* obs_out, float* rew_out, uint8_t* done_out) {
     if (!h) return EJ_ERR_PARAM;
     if (!actions) return fail(h, EJ_ERR_PARAM, "bad field: %s", "actions");

@@ -1104,4 +1104,52 @@ __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ 
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)sblob)[i];
 }
 
+// f1: action mask of the current state (unavailable actions get zero probability;
+// P:199 "cannot sell a resource it does not have"; preconditions of P:145-168; order cap P:277):
+//   gather, no-op: 1;  craft: #{r : inv[r] >= R_kappa} >= R_d (PER_RESOURCE r: inv[r] >= R_kappa);
+//   buy (r, p): coin >= price_p and live orders < M;  sell (r, p): inv[r] >= 1 and live orders < M.
+// The per-book cap K (G15) depends on the step's arrival order and is not part of the mask.
+// HBM-bound writer of [E][N][A] bytes: one thread per 4 output bytes (the flat byte index is
+// split into env / agent / action once, then carried), state read from the blob in HBM (a few
+// words per agent, L1/L2 hits); a 32-bit store per thread, coalesced.
+__global__ void __launch_bounds__(256) ej_mask_kernel(const __grid_constant__ DevCfg c, const uint8_t* __restrict__ state,
+                                                      uint8_t* __restrict__ mask_out, unsigned long long total) {
+    const unsigned long long w = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    unsigned long long g = w * 4ull;
+    if (g >= total) return;
+    const int A = c.A, N = c.N, R = c.R, P = c.P, NS = c.N4;
+    unsigned long long row = g / (unsigned long long)A;  // e * N + i
+    int a = (int)(g - row * (unsigned long long)A);
+    int e = (int)(row / (unsigned long long)N), i = (int)(row - (unsigned long long)e * N);
+    const int n_out = (total - g) < 4ull ? (int)(total - g) : 4;
+    uint32_t packed = 0;
+    const uint8_t* blob = state + (size_t)e * c.blob_bytes;
+    int cached_i = -1, cached_e = -1;
+    bool room = false, craft_ok = false;
+    float coin = 0.f;
+    for (int k = 0; k < n_out; ++k) {
+        if (i != cached_i || e != cached_e) {
+            blob = state + (size_t)e * c.blob_bytes;
+            coin = ((const float*)(blob + c.o_coin))[i];
+            room = __popc(((const uint32_t*)(blob + c.o_mask))[i]) < c.M;
+            int enough = 0;
+            const int* inv = (const int*)(blob + c.o_inv);
+            for (int r = 0; r < R; ++r) enough += inv[r * NS + i] >= c.craft_units;
+            craft_ok = enough >= c.craft_distinct;
+            cached_i = i; cached_e = e;
+        }
+        const int* inv = (const int*)(blob + c.o_inv);
+        bool ok;
+        if (a < R) ok = true;
+        else if (a < c.base_buy) ok = c.craft_mode == EJ_CRAFT_PER_RESOURCE ? inv[(a - R) * NS + i] >= c.craft_units : craft_ok;
+        else if (a < c.base_sell) ok = room && coin >= (float)c.prices[(a - c.base_buy) % P];
+        else if (a < c.base_sell + R * P) ok = room && inv[((a - c.base_sell) / P) * NS + i] >= 1;
+        else ok = true;
+        packed |= (ok ? 1u : 0u) << (8 * k);
+        if (++a == A) { a = 0; if (++i == N) { i = 0; ++e; } }
+    }
+    if (n_out == 4) *(uint32_t*)(mask_out + g) = packed;
+    else for (int k = 0; k < n_out; ++k) mask_out[g + k] = (uint8_t)(packed >> (8 * k));
+}
+
 }  // namespace
