@@ -84,6 +84,9 @@ int for_stride(int ns, F&& f) {
 
 template <typename F>
 int for_variant(int Npad, int ns, F&& f) {
+#ifdef EJ_DEV_ONLY_128  // development builds: only the N = 65..128 variants (build time)
+    return for_stride<128>(ns, f);
+#endif
     switch (Npad) {
         case 32: return for_stride<32>(ns, f);
         case 64: return for_stride<64>(ns, f);
@@ -160,16 +163,34 @@ void build_layout(DevCfg& c) {
 template <int MT, int NS>
 void select_step_kernel(ej_env* h) {
     const DevCfg& c = h->c;
-    h->step_fn = ej_step_kernel<MT, NS, 0, 0>;
+    h->step_fn = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0>;
     h->step_RT = h->step_PT = 0;
+    auto pick = [&](auto rt, auto pt, auto nt, auto bt) {
+        constexpr int RT = decltype(rt)::value, PT = decltype(pt)::value, NT = decltype(nt)::value, BT = decltype(bt)::value;
+        // NT > 0 variants also fix the paper's mechanics (PF = 1 in ej_device.cuh)
+        const bool paper = c.M == 15 && c.Mp_log2 == 4 && c.K == 0 && c.craft_mode == EJ_CRAFT_SINGLE && c.craft_units == 2 &&
+                           c.craft_distinct == 2 && c.allow_noop == 1 && c.stage_obs == 1;
+        if (c.R == RT && c.P == PT && (NT == 0 || (c.N == NT && c.B == BT && paper))) {
+            h->step_fn = ej_step_kernel<MT, NS, RT, PT, NT, BT, (NT > 0)>;
+            h->step_RT = RT; h->step_PT = PT;
+        }
+    };
+    using std::integral_constant;
     if constexpr (MT == 128) {
-        if (c.P == 10 && c.R == 2) { h->step_fn = ej_step_kernel<MT, NS, 2, 10>; h->step_RT = 2; h->step_PT = 10; }
-        if (c.P == 10 && c.R == 3) { h->step_fn = ej_step_kernel<MT, NS, 3, 10>; h->step_RT = 3; h->step_PT = 10; }
-        if (c.P == 10 && c.R == 6) { h->step_fn = ej_step_kernel<MT, NS, 6, 10>; h->step_RT = 6; h->step_PT = 10; }
-        if (c.P == 5 && c.R == 2) { h->step_fn = ej_step_kernel<MT, NS, 2, 5>; h->step_RT = 2; h->step_PT = 5; }
+        // BASELINE.json's N = 100 shapes: R, P, N and B are compile-time constants
+        if constexpr (NS == tight_stride(128)) {
+            pick(integral_constant<int, 2>(), integral_constant<int, 10>(), integral_constant<int, 100>(), integral_constant<int, 7>());
+#ifndef EJ_DEV_ONLY_128
+            pick(integral_constant<int, 3>(), integral_constant<int, 10>(), integral_constant<int, 100>(), integral_constant<int, 7>());
+            pick(integral_constant<int, 6>(), integral_constant<int, 10>(), integral_constant<int, 100>(), integral_constant<int, 7>());
+#endif
+        }
+#ifndef EJ_DEV_ONLY_128
+        if (h->step_RT == 0) pick(integral_constant<int, 2>(), integral_constant<int, 5>(), integral_constant<int, 0>(), integral_constant<int, 0>());
+#endif
     }
     if constexpr (MT == 1024 && NS == 1024) {
-        if (c.P == 10 && c.R == 2) { h->step_fn = ej_step_kernel<MT, NS, 2, 10>; h->step_RT = 2; h->step_PT = 10; }
+        pick(integral_constant<int, 2>(), integral_constant<int, 10>(), integral_constant<int, 0>(), integral_constant<int, 0>());
     }
 }
 

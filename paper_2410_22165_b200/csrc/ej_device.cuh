@@ -356,11 +356,13 @@ __device__ __forceinline__ bool walk_select(const float (&x)[EPL], int lane, int
     return true;
 }
 
-template <int NP>
+template <int NP, int NT>
 __device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm<NP>& m, int k, double mean, float q_sum, float lo, float hi,
                                            float scale) {
-    const float sd = __fsqrt_rn((float)((double)q_sum * c.inv_n));
-    const float med = (c.N & 1) ? hi : __fmul_rn(0.5f, __fadd_rn(lo, hi));
+    const int N = NT > 0 ? NT : c.N;
+    const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
+    const float sd = __fsqrt_rn((float)((double)q_sum * inv_n));
+    const float med = (N & 1) ? hi : __fmul_rn(0.5f, __fadd_rn(lo, hi));
     m.govrow()[3 * k + 0] = (float)(mean * (double)scale);
     m.govrow()[3 * k + 1] = __fmul_rn(sd, scale);
     m.govrow()[3 * k + 2] = __fmul_rn(med, scale);
@@ -374,10 +376,11 @@ __device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm<NP>& m, int
 // the register sorting network.  ONE instance of this code per kernel (the caller loops over k
 // without unrolling): the unrolled network is most of the kernel's instruction footprint.
 //   mode 0 = step, 1 = finished env (reward 0), 2 = observe only
-template <int EPL, int NS>
+template <int EPL, int NS, int NT>
 __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, int k, int lane, int mode, int e, float* rew,
                                              int* hist) {
-    const int N = c.N;
+    const int N = NT > 0 ? NT : c.N;  // NT > 0: population size known at compile time
+    const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
     const bool is_int = k >= 3;
     const float* farr = k == 0 ? m.coin() : k == 1 ? m.labor() : m.income();
     const int* iarr = m.inv() + (is_int ? k - 3 : 0) * NS;
@@ -407,7 +410,7 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, i
     } else {
         s = warp_sum(s);
     }
-    const double mean = s * c.inv_n;
+    const double mean = s * inv_n;
     float qs = 0.0f;
 #pragma unroll
     for (int q = 0; q < EPL; ++q) {
@@ -467,7 +470,7 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, i
             if (lane == 0) {
                 // u_g = (omega (1 - gini) + (1 - omega)) prod = prod - omega * gini * prod; gini = 0 when
                 // prod = 0 or N = 1 (then gn = 0 as well)
-                const double ug = s - (double)c.omega * (g * c.inv_n);
+                const double ug = s - (double)c.omega * (g * inv_n);
                 if (mode == 0) {
                     if (rew) rew[(size_t)e * (N + 1) + N] = (float)(ug - m.hdr()->u_g_prev);
                     m.hdr()->u_g_prev = ug;
@@ -477,7 +480,7 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, i
             }
         }
     }
-    if (lane == 0) gov_triple(c, m, k, mean, qs, lo, hi, is_int ? c.s_count : k == 1 ? c.s_labor : c.s_coin);
+    if (lane == 0) gov_triple<NS, NT>(c, m, k, mean, qs, lo, hi, is_int ? c.s_count : k == 1 ? c.s_labor : c.s_coin);
 }
 
 // Shared tail of the population rows: market statistics of the post-step books.
@@ -510,15 +513,18 @@ __device__ __forceinline__ void write_timers(const DevCfg& c, const Sm<NP>& m, i
 //   mode     0 = step, 1 = finished env (rewards 0), 2 = observe only
 //   rows     0 = rewrite only the columns that change every step, 1 = also the tax rates,
 //            2 = every column (first step of a launch: skills)
-template <int NPAD, int NS, int RT>
+template <int NPAD, int NS, int RT, int NT, int BT, int PF>
 __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
                         double cf_pre, float* obs, float* rew) {
     constexpr int NW = NPAD / 32, EPL = NPAD / 32;
-    const int N = c.N, R = RT > 0 ? RT : c.R;  // RT > 0: resource count known at compile time (loops unroll)
+    // RT, NT, BT > 0: resource count, population size, bracket count known at compile time
+    const int N = NT > 0 ? NT : c.N, R = RT > 0 ? RT : c.R, B = BT > 0 ? BT : c.B;
+    const int D_pop = (RT > 0 && BT > 0) ? 6 + 8 * RT + BT : c.D_pop;
     constexpr int N4 = NS;  // stride of the per-agent arrays
     const bool act = tid < N;
     const int lane = tid & 31, warp = tid >> 5;
-    const bool staged = c.stage_obs && obs;
+    const bool staged = (PF || c.stage_obs) && obs;
+    const int stage_alias_bytes = PF ? 2 * R * NS * 4 : c.stage_alias_bytes, n_metrics = RT > 0 ? 3 + RT : c.n_metrics;
 
     if (act) {
         const float coin = m.coin()[tid], labor = m.labor()[tid];
@@ -535,7 +541,7 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
         }
         // ---- this agent's observation row (G25) in the staging tile ----
         if (staged) {
-            float* o = m.stage() + tid * c.D_pop;
+            float* o = m.stage() + tid * D_pop;
             o[0] = __fmul_rn(coin, c.s_coin);
             for (int r = 0; r < R; ++r) o[1 + r] = __fmul_rn((float)m.inv()[r * N4 + tid], c.s_count);
             o[R + 1] = __fmul_rn((float)m.esc_coin()[tid], c.s_coin);
@@ -543,12 +549,12 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
             o[3 * R + 3] = __fmul_rn(labor, c.s_labor);
             float* tl = o + 3 * R + 4;
             for (int k = 0; k < 5 * R; ++k) tl[k] = m.shrow()[k];
-            tl[5 * R + c.B] = m.shrow()[5 * R + c.B];
-            tl[5 * R + c.B + 1] = m.shrow()[5 * R + c.B + 1];
+            tl[5 * R + B] = m.shrow()[5 * R + B];
+            tl[5 * R + B + 1] = m.shrow()[5 * R + B + 1];
             // rows whose bytes the matched-order lists reuse are rewritten in full every step
-            const int rows_eff = (tid * c.D_pop * 4 < c.stage_alias_bytes) ? 2 : rows;
+            const int rows_eff = (tid * D_pop * 4 < stage_alias_bytes) ? 2 : rows;
             if (rows_eff >= 1)
-                for (int b = 0; b < c.B; ++b) tl[5 * R + b] = m.shrow()[5 * R + b];
+                for (int b = 0; b < B; ++b) tl[5 * R + b] = m.shrow()[5 * R + b];
             if (rows_eff >= 2) {
                 for (int r = 0; r < R; ++r) o[2 * R + 2 + r] = m.SG()[r * N4 + tid];
                 o[3 * R + 2] = m.SC()[tid];
@@ -562,21 +568,21 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
     for (int it = 0; it < 2; ++it) {
         // it 0: float metrics k = warp, warp + NW, ... < 3; it 1: integer metrics of resources
         // r = NW-1-warp, + NW, ... < R.  One instance of metric_stats (instruction footprint).
-        const int first = it == 0 ? warp : 3 + (NW - 1 - warp), last = it == 0 ? 3 : c.n_metrics;
+        const int first = it == 0 ? warp : 3 + (NW - 1 - warp), last = it == 0 ? 3 : n_metrics;
 #pragma unroll 1
         for (int k = first; k < last; k += NW)
-            metric_stats<EPL, NS>(c, m, k, lane, mode, e, rew, m.hist() + (NW - 1 - warp) * HB);
+            metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew, m.hist() + (NW - 1 - warp) * HB);
     }
-    if (tid < c.B + 2) m.govrow()[3 * c.n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
+    if (tid < B + 2) m.govrow()[3 * n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
 
     if (obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 
     if (obs && tid == 0) {  // bulk stores: the env's contiguous [N][D_pop] tile and its government row
         if (staged) {
-            float* dst = obs + (size_t)e * N * c.D_pop;
+            float* dst = obs + (size_t)e * N * D_pop;
             const uint32_t src = (uint32_t)__cvta_generic_to_shared(m.stage());
-            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(N * c.D_pop * 4) : "memory");
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(N * D_pop * 4) : "memory");
         }
         float* gdst = obs + c.gov_obs_offset + (size_t)e * c.D_gov_pad;
         const uint32_t gsrc = (uint32_t)__cvta_generic_to_shared(m.govrow());
@@ -585,7 +591,7 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
     }
     // ---- population rows when they cannot go out as one bulk store: coalesced loop ----
     if (obs && !staged) {
-        const int D = c.D_pop, priv = 3 * R + 4, total = N * D;
+        const int D = D_pop, priv = 3 * R + 4, total = N * D;
         float* dst = obs + (size_t)e * total;
         for (int idx = tid; idx < total; idx += NPAD) {
             const int i = idx / D, k = idx - i * D;
@@ -622,11 +628,16 @@ struct StepPtrs {
 // Phases P1-P4 of one environment step on the state in shared memory (G1: actions -> match ->
 // expire -> tax); returns the pre-step values the rewards need.  `first` = first step of this
 // launch (full observation rows).
-template <int NPAD, int NS, int RT, int PT>
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF>
 __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int tid, int e, const StepPtrs& io, bool first, int t,
                                           float& coin_pre, float& labor_pre, double& cf_pre, int& rows) {
     // RT, PT > 0: resource and price counts known at compile time (shape-specialised variants)
-    const int N = c.N, R = RT > 0 ? RT : c.R, P = PT > 0 ? PT : c.P, nl = (RT > 0 && PT > 0) ? 2 * RT * PT : c.n_levels;
+    const int N = NT > 0 ? NT : c.N, B = BT > 0 ? BT : c.B, R = RT > 0 ? RT : c.R, P = PT > 0 ? PT : c.P, nl = (RT > 0 && PT > 0) ? 2 * RT * PT : c.n_levels;
+    // PF = 1: the paper's mechanics (Table 2: 15 live orders per agent, one craft action
+    // over R_d = R_kappa = 2, no-op on) with no book cap, as compile-time constants
+    const int K = PF ? 0 : c.K, M = PF ? 15 : c.M, MPL = PF ? 4 : c.Mp_log2;
+    const int craft_mode = PF ? EJ_CRAFT_SINGLE : c.craft_mode, craft_units = PF ? 2 : c.craft_units, craft_distinct = PF ? 2 : c.craft_distinct;
+    const int base_buy = PF ? R + 1 : c.base_buy, base_sell = PF ? R + 1 + R * P : c.base_sell, A = PF ? 2 * R * P + R + 2 : c.A;
     constexpr int N4 = NS;  // stride of the per-agent arrays
     const bool act = tid < N;
     const uint32_t gid = c.env_id_base + (uint32_t)e;
@@ -641,7 +652,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
         if (io.io.actions) {
             a = io.actions()[(size_t)e * N + tid];
         } else {  // smallest a with x0 < cdf[a]; last entry read as 2^32 (G30)
-            int lo = 0, hi = c.A - 1;
+            int lo = 0, hi = A - 1;
             while (lo < hi) {
                 const int mid = (lo + hi) >> 1;
                 if (x0 < m.cdf()[mid]) hi = mid;
@@ -657,16 +668,16 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
     const int tp = m.hdr()->t_in_period;
     const bool period_end = tp + 1 == c.period;
     const bool boundary = c.taxes_enabled && period_end;
-    if (tid < c.B && (boundary || io.io.gov_out)) {
+    if (tid < B && (boundary || io.io.gov_out)) {
         if (io.io.gov_actions) {
-            gov_lvl = io.gov_actions()[(size_t)e * c.B + tid];
+            gov_lvl = io.gov_actions()[(size_t)e * B + tid];
         } else {
             uint32_t g0, g1, g2, g3;
             philox4x32_10(gid, (uint32_t)N, (uint32_t)t, (uint32_t)(1 + tid / 4), c.seed_lo, c.seed_hi, g0, g1, g2, g3);
             const uint32_t gx = (tid & 3) == 0 ? g0 : (tid & 3) == 1 ? g1 : (tid & 3) == 2 ? g2 : g3;
             gov_lvl = (int)(((unsigned long long)gx * (unsigned long long)c.L) >> 32);
         }
-        if (io.io.gov_out) io.gov_out()[(size_t)e * c.B + tid] = gov_lvl;
+        if (io.io.gov_out) io.gov_out()[(size_t)e * B + tid] = gov_lvl;
     }
 
     int lvl = -1, grp = 0, pos = 0, price_c = 0, r_c = 0, side_c = 0;
@@ -677,26 +688,26 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
         cf_pre = m.cf()[tid];
         mymask = m.mask()[tid];
         bool invalid = false;
-        if (a < 0 || a >= c.A) {
+        if (a < 0 || a >= A) {
             invalid = true;  // G2
         } else if (a < R) {  // gather: floor(SG + rho), rho = u * 1.1 (G8)
             const float rho = __fmul_rn(u01(x1), 1.1f);
             const float s = __fadd_rn(m.SG()[a * N4 + tid], rho);
             m.inv()[a * N4 + tid] += (int)floorf(s);
             m.labor()[tid] = __fadd_rn(labor_pre, c.labor_gather);
-        } else if (a < c.base_buy) {  // craft
+        } else if (a < base_buy) {  // craft
             bool ok;
-            if (c.craft_mode == EJ_CRAFT_PER_RESOURCE) {
+            if (craft_mode == EJ_CRAFT_PER_RESOURCE) {
                 const int r = a - R;
-                ok = m.inv()[r * N4 + tid] >= c.craft_units;
-                if (ok) m.inv()[r * N4 + tid] -= c.craft_units;
+                ok = m.inv()[r * N4 + tid] >= craft_units;
+                if (ok) m.inv()[r * N4 + tid] -= craft_units;
             } else {
                 int enough = 0;
-                for (int r = 0; r < R; ++r) enough += m.inv()[r * N4 + tid] >= c.craft_units;
-                ok = enough >= c.craft_distinct;
+                for (int r = 0; r < R; ++r) enough += m.inv()[r * N4 + tid] >= craft_units;
+                ok = enough >= craft_distinct;
                 if (ok) {  // the R_d most-held resources, ties to the lowest index (G7)
                     uint32_t used = 0;
-                    for (int k = 0; k < c.craft_distinct; ++k) {
+                    for (int k = 0; k < craft_distinct; ++k) {
                         int best = -1, bestv = 0;
                         for (int r = 0; r < R; ++r) {
                             if ((used >> r) & 1u) continue;
@@ -704,7 +715,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
                             if (best < 0 || v > bestv) { best = r; bestv = v; }
                         }
                         used |= 1u << best;
-                        m.inv()[best * N4 + tid] = bestv - c.craft_units;
+                        m.inv()[best * N4 + tid] = bestv - craft_units;
                     }
                 }
             }
@@ -716,21 +727,21 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             } else {
                 invalid = true;
             }
-        } else if (a < c.base_sell + R * P) {  // market order
-            side_c = a >= c.base_sell;
-            const int k = a - (side_c ? c.base_sell : c.base_buy);
+        } else if (a < base_sell + R * P) {  // market order
+            side_c = a >= base_sell;
+            const int k = a - (side_c ? base_sell : base_buy);
             r_c = PT > 0 ? k / (PT > 0 ? PT : 1) : (k * c.recipP) >> 16;
             const int pidx = k - r_c * P;
             price_c = c.prices[pidx];
-            bool ok = __popc(mymask) < c.M;
+            bool ok = __popc(mymask) < M;
             if (side_c == 0) ok = ok && (coin_pre >= (float)price_c);
             else ok = ok && (m.inv()[r_c * N4 + tid] >= 1);
             if (ok) {
                 lvl = (r_c * 2 + side_c) * P + pidx;
-                slot = ((uint32_t)tid << c.Mp_log2) + (uint32_t)(__ffs(~mymask) - 1);
+                slot = ((uint32_t)tid << MPL) + (uint32_t)(__ffs(~mymask) - 1);
                 m.cslot()[tid] = slot;
                 old_tail = m.tail()[lvl];  // read before anyone links (tails change after barrier #1)
-                if (c.K) {
+                if (K) {
                     grp = r_c * 2 + side_c;
                     pos = atomicAdd(&m.gcnt()[grp], 1);
                     m.cinfo()[tid] = lvl;
@@ -751,7 +762,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
     int lrank = 0;
     bool accepted = false;
     uint32_t nxt = NIL;
-    if (c.K == 0) {
+    if (K == 0) {
         if (lvl >= 0) {
             int succ = -1;
             uint32_t sk = 0;
@@ -804,7 +815,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             }
             int n_rest = 0;
             for (int p = 0; p < P; ++p) n_rest += cnt_cur[grp * P + p];
-            accepted = n_rest + brank < c.K;
+            accepted = n_rest + brank < K;
             m.sorted()[gbase + before] = (uint32_t)tid | (accepted ? 0x10000u : 0u);
         }
         __syncthreads();
@@ -825,7 +836,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             }
             if (nxt == NIL) m.tail()[lvl] = (uint16_t)slot;
             atomicAdd(&cnt_cur[lvl], 1);
-            m.mask()[tid] = mymask | (1u << (slot & ((1u << c.Mp_log2) - 1u)));
+            m.mask()[tid] = mymask | (1u << (slot & ((1u << MPL) - 1u)));
             if (side_c == 0) {  // escrow
                 m.coin()[tid] = __fsub_rn(coin_pre, (float)price_c);
                 m.esc_coin()[tid] += price_c;
@@ -876,7 +887,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             const uint32_t pe = m.pool()[h];
             const uint32_t age = ((uint32_t)t - (pe >> 16)) & 0xFFFFu;
             if ((int)age < c.expiry) break;
-            const int owner = (int)(h >> c.Mp_log2);
+            const int owner = (int)(h >> MPL);
             if (side == 0) {
                 atomicSub(&m.esc_coin()[owner], price);
                 atomicAdd(&m.credit()[owner], price);
@@ -884,7 +895,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
                 atomicSub(&m.esc_res()[r * N4 + owner], 1);
                 atomicAdd(&m.inv()[r * N4 + owner], 1);
             }
-            atomicAnd(&m.mask()[owner], ~(1u << (h & ((1u << c.Mp_log2) - 1u))));
+            atomicAnd(&m.mask()[owner], ~(1u << (h & ((1u << MPL) - 1u))));
             ++nexp;
             --n;
             h = pe & 0xFFFFu;
@@ -895,7 +906,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             if (nexp) atomicAdd(&m.hdr()->n_expired, nexp);
         }
         cnt_nxt[l] = n;
-        if (c.K == 0) m.ahead()[l] = NIL;
+        if (K == 0) m.ahead()[l] = NIL;
         if (side == 0 && pidx == 0) m.resq()[r] = q;
     }
     __syncthreads();  // #3 matched lists complete
@@ -910,7 +921,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
                 const uint32_t eb = m.mb()[r * N4 + tid], ea = m.ma()[r * N4 + tid];
                 const uint32_t sb = eb & 0xFFFFu, sa = ea & 0xFFFFu;
                 const int pb = c.prices[eb >> 16], pa = c.prices[ea >> 16];
-                const int ob = (int)(sb >> c.Mp_log2), oa = (int)(sa >> c.Mp_log2);
+                const int ob = (int)(sb >> MPL), oa = (int)(sa >> MPL);
                 const uint32_t age_b = ((uint32_t)t - (m.pool()[sb] >> 16)) & 0xFFFFu;
                 const uint32_t age_a = ((uint32_t)t - (m.pool()[sa] >> 16)) & 0xFFFFu;
                 bool bid_later;
@@ -918,7 +929,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
                 else if (m.key()[ob] != m.key()[oa]) bid_later = m.key()[ob] > m.key()[oa];
                 else bid_later = ob > oa;
                 const int pi = bid_later ? pb : pa;
-                const uint32_t bitmask = (1u << c.Mp_log2) - 1u;
+                const uint32_t bitmask = (1u << MPL) - 1u;
                 atomicSub(&m.esc_coin()[ob], pb);
                 if (pb - pi) atomicAdd(&m.credit()[ob], pb - pi);  // refund of the escrowed excess
                 atomicAdd(&m.inv()[r * N4 + ob], 1);
@@ -949,8 +960,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
         if (act) {
             const float income = m.income()[tid];
             float tax = 0.0f, lo = 0.0f;
-            for (int b = 0; b < c.B; ++b) {
-                const float hi = (b < c.B - 1) ? c.thresholds[b] : INFINITY;
+            for (int b = 0; b < B; ++b) {
+                const float hi = (b < B - 1) ? c.thresholds[b] : INFINITY;
                 const float top = (income < hi) ? income : hi;
                 float por = __fsub_rn(top, lo);
                 if (por < 0.0f) por = 0.0f;
@@ -972,12 +983,12 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             m.coin()[tid] = __fadd_rn(m.coin()[tid], share);
             m.income()[tid] = 0.0f;
         }
-        if (tid < c.B) {  // rates of the upcoming period
+        if (tid < B) {  // rates of the upcoming period
             if (gov_lvl < 0 || gov_lvl >= c.L) atomicAdd(&m.hdr()->n_bad_gov, 1);
             else m.hdr()->rates[tid] = c.rate_table[gov_lvl];
         }
     }
-    if (tid < c.B && (boundary || first)) m.shrow()[5 * R + tid] = m.hdr()->rates[tid];
+    if (tid < B && (boundary || first)) m.shrow()[5 * R + tid] = m.hdr()->rates[tid];
     __syncthreads();  // #5 state final
     if (tid == 0) {
         m.hdr()->t = t + 1;
@@ -991,7 +1002,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
 
 // One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
 // observations.  outputs() has this single call site (instruction footprint).
-template <int NPAD, int NS, int RT, int PT>
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF>
 __device__ void env_step(const DevCfg& c, const Sm<NS>& m, int tid, int e, const StepPtrs& io, bool first) {
     const int t = m.hdr()->t;
     // the previous step's bulk stores must have read the staging tile before it is rewritten
@@ -1006,17 +1017,17 @@ __device__ void env_step(const DevCfg& c, const Sm<NS>& m, int tid, int e, const
         __syncthreads();
         mode = 1;
     } else {
-        step_body<NPAD, NS, RT, PT>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
+        step_body<NPAD, NS, RT, PT, NT, BT, PF>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
     }
     // ---------------- P5 rewards, P6 observations ----------------
-    outputs<NPAD, NS, RT>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs(), io.rew());
+    outputs<NPAD, NS, RT, NT, BT, PF>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs(), io.rew());
     if (mode == 1) {
         if (tid == 0 && io.io.done) io.done()[e] = 1;
         __syncthreads();  // shrow is rewritten at the very start of the next finished step
     }
 }
 
-template <int NPAD, int NS, int RT, int PT>
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF>
 __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const __grid_constant__ StepIO io) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
@@ -1037,7 +1048,7 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
 #pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
         p.s = s;
-        env_step<NPAD, NS, RT, PT>(c, m, tid, e, p, s == 0);
+        env_step<NPAD, NS, RT, PT, NT, BT, PF>(c, m, tid, e, p, s == 0);
         p.slot = (p.slot + 1 == io.ring_depth) ? 0 : p.slot + 1;
     }
     __syncthreads();
@@ -1060,7 +1071,7 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
     if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
     __syncthreads();
-    outputs<NPAD, NS, 0>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
+    outputs<NPAD, NS, 0, 0, 0, 0>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
