@@ -133,10 +133,6 @@ void build_layout(DevCfg& c) {
     } else {
         c.o_bucket = c.o_sorted = c.o_gcnt = c.o_goff = c.o_ahead;  // unused
     }
-    // histograms of the integer-metric medians: alias the arrival scratch (key | cslot | anext,
-    // dead once the trades are settled) when they fit
-    const int hist_bytes = (R < c.n_warps ? R : c.n_warps) * HB * 4;
-    c.o_hist = hist_bytes <= 3 * NP * 4 ? c.o_key : take(hist_bytes);
     // staging tile of the population observation rows (not zeroed); the matched-order lists
     // mb | ma alias its head (written after the previous step's bulk store has been read,
     // consumed before the rows are staged)

@@ -31,12 +31,11 @@ namespace {
 
 constexpr uint32_t NIL = 0xFFFFu;      // null slot of the order pool
 constexpr uint32_t FULL = 0xffffffffu;
-constexpr int HB = 128;                // histogram bins of the integer-metric medians
 
 struct EnvHdr {
     int32_t t;
     int32_t n_trades, n_placed, n_invalid, n_expired, n_bad_gov;
-    uint32_t med_prev[2];  // bit patterns of the previous lower medians of labor and income (a hint, not state)
+    uint32_t med_prev[2 + EJ_MAX_RESOURCES];  // previous lower medians of labor, income (float bits) and inv[r]: hints, not state
     double u_g_prev;
     int32_t t_in_period;  // t % tax_period, kept incrementally (no integer division on the step path)
     int32_t pad1;
@@ -66,7 +65,7 @@ struct DevCfg {
     int o_blob, o_scratch1;  // absolute: blob start (= Lay<Npad>::blob), first byte after the blob
     // scratch section offsets (bytes from the shared-memory base; all after the blob)
     int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma, o_bucket, o_sorted;
-    int o_gcnt, o_goff, o_resq, o_hist, o_shrow, o_govrow, o_misc, o_cdf, o_stage;
+    int o_gcnt, o_goff, o_resq, o_shrow, o_govrow, o_misc, o_cdf, o_stage;
     int smem_bytes;
     unsigned long long gov_obs_offset, obs_floats;
 };
@@ -158,7 +157,6 @@ struct Sm {
     __device__ __forceinline__ uint32_t* sorted() const { return at<uint32_t>(c.o_sorted); }
     __device__ __forceinline__ int* gcnt() const { return at<int>(c.o_gcnt); }
     __device__ __forceinline__ int* goff() const { return at<int>(c.o_goff); }
-    __device__ __forceinline__ int* hist() const { return at<int>(c.o_hist); }
     __device__ __forceinline__ uint32_t* cdf() const { return at<uint32_t>(c.o_cdf); }
     __device__ __forceinline__ float* stage() const { return at<float>(c.o_stage); }
 };
@@ -306,12 +304,11 @@ __device__ __forceinline__ float warp_pick(const float (&x)[EPL], int rank) {
 // sorts) after WALK_MAX moves or if a value has its sign bit set (keys would not be monotone).
 constexpr int WALK_MAX = 8;
 template <int EPL>
-__device__ __forceinline__ bool walk_select(const float (&x)[EPL], int lane, int N, int r0, int r1, uint32_t* pivot, float& lo,
-                                            float& hi) {
-    uint32_t key[EPL];
+__device__ __forceinline__ bool walk_select(const uint32_t (&key)[EPL], int lane, int r0, int r1, uint32_t* pivot, uint32_t& lo,
+                                            uint32_t& hi) {
     uint32_t any = 0;
 #pragma unroll
-    for (int q = 0; q < EPL; ++q) { key[q] = __float_as_uint(x[q]); any |= key[q]; }
+    for (int q = 0; q < EPL; ++q) any |= key[q];
     if (__reduce_or_sync(FULL, any) & 0x80000000u) return false;
     uint32_t p = *pivot;
     int a = 0, b = 0;
@@ -351,65 +348,66 @@ __device__ __forceinline__ bool walk_select(const float (&x)[EPL], int lane, int
         p1 = __reduce_min_sync(FULL, mn);
     }
     if (lane == 0) *pivot = p;
-    lo = __uint_as_float(p);
-    hi = __uint_as_float(p1);
+    lo = p;
+    hi = p1;
     return true;
 }
 
+// The same two order statistics without a hint, by bitwise search on the keys (31 counting
+// rounds in a loop of a dozen instructions): the rarely taken fall-back of the integer metrics.
+template <int EPL>
+__device__ __forceinline__ void bit_select(const uint32_t (&key)[EPL], int r0, int r1, uint32_t& lo, uint32_t& hi) {
+    uint32_t res = 0;
+#pragma unroll 1
+    for (int bit = 30; bit >= 0; --bit) {  // largest res with #{x < res} <= r0 = the statistic of rank r0
+        const uint32_t cand = res | (1u << bit);
+        int a = 0;
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) a += key[q] < cand;
+        if (__reduce_add_sync(FULL, a) <= r0) res = cand;
+    }
+    int b = 0;
+    uint32_t mn = 0xFFFFFFFFu;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) { b += key[q] <= res; mn = min(mn, key[q] > res ? key[q] : 0xFFFFFFFFu); }
+    lo = res;
+    hi = r1 >= __reduce_add_sync(FULL, b) ? __reduce_min_sync(FULL, mn) : res;
+}
+
 template <int NP, int NT>
-__device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm<NP>& m, int k, double mean, float q_sum, float lo, float hi,
+__device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm<NP>& m, int k, double mean, double var, float lo, float hi,
                                            float scale) {
     const int N = NT > 0 ? NT : c.N;
-    const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
-    const float sd = __fsqrt_rn((float)((double)q_sum * inv_n));
+    const float sd = __fsqrt_rn((float)var);
     const float med = (N & 1) ? hi : __fmul_rn(0.5f, __fadd_rn(lo, hi));
     m.govrow()[3 * k + 0] = (float)(mean * (double)scale);
     m.govrow()[3 * k + 1] = __fmul_rn(sd, scale);
     m.govrow()[3 * k + 2] = __fmul_rn(med, scale);
 }
 
-// One warp computes mean, std, median (Fig.1, G26) of metric k (0 coin, 1 labor,
-// 2 income, 3 + r inventory of resource r); for coin also the welfare u_g = eq * prod (Eq.3-5,
-// P:175-188; G22, G23) and the government reward.  Sum in binary64 (integers: exact REDUX sum);
-// squared deviations in binary32 (non-negative terms: relative error < 1e-6).  Median: integer
-// metrics whose values are all below HB use a per-warp shared-memory histogram, everything else
-// the register sorting network.  ONE instance of this code per kernel (the caller loops over k
-// without unrolling): the unrolled network is most of the kernel's instruction footprint.
+// One warp computes mean, std, median (Fig.1, G26) of FLOAT metric k (0 coin,
+// 1 labor, 2 income); for coin also the welfare u_g = eq * prod (Eq.3-5; G22, G23)
+// and the government reward.  Sum in binary64; squared deviations in binary32 (non-negative
+// terms: relative error < 1e-6).  Median: labor and income walk from last step's median (the
+// sorting network when the walk gives up), coin is sorted (the order also gives gini).  ONE
+// instance of this code per kernel (the caller loops over k without unrolling): the unrolled
+// network is most of the kernel's instruction footprint.
 //   mode 0 = step, 1 = finished env (reward 0), 2 = observe only
 template <int EPL, int NS, int NT>
-__device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, int k, int lane, int mode, int e, float* rew,
-                                             int* hist) {
+__device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, int k, int lane, int mode, int e, float* rew) {
     const int N = NT > 0 ? NT : c.N;  // NT > 0: population size known at compile time
     const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
-    const bool is_int = k >= 3;
     const float* farr = k == 0 ? m.coin() : k == 1 ? m.labor() : m.income();
-    const int* iarr = m.inv() + (is_int ? k - 3 : 0) * NS;
     float x[EPL];
     double s = 0.0;
-    int si = 0, mx = 0;
 #pragma unroll
     for (int q = 0; q < EPL; ++q) {
         const int idx = lane * EPL + q;  // blocked layout (warp_sort)
-        x[q] = INFINITY;
-        if (idx < N) {
-            if (is_int) {
-                const int v = iarr[idx];
-                x[q] = (float)v;
-                si += v;
-                mx = max(mx, v);
-            } else {
-                x[q] = farr[idx];
-                s += (double)x[q];
-            }
-        }
+        const float v = farr[idx < N ? idx : 0];
+        x[q] = idx < N ? v : INFINITY;
+        s += idx < N ? (double)v : 0.0;
     }
-    bool use_hist = false;
-    if (is_int) {
-        s = (double)__reduce_add_sync(FULL, si);
-        use_hist = __reduce_max_sync(FULL, mx) < HB;
-    } else {
-        s = warp_sum(s);
-    }
+    s = warp_sum(s);
     const double mean = s * inv_n;
     float qs = 0.0f;
 #pragma unroll
@@ -419,45 +417,21 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, i
     }
     qs = warp_sum(qs);
     float lo, hi;
-    if (use_hist) {
-        ((int4*)hist)[lane] = make_int4(0, 0, 0, 0);
-        __syncwarp();
+    const int r0 = N >= 2 ? (N >> 1) - 1 : 0, r1 = N >> 1;
+    bool found = false;
+    if (k != 0) {  // labor, income: med_prev holds last step's lower median
+        uint32_t key[EPL], klo, khi;
 #pragma unroll
-        for (int q = 0; q < EPL; ++q)
-            if (lane * EPL + q < N) atomicAdd(&hist[__float2int_rz(x[q])], 1);
-        __syncwarp();
-        const int4 h4 = ((int4*)hist)[lane];
-        const int c0 = h4.x, c1 = c0 + h4.y, c2 = c1 + h4.z, c3 = c2 + h4.w;
-        int incl = c3;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int y = __shfl_up_sync(FULL, incl, o);
-            if (lane >= o) incl += y;
-        }
-        const int excl = incl - c3;
-        int vals[2];
-#pragma unroll
-        for (int j = 0; j < 2; ++j) {  // value of 0-based rank r = smallest value with cum(value) > r
-            const int rk = max((N >> 1) - 1 + j, 0);
-            const unsigned ball = __ballot_sync(FULL, incl > rk);
-            const int src = __ffs(ball) - 1;
-            const int rel = rk - __shfl_sync(FULL, excl, src);
-            const int a0 = __shfl_sync(FULL, c0, src), a1 = __shfl_sync(FULL, c1, src), a2 = __shfl_sync(FULL, c2, src);
-            vals[j] = src * 4 + (rel < a0 ? 0 : rel < a1 ? 1 : rel < a2 ? 2 : 3);
-        }
-        lo = (float)vals[0];
-        hi = (float)vals[1];
-    } else {
-        const int r0 = N >= 2 ? (N >> 1) - 1 : 0, r1 = N >> 1;
-        bool found = false;
-        const bool hinted = k == 1 || k == 2;  // labor, income: med_prev holds last step's lower median
-        if (hinted) found = walk_select<EPL>(x, lane, N, r0, r1, &m.hdr()->med_prev[k - 1], lo, hi);
-        if (!found) {
-            warp_sort<EPL>(x, lane);
-            lo = warp_pick<EPL>(x, r0);
-            hi = warp_pick<EPL>(x, r1);
-            if (hinted && lane == 0) m.hdr()->med_prev[k - 1] = __float_as_uint(lo);
-        }
+        for (int q = 0; q < EPL; ++q) key[q] = __float_as_uint(x[q]);
+        found = walk_select<EPL>(key, lane, r0, r1, &m.hdr()->med_prev[k - 1], klo, khi);
+        lo = __uint_as_float(klo);
+        hi = __uint_as_float(khi);
+    }
+    if (!found) {
+        warp_sort<EPL>(x, lane);
+        lo = warp_pick<EPL>(x, r0);
+        hi = warp_pick<EPL>(x, r1);
+        if (k != 0 && lane == 0) m.hdr()->med_prev[k - 1] = __float_as_uint(lo);
         if (k == 0 && mode != 2) {
             // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)  =>  gini * prod = gn / N   (G23)
             double g = 0.0;
@@ -480,7 +454,54 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, i
             }
         }
     }
-    if (lane == 0) gov_triple<NS, NT>(c, m, k, mean, qs, lo, hi, is_int ? c.s_count : k == 1 ? c.s_labor : c.s_coin);
+    if (lane == 0) gov_triple<NS, NT>(c, m, k, mean, (double)qs * inv_n, lo, hi, k == 1 ? c.s_labor : c.s_coin);
+}
+
+// The same triple for the INTEGER metric "inventory of resource r" (metric 3 + r).  Sum and
+// sum of squares are exact integers (REDUX), so mean and variance (N sum x^2 - (sum x)^2) / N^2
+// need no second pass; the median walks from last step's value on the integer keys, with the
+// bitwise search as fall-back.
+template <int EPL, int NS, int NT>
+__device__ __forceinline__ void int_metric_stats(const DevCfg& c, const Sm<NS>& m, int r, int lane) {
+    const int N = NT > 0 ? NT : c.N;
+    const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
+    const int* iarr = m.inv() + r * NS;
+    uint32_t key[EPL];
+    int si = 0, mx = 0;
+    uint32_t sq = 0;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) {
+        const int idx = lane * EPL + q;
+        const int v = iarr[idx < N ? idx : 0];
+        key[q] = idx < N ? (uint32_t)v : 0x7FFFFFFFu;  // pads sort last; a negative value makes the walk give up
+        si += idx < N ? v : 0;
+        mx = max(mx, idx < N ? (v < 0 ? 0x7FFFFFFF : v) : 0);
+        sq += idx < N ? (uint32_t)(v * v) : 0u;
+    }
+    const long long sum = (long long)__reduce_add_sync(FULL, si);
+    unsigned long long sum2;
+    if (EPL <= 8 && __reduce_max_sync(FULL, mx) < 4096) {  // 32 x EPL x 4096^2 <= 2^32 - 1 for EPL <= 8
+        sum2 = (unsigned long long)__reduce_add_sync(FULL, sq);
+    } else {
+        unsigned long long w = 0;
+#pragma unroll
+        for (int q = 0; q < EPL; ++q) {
+            const long long v = (lane * EPL + q) < N ? (long long)(int)key[q] : 0ll;
+            w += (unsigned long long)(v * v);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(FULL, w, o);
+        sum2 = w;
+    }
+    const double mean = (double)sum * inv_n;
+    const double var = (double)((long long)N * (long long)sum2 - sum * sum) * inv_n * inv_n;
+    const int r0 = N >= 2 ? (N >> 1) - 1 : 0, r1 = N >> 1;
+    uint32_t klo, khi;
+    if (!walk_select<EPL>(key, lane, r0, r1, &m.hdr()->med_prev[2 + r], klo, khi)) {
+        bit_select<EPL>(key, r0, r1, klo, khi);
+        if (lane == 0) m.hdr()->med_prev[2 + r] = klo;
+    }
+    if (lane == 0) gov_triple<NS, NT>(c, m, 3 + r, mean, var, (float)(int)klo, (float)(int)khi, c.s_count);
 }
 
 // Shared tail of the population rows: market statistics of the post-step books.
@@ -565,14 +586,9 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
     // ---- government statistics: metric k is owned by one warp (floats from warp 0 up, integer
     // metrics from the last warp down) ----
 #pragma unroll 1
-    for (int it = 0; it < 2; ++it) {
-        // it 0: float metrics k = warp, warp + NW, ... < 3; it 1: integer metrics of resources
-        // r = NW-1-warp, + NW, ... < R.  One instance of metric_stats (instruction footprint).
-        const int first = it == 0 ? warp : 3 + (NW - 1 - warp), last = it == 0 ? 3 : n_metrics;
+    for (int k = warp; k < 3; k += NW) metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
 #pragma unroll 1
-        for (int k = first; k < last; k += NW)
-            metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew, m.hist() + (NW - 1 - warp) * HB);
-    }
+    for (int r = NW - 1 - warp; r < R; r += NW) int_metric_stats<EPL, NS, NT>(c, m, r, lane);
     if (tid < B + 2) m.govrow()[3 * n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
 
     if (obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
