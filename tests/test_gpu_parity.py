@@ -347,3 +347,44 @@ def test_error_paths():
     with pytest.raises(binding.EjError) as ei:
         env.step(torch.zeros((1, 4), dtype=torch.int32, device="cuda"), torch.zeros((1, 3), dtype=torch.int32, device="cuda"))
     assert ei.value.code == binding.EJ_ERR_STATE
+
+
+@pytest.mark.parametrize("name", ["config2_paper", "tiny_dense", "config3_resources"])
+def test_government_statistics_on_adversarial_states(name):
+    """a10 on states the episodes never reach: inventories from 0 to 60,000 (the 64-bit sum path of
+    the integer metrics), all-equal and two-valued populations, and jumps between rounds so that the
+    median hints kept from the previous call are useless (walk-select gives up -> bitwise search /
+    sorting network).  Each round: oracle state -> ej_set_state -> ej_observe, then one no-op step."""
+    import torch
+
+    cfg = inputs.configs()[name]
+    E, N, R = 2, cfg["N"], cfg["R"]
+    params = dict(cfg["params"], episode_length=1000)
+    pair = Pair(E, N, R, params, 11)
+    rng = np.random.default_rng(5)
+    A = pair.g.A
+    shapes = ["wide", "equal", "two", "small", "huge", "zero", "wide"]
+    for rnd, shape in enumerate(shapes):
+        for e in range(E):
+            for i in range(N):
+                if shape == "wide":
+                    inv = rng.integers(0, 3000, R)
+                    coin = float(np.float32(rng.uniform(0, 5000)))
+                elif shape == "equal":
+                    inv, coin = np.full(R, 7), 12.5
+                elif shape == "two":
+                    inv, coin = np.where(rng.random(R) < 0.5, 1, 50000), float(rng.choice([0.0, 1e4]))
+                elif shape == "small":
+                    inv, coin = rng.integers(0, 4, R), float(np.float32(rng.uniform(0, 3)))
+                elif shape == "huge":
+                    inv, coin = rng.integers(4000, 60000, R), float(np.float32(rng.uniform(0, 1e5)))
+                else:
+                    inv, coin = np.zeros(R, np.int64), 0.0
+                pair.o[0].set_agent(e, i, coin, [int(v) for v in inv], [1.0] * R, 1.0)
+        pair.g.set_state(pair.o[0].get_state())
+        pop, gov = pair.g.split_obs(pair.g.observe())
+        o_pop, o_gov = pair.o[0].observe()
+        exact(pop.cpu().numpy(), o_pop, "%s round %d (%s) pop obs" % (name, rnd, shape))
+        close(gov.cpu().numpy(), o_gov, "%s round %d (%s) gov obs" % (name, rnd, shape))
+        acts = np.full((E, N), A - 1, np.int32)  # everyone idles: the step kernel's statistics of the same state
+        pair.step_and_compare(acts, np.zeros((E, pair.g.B), np.int32), "%s round %d (%s) noop step" % (name, rnd, shape))
