@@ -181,7 +181,9 @@ int ej_step_host(ej_env* h, const int32_t* actions, const int32_t* gov_actions, 
 /* T steps in ONE persistent launch: each env's state stays in shared memory for the whole
  * call.  Actions come from io->actions_in / gov_actions_in or, when NULL, from the Philox/CDF
  * generator (ej_set_action_cdf; uniform over the A actions by default).  io may be NULL
- * (no outputs).  No auto-reset: envs that reach episode_length stay done (G28). */
+ * (no outputs).  No auto-reset: envs that reach episode_length stay done (G28).
+ * Limits (EJ_ERR_PARAM): ring_depth * obs_floats < 2^32 and, with actions_in, T * E * N < 2^32
+ * (the kernels index rings and action streams with 32-bit element offsets). */
 int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* io);
 
 /* Cumulative uint32 thresholds of the rollout's action generator: action = smallest a with

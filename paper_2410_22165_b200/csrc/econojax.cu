@@ -608,6 +608,10 @@ int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* rio) {
     if (rio) {
         if (rio->struct_size != sizeof(ej_rollout_io)) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.struct_size");
         if (rio->ring_depth < 1) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.ring_depth");
+        // the kernels index rings and action streams with 32-bit element offsets
+        const unsigned long long lim = 1ull << 32;
+        if ((unsigned long long)rio->ring_depth * h->c.obs_floats >= lim) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.ring_depth (ring_depth * obs_floats must stay below 2^32)");
+        if (rio->actions_in && (unsigned long long)T * h->c.E * h->c.N >= lim) return fail(h, EJ_ERR_PARAM, "bad field: %s", "T (T * E * N must stay below 2^32 with actions_in)");
         io.ring_depth = rio->ring_depth;
         io.actions = rio->actions_in; io.gov_actions = rio->gov_actions_in;
         io.obs = rio->obs_ring; io.rew = rio->rew_ring; io.done = rio->done_ring;

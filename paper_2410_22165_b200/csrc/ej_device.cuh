@@ -446,10 +446,10 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, i
                 // prod = 0 or N = 1 (then gn = 0 as well)
                 const double ug = s - (double)c.omega * (g * inv_n);
                 if (mode == 0) {
-                    if (rew) rew[(size_t)e * (N + 1) + N] = (float)(ug - m.hdr()->u_g_prev);
+                    if (rew) rew[(uint32_t)(e * (N + 1) + N)] = (float)(ug - m.hdr()->u_g_prev);
                     m.hdr()->u_g_prev = ug;
                 } else if (rew) {
-                    rew[(size_t)e * (N + 1) + N] = 0.0f;
+                    rew[(uint32_t)(e * (N + 1) + N)] = 0.0f;
                 }
             }
         }
@@ -556,9 +556,9 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
                 cf_post = coin_utility(coin, c.ua, c.inv_ua);
                 m.cf()[tid] = cf_post;
             }
-            if (rew) rew[(size_t)e * (N + 1) + tid] = (float)((cf_post - (double)labor) - (cf_pre - (double)labor_pre));
+            if (rew) rew[(uint32_t)(e * (N + 1) + tid)] = (float)((cf_post - (double)labor) - (cf_pre - (double)labor_pre));
         } else if (mode == 1 && rew) {
-            rew[(size_t)e * (N + 1) + tid] = 0.0f;
+            rew[(uint32_t)(e * (N + 1) + tid)] = 0.0f;
         }
         // ---- this agent's observation row (G25) in the staging tile ----
         if (staged) {
@@ -596,11 +596,11 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
 
     if (obs && tid == 0) {  // bulk stores: the env's contiguous [N][D_pop] tile and its government row
         if (staged) {
-            float* dst = obs + (size_t)e * N * D_pop;
+            float* dst = obs + (uint32_t)(e * N * D_pop);
             const uint32_t src = (uint32_t)__cvta_generic_to_shared(m.stage());
             asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(N * D_pop * 4) : "memory");
         }
-        float* gdst = obs + c.gov_obs_offset + (size_t)e * c.D_gov_pad;
+        float* gdst = obs + (uint32_t)((uint32_t)c.gov_obs_offset + (uint32_t)(e * c.D_gov_pad));
         const uint32_t gsrc = (uint32_t)__cvta_generic_to_shared(m.govrow());
         asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(gsrc), "r"(c.D_gov_pad * 4) : "memory");
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
@@ -629,16 +629,17 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
 // Inputs and outputs of step `s` of a launch (ring slot `slot`), resolved where they are used:
 // keeping seven running pointers alive in every thread cost ~6 % of the executed instructions.
 struct StepPtrs {
+    // element offsets are 32-bit (the host rejects rings / action streams of 2^32 elements or more)
     const StepIO& io;
     const DevCfg& c;
     int s, slot;
-    __device__ __forceinline__ const int32_t* actions() const { return io.actions ? io.actions + (size_t)s * c.E * c.N : nullptr; }
-    __device__ __forceinline__ const int32_t* gov_actions() const { return io.gov_actions ? io.gov_actions + (size_t)s * c.E * c.B : nullptr; }
-    __device__ __forceinline__ float* obs() const { return io.obs ? io.obs + (size_t)slot * c.obs_floats : nullptr; }
-    __device__ __forceinline__ float* rew() const { return io.rew ? io.rew + (size_t)slot * c.E * (c.N + 1) : nullptr; }
-    __device__ __forceinline__ uint8_t* done() const { return io.done ? io.done + (size_t)slot * c.E : nullptr; }
-    __device__ __forceinline__ int32_t* actions_out() const { return io.actions_out ? io.actions_out + (size_t)slot * c.E * c.N : nullptr; }
-    __device__ __forceinline__ int32_t* gov_out() const { return io.gov_out ? io.gov_out + (size_t)slot * c.E * c.B : nullptr; }
+    __device__ __forceinline__ const int32_t* actions() const { return io.actions ? io.actions + (uint32_t)s * (uint32_t)(c.E * c.N) : nullptr; }
+    __device__ __forceinline__ const int32_t* gov_actions() const { return io.gov_actions ? io.gov_actions + (uint32_t)s * (uint32_t)(c.E * c.B) : nullptr; }
+    __device__ __forceinline__ float* obs() const { return io.obs ? io.obs + (uint32_t)slot * (uint32_t)c.obs_floats : nullptr; }
+    __device__ __forceinline__ float* rew() const { return io.rew ? io.rew + (uint32_t)slot * (uint32_t)(c.E * (c.N + 1)) : nullptr; }
+    __device__ __forceinline__ uint8_t* done() const { return io.done ? io.done + (uint32_t)slot * (uint32_t)c.E : nullptr; }
+    __device__ __forceinline__ int32_t* actions_out() const { return io.actions_out ? io.actions_out + (uint32_t)slot * (uint32_t)(c.E * c.N) : nullptr; }
+    __device__ __forceinline__ int32_t* gov_out() const { return io.gov_out ? io.gov_out + (uint32_t)slot * (uint32_t)(c.E * c.B) : nullptr; }
 };
 
 // Phases P1-P4 of one environment step on the state in shared memory (G1: actions -> match ->
@@ -666,7 +667,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
     if (act) {
         philox4x32_10(gid, (uint32_t)tid, (uint32_t)t, 0u, c.seed_lo, c.seed_hi, x0, x1, x2, x3);
         if (io.io.actions) {
-            a = io.actions()[(size_t)e * N + tid];
+            a = io.actions()[(uint32_t)(e * N + tid)];
         } else {  // smallest a with x0 < cdf[a]; last entry read as 2^32 (G30)
             int lo = 0, hi = A - 1;
             while (lo < hi) {
@@ -676,7 +677,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             }
             a = lo;
         }
-        if (io.io.actions_out) io.actions_out()[(size_t)e * N + tid] = a;
+        if (io.io.actions_out) io.actions_out()[(uint32_t)(e * N + tid)] = a;
         m.key()[tid] = x2;
     }
     // government levels for the period boundary
@@ -686,14 +687,14 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
     const bool boundary = c.taxes_enabled && period_end;
     if (tid < B && (boundary || io.io.gov_out)) {
         if (io.io.gov_actions) {
-            gov_lvl = io.gov_actions()[(size_t)e * B + tid];
+            gov_lvl = io.gov_actions()[(uint32_t)(e * B + tid)];
         } else {
             uint32_t g0, g1, g2, g3;
             philox4x32_10(gid, (uint32_t)N, (uint32_t)t, (uint32_t)(1 + tid / 4), c.seed_lo, c.seed_hi, g0, g1, g2, g3);
             const uint32_t gx = (tid & 3) == 0 ? g0 : (tid & 3) == 1 ? g1 : (tid & 3) == 2 ? g2 : g3;
             gov_lvl = (int)(((unsigned long long)gx * (unsigned long long)c.L) >> 32);
         }
-        if (io.io.gov_out) io.gov_out()[(size_t)e * B + tid] = gov_lvl;
+        if (io.io.gov_out) io.gov_out()[(uint32_t)(e * B + tid)] = gov_lvl;
     }
 
     int lvl = -1, grp = 0, pos = 0, price_c = 0, r_c = 0, side_c = 0;
