@@ -97,6 +97,7 @@ def lib():
             L.orc_step.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.c_void_p] * 6
             L.orc_draw_actions.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
             L.orc_action_mask.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
+            L.orc_draw_actions_masked.argtypes = L.orc_draw_actions.argtypes
             L.orc_state_words.argtypes = [C.c_void_p]; L.orc_state_words.restype = C.c_size_t
             L.orc_get_state.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p]
             L.orc_set_agent.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_float, i32p, f32p, C.c_float]
@@ -180,13 +181,15 @@ class OracleEnv:
                         _ptr(rew), _ptr(done))
         return obs_pop, obs_gov, rew, done
 
-    def draw_actions(self, cdf, env_begin=0, env_count=None):
+    def draw_actions(self, cdf, env_begin=0, env_count=None, masked=False):
+        """Rollout-mode generator (G30); masked=True: restricted to the available actions (f1)."""
         n = self.E - env_begin if env_count is None else env_count
         cdf = np.ascontiguousarray(cdf, np.uint32)
         assert cdf.shape == (self.A,)
         actions = np.zeros((n, self.N), np.int32)
         gov = np.zeros((n, self.B), np.int32)
-        self.L.orc_draw_actions(self.h, env_begin, n, _ptr(cdf), _ptr(actions), _ptr(gov))
+        fn = self.L.orc_draw_actions_masked if masked else self.L.orc_draw_actions
+        fn(self.h, env_begin, n, _ptr(cdf), _ptr(actions), _ptr(gov))
         return actions, gov
 
     def action_mask(self, env_begin=0, env_count=None):

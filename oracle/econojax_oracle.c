@@ -790,3 +790,49 @@ void orc_action_mask(const orc_sim* s, int32_t env_begin, int32_t env_count, uin
         }
     }
 }
+
+/* f1, masked sampling (the policy's categorical gives zero probability to
+ * unavailable actions): the rollout-mode generator restricted to the available actions of the
+ * current state and renormalised.  With the caller's table, action a has integer weight
+ * w_a = cdf[a] - cdf[a-1] (cdf[-1] = 0, the last entry read as 2^32, as in orc_draw_actions);
+ * S = sum of w_a over available a;  target = floor(x0 * S / 2^32) with x0 = Philox stream 0
+ * word 0;  action = first available a whose running sum of available weights exceeds target.
+ * All integers, so the draw is exact.  With every action available S = 2^32, target = x0 and
+ * the rule is orc_draw_actions'.  If S = 0 (the table gives the available actions no mass) the
+ * first available action is returned.  Government levels are not masked. */
+void orc_draw_actions_masked(const orc_sim* s, int32_t env_begin, int32_t env_count, const uint32_t* cdf,
+                             int32_t* actions, int32_t* gov_actions) {
+    const int32_t N = s->N;
+    const int32_t A = orc_num_actions(s->R, s->p.num_prices, s->p.craft_mode, s->p.allow_noop);
+    uint8_t* mask = (uint8_t*)malloc((size_t)N * A);
+    orc_draw_actions(s, env_begin, env_count, cdf, actions, gov_actions);  /* government part; population overwritten */
+    for (int32_t k = 0; k < env_count; ++k) {
+        const int32_t e = env_begin + k;
+        const uint32_t gid = s->p.env_id_base + (uint32_t)e;
+        const uint32_t t = (uint32_t)s->env[e].t;
+        orc_action_mask(s, e, 1, mask);
+        for (int32_t i = 0; i < N; ++i) {
+            uint32_t x[4];
+            draw(s, gid, (uint32_t)i, t, 0u, x);
+            uint64_t S = 0;
+            for (int32_t a = 0; a < A; ++a) {
+                const uint64_t hi = (a == A - 1) ? ((uint64_t)1 << 32) : (uint64_t)cdf[a];
+                const uint64_t lo = (a == 0) ? 0 : (uint64_t)cdf[a - 1];
+                if (mask[(size_t)i * A + a]) S += hi - lo;
+            }
+            const uint64_t target = ((uint64_t)x[0] * S) >> 32;  /* S <= 2^32: the product fits 64 bits */
+            int32_t pick = -1, first = -1;
+            uint64_t run = 0;
+            for (int32_t a = 0; a < A && pick < 0; ++a) {
+                if (!mask[(size_t)i * A + a]) continue;
+                if (first < 0) first = a;
+                const uint64_t hi = (a == A - 1) ? ((uint64_t)1 << 32) : (uint64_t)cdf[a];
+                const uint64_t lo = (a == 0) ? 0 : (uint64_t)cdf[a - 1];
+                run += hi - lo;
+                if (run > target) pick = a;
+            }
+            actions[(size_t)k * N + i] = pick >= 0 ? pick : first;
+        }
+    }
+    free(mask);
+}

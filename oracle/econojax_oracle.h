@@ -140,6 +140,11 @@ void orc_draw_actions(const orc_sim* s, int32_t env_begin, int32_t env_count, co
 /* f1: availability of every action for every agent in the current state (rules in the .c file):
  * mask [env_count][N][A] bytes, 1 = available. */
 void orc_action_mask(const orc_sim* s, int32_t env_begin, int32_t env_count, uint8_t* mask);
+
+/* f1 masked sampling: orc_draw_actions restricted to the available actions of the
+ * current state and renormalised with integer weights (exact); definition in the .c file. */
+void orc_draw_actions_masked(const orc_sim* s, int32_t env_begin, int32_t env_count, const uint32_t* cdf,
+                             int32_t* actions, int32_t* gov_actions);
 /* Canonical, representation-free state dump (layout in DESIGN.md "Canonical state dump"). */
 size_t orc_state_words(const orc_sim* s);
 void orc_get_state(const orc_sim* s, int32_t env_begin, int32_t env_count, int32_t* words);

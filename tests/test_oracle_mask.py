@@ -81,3 +81,96 @@ def test_mask_is_sound_and_complete_against_the_step(name, craft_mode):
             assert (after == before) == bool(m[e, i, a]), "t=%d env %d agent %d action %d: mask %d, invalid counter %d -> %d" % (t, e, i, a, m[e, i, a], before, after)
             checked += 1
     assert checked >= 150
+
+
+# ---- f1 masked sampling (orc_draw_actions_masked) ----
+
+def _x0(seed, gid, agent, t):
+    """Philox stream 0 word 0 of (global env, agent, t): the word the generator consumes (G30)."""
+    import ctypes as C
+    L = oracle.lib()
+    c = (C.c_uint32 * 4)(gid, agent, t, 0)
+    k = (C.c_uint32 * 2)(seed & 0xFFFFFFFF, seed >> 32)
+    o = (C.c_uint32 * 4)()
+    L.orc_philox4x32_10(c, k, o)
+    return int(o[0])
+
+
+def test_masked_draw_equals_unmasked_when_everything_is_available(small_params):
+    o = oracle.OracleEnv(3, 4, 2, small_params)
+    o.reset(4)
+    for e in range(3):
+        for i in range(4):
+            o.set_agent(e, i, 100.0, [5, 5], [1.0, 1.0], 1.0)
+    assert o.action_mask().all()
+    cfg = dict(inputs.configs()["config4_population"], R=2)
+    for cdf in (inputs.action_cdf(inputs.configs()["tiny_dense"]), inputs.action_cdf(cfg)):
+        a0, g0 = o.draw_actions(cdf)
+        a1, g1 = o.draw_actions(cdf, masked=True)
+        assert np.array_equal(a0, a1) and np.array_equal(g0, g1)
+
+
+def test_masked_draw_matches_big_integer_arithmetic(small_params):
+    """Every draw recomputed with Python integers from the Philox word, the mask and the table:
+    target = x0 * S >> 32 over the available weights (definition in the oracle's header)."""
+    seed, E, N = 9, 6, 4
+    cfg = inputs.configs()["tiny_dense"]
+    o = oracle.OracleEnv(E, N, 2, cfg["params"])
+    o.reset(seed)
+    acts, gov = inputs.action_stream(cfg, 12, seed=seed, E=E)
+    mix = inputs.action_cdf(dict(inputs.configs()["config4_population"], R=2))
+    for t in range(12):
+        o.step(acts[t], gov[t], want_obs=False)
+        for cdf in (inputs.action_cdf(cfg), mix):
+            m = o.action_mask()
+            a, _ = o.draw_actions(cdf, masked=True)
+            edges = [0] + [int(v) for v in cdf[:-1]] + [1 << 32]
+            w = [edges[k + 1] - edges[k] for k in range(o.A)]
+            for e in range(E):
+                for i in range(N):
+                    S = sum(w[k] for k in range(o.A) if m[e, i, k])
+                    target = (_x0(seed, e, i, t + 1) * S) >> 32
+                    run, want = 0, None
+                    for k in range(o.A):
+                        if m[e, i, k]:
+                            run += w[k]
+                            if run > target:
+                                want = k
+                                break
+                    assert a[e, i] == want, (t, e, i, a[e, i], want)
+                    assert m[e, i, a[e, i]] == 1
+
+
+def test_masked_draw_frequencies_follow_the_renormalised_table(small_params):
+    """Broke agents (coin 0, nothing held): only gather 0, gather 1 and the no-op are available
+    (P:199); their frequencies must be the table's masses renormalised over those three."""
+    E, N = 3000, 4
+    p = dict(small_params, starting_coin=0.0)
+    o = oracle.OracleEnv(E, N, 2, p)
+    o.reset(21)
+    act = Act(2, 10)
+    cdf = inputs.action_cdf(dict(inputs.configs()["config4_population"], R=2))
+    edges = [0] + [int(v) for v in cdf[:-1]] + [1 << 32]
+    w = np.array([edges[k + 1] - edges[k] for k in range(o.A)], np.float64)
+    a, _ = o.draw_actions(cdf, masked=True)
+    avail = [act.gather(0), act.gather(1), act.noop]
+    assert set(np.unique(a)) <= set(avail)
+    n = a.size
+    for k in avail:
+        pk = w[k] / w[avail].sum()
+        assert abs((a == k).mean() - pk) < 4.5 * np.sqrt(pk * (1 - pk) / n), (k, (a == k).mean(), pk)
+
+
+def test_masked_rollout_never_submits_an_invalid_action():
+    cfg = inputs.configs()["config2_paper"]
+    E = 2
+    cdf = inputs.action_cdf(cfg)
+    counts = {}
+    for masked in (False, True):
+        o = oracle.OracleEnv(E, cfg["N"], cfg["R"], cfg["params"])
+        o.reset(3)
+        for t in range(80):
+            a, g = o.draw_actions(cdf, masked=masked)
+            o.step(a, g, want_obs=False)
+        counts[masked] = sum(int(oracle.parse_state(w)["counters"][2]) for w in o.get_state())
+    assert counts[True] == 0 and counts[False] > 0
