@@ -196,6 +196,17 @@ int ej_set_action_cdf(ej_env* h, const uint32_t* cdf, int32_t A);
 int ej_get_state(ej_env* h, int32_t env_begin, int32_t env_count, int32_t* words, size_t n_words);
 int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t* words, size_t n_words);
 
+/* f1 masked sampling ("unavailable actions" get zero probability).  on != 0: whenever
+ * ej_rollout / ej_policy_act draw population actions themselves, they draw among the actions that
+ * ej_action_mask marks available in the state the step starts from:
+ *  - table generator: integer weights w_a = cdf[a] - cdf[a-1] (last entry read as 2^32); S = sum of
+ *    the available w_a; target = floor(x0 * S / 2^32), x0 = Philox stream 0 word 0; action = first
+ *    available a whose running sum of available weights exceeds target (exact integer arithmetic);
+ *  - policy: unavailable logits are excluded from the max, the sum and the running sum of the
+ *    sampling rule of ej_set_policy.
+ * Government levels and caller-supplied actions (actions_in) are never masked.  Default: off. */
+int ej_set_action_masking(ej_env* h, int32_t on);
+
 /* a12 (G33): install (or, with two NULLs, remove) the shared population policy and the
  * government policy.  While installed, ej_rollout draws its actions from them whenever
  * io->actions_in / gov_actions_in is NULL: logits = W3 tanh(W2 tanh(W1 bf16(obs) + b1) + b2) + b3

@@ -70,7 +70,7 @@ class EjMlp(C.Structure):
 
 EXPORTS = ("ej_create", "ej_destroy", "ej_set_stream", "ej_layout", "ej_last_error", "ej_reset", "ej_observe",
            "ej_step", "ej_step_host", "ej_rollout", "ej_set_action_cdf", "ej_get_state", "ej_set_state",
-           "ej_launch_count", "ej_set_policy", "ej_policy_act", "ej_action_mask")
+           "ej_launch_count", "ej_set_policy", "ej_policy_act", "ej_action_mask", "ej_set_action_masking")
 
 _lib = None
 
@@ -92,6 +92,7 @@ def lib():
         L.ej_reset.argtypes = [vp, C.c_uint64]
         L.ej_observe.argtypes = [vp, vp]
         L.ej_action_mask.argtypes = [vp, vp]
+        L.ej_set_action_masking.argtypes = [vp, C.c_int32]
         L.ej_step.argtypes = [vp, vp, vp, vp, vp, vp]
         L.ej_step_host.argtypes = [vp, vp, vp, vp, vp, vp]
         L.ej_rollout.argtypes = [vp, C.c_int32, C.POINTER(EjRolloutIO)]
@@ -177,6 +178,10 @@ def ej_reset(h, seed: int):
 
 def ej_observe(h, obs_out: int):
     _check(h, lib().ej_observe(h, obs_out))
+
+
+def ej_set_action_masking(h, on: bool):
+    _check(h, lib().ej_set_action_masking(h, 1 if on else 0))
 
 
 def ej_action_mask(h, mask_out: int):
@@ -299,6 +304,9 @@ class Env:
         obs = self.new_obs() if obs is None else obs
         ej_observe(self.h, obs.data_ptr())
         return obs
+
+    def set_action_masking(self, on=True):
+        ej_set_action_masking(self.h, on)
 
     def action_mask(self, mask=None):
         """f1: [E, N, A] uint8 availability mask of the current state."""

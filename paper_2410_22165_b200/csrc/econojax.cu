@@ -33,6 +33,7 @@ struct ej_env {
     uint32_t* d_cdf = nullptr;
     cudaStream_t stream = 0;
     bool was_reset = false;
+    bool masking = false;  // f1: generator-drawn actions respect the action mask
     int64_t launches = 0;
     char err[256] = "";
     // staging for ej_step_host
@@ -604,7 +605,7 @@ int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* rio) {
     if (T == 0) return EJ_OK;
     StepIO io;
     memset(&io, 0, sizeof(io));
-    io.cdf = h->d_cdf; io.n_steps = T; io.ring_depth = 1;
+    io.cdf = h->d_cdf; io.n_steps = T; io.ring_depth = 1; io.masked = h->masking ? 1 : 0;
     if (rio) {
         if (rio->struct_size != sizeof(ej_rollout_io)) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.struct_size");
         if (rio->ring_depth < 1) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.ring_depth");
@@ -657,6 +658,12 @@ int ej_policy_act(ej_env* h, const float* obs, int32_t* actions_out, int32_t* go
     const DevCfg& c = h->c;
     (void)c;
     return launch_policy(h, obs, actions_out, gov_actions_out, pop_logits_out, gov_logits_out);
+}
+
+int ej_set_action_masking(ej_env* h, int32_t on) {
+    if (!h) return EJ_ERR_PARAM;
+    h->masking = on != 0;
+    return EJ_OK;
 }
 
 int ej_set_action_cdf(ej_env* h, const uint32_t* cdf, int32_t A) {

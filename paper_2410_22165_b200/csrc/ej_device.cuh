@@ -80,6 +80,7 @@ struct StepIO {
     int32_t* gov_out;            // ring [E][B] or null
     const uint32_t* cdf;         // [A] device
     int n_steps, ring_depth;
+    int masked;                  // f1: the generator draws among the available actions only
 };
 
 // Shared-memory layout of one economy.  Everything whose size depends only on the CTA size NP
@@ -626,6 +627,57 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
     }
 }
 
+// f1 masked sampling, the table generator.  Out of line: the unmasked hot path
+// keeps its registers and instruction footprint.
+template <int NS>
+__device__ __noinline__ int masked_draw(const DevCfg& c, const Sm<NS>& m, int tid, uint32_t x0, int R, int P, int M, int craft_mode,
+                            int craft_units, int craft_distinct, int base_buy, int base_sell, int A) {
+    constexpr int N4 = NS;
+    // f1: the table restricted to this agent's available actions, renormalised with
+    // integer weights w_a = cdf[a] - cdf[a-1]: target = floor(x0 S / 2^32), S = sum of available
+    // w_a; action = first available a whose running sum exceeds target (first available if S = 0)
+    const float coin = m.coin()[tid];
+    const bool room = __popc(m.mask()[tid]) < M;
+    bool craft_ok = false;
+    if (craft_mode != EJ_CRAFT_PER_RESOURCE) {
+        int enough = 0;
+        for (int r = 0; r < R; ++r) enough += m.inv()[r * N4 + tid] >= craft_units;
+        craft_ok = enough >= craft_distinct;
+    }
+    const int end_sell = base_sell + R * P;
+    unsigned long long S = 0, run = 0, target = 0;
+    int pick = -1, first_ok = -1;
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+        uint32_t prev = 0;
+#pragma unroll 1
+        for (int k = 0; k < A && pick < 0; ++k) {
+            const unsigned long long hi = k == A - 1 ? (1ull << 32) : (unsigned long long)m.cdf()[k];
+            const unsigned long long w = hi - (unsigned long long)prev;
+            prev = (uint32_t)hi;
+            bool ok = true;
+            if (k >= R && k < base_buy) {
+                ok = craft_mode == EJ_CRAFT_PER_RESOURCE ? m.inv()[(k - R) * N4 + tid] >= craft_units : craft_ok;
+            } else if (k >= base_buy && k < base_sell) {
+                const int j = k - base_buy, rr = (j * c.recipP) >> 16;
+                ok = room && coin >= (float)c.prices[j - rr * P];
+            } else if (k >= base_sell && k < end_sell) {
+                ok = room && m.inv()[(((k - base_sell) * c.recipP) >> 16) * N4 + tid] >= 1;
+            }
+            if (!ok) continue;
+            if (pass == 0) {
+                S += w;
+                if (first_ok < 0) first_ok = k;
+            } else {
+                run += w;
+                if (run > target) pick = k;
+            }
+        }
+        target = ((unsigned long long)x0 * S) >> 32;  // S <= 2^32: no overflow
+    }
+    return pick >= 0 ? pick : first_ok;
+}
+
 // Inputs and outputs of step `s` of a launch (ring slot `slot`), resolved where they are used:
 // keeping seven running pointers alive in every thread cost ~6 % of the executed instructions.
 struct StepPtrs {
@@ -668,6 +720,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
         philox4x32_10(gid, (uint32_t)tid, (uint32_t)t, 0u, c.seed_lo, c.seed_hi, x0, x1, x2, x3);
         if (io.io.actions) {
             a = io.actions()[(uint32_t)(e * N + tid)];
+        } else if (io.io.masked) {
+            a = masked_draw<NS>(c, m, tid, x0, R, P, M, craft_mode, craft_units, craft_distinct, base_buy, base_sell, A);
         } else {  // smallest a with x0 < cdf[a]; last entry read as 2^32 (G30)
             int lo = 0, hi = A - 1;
             while (lo < hi) {

@@ -89,3 +89,56 @@ def test_mask_errors():
     m = env.action_mask()
     with pytest.raises(binding.EjError):
         binding.ej_action_mask(env.h, m.data_ptr() + 1)  # misaligned
+
+
+# ---- f1 masked sampling: the rollout's table generator under the mask ----
+
+def _masked_rollout(name, E, steps, params_over=None, seed=6, env_ids=None, mix=None):
+    import torch
+    from parity import Pair, compare_state
+
+    cfg = inputs.configs()[name]
+    params = dict(cfg["params"], **(params_over or {}))
+    pair = Pair(E, cfg["N"], cfg["R"], params, seed, env_ids=env_ids)
+    cdf = inputs.action_cdf(cfg if mix is None else dict(inputs.configs()[mix], R=cfg["R"], params=params))
+    pair.g.set_action_cdf(cdf)
+    pair.g.set_action_masking(True)
+    depth = steps
+    actions_ring = torch.zeros((depth, E, cfg["N"]), dtype=torch.int32, device="cuda")
+    pair.g.rollout(steps, ring_depth=depth, actions_ring=actions_ring)
+    torch.cuda.synchronize()
+    got = actions_ring.cpu().numpy()
+    ids = pair.env_ids
+    for t in range(steps):
+        for o, e in zip(pair.o, ids) if env_ids is not None else [(pair.o[0], None)]:
+            a, g = o.draw_actions(cdf, masked=True)
+            want = got[t] if e is None else got[t, e:e + 1]
+            assert np.array_equal(a, want), "%s t=%d env %s: masked draws differ" % (name, t, e)
+            o.step(a, g, want_obs=False)
+    compare_state(pair.g_state(), pair.o_state(), name + " masked rollout")
+    return pair
+
+
+def test_masked_rollout_tiny():
+    pair = _masked_rollout("tiny_dense", 8, 50)
+    import oracle
+    assert sum(int(oracle.parse_state(w)["counters"][2]) for w in pair.g.get_state()) == 0  # no invalid action
+
+
+def test_masked_rollout_tiny_per_resource_low_cap_mixed_table():
+    _masked_rollout("tiny_dense", 5, 50, dict(craft_mode=1, max_active_orders=2), mix="config4_population")
+
+
+def test_masked_rollout_paper_shape_specialised_kernel():
+    import oracle
+    pair = _masked_rollout("config2_paper", 6, 120)
+    assert sum(int(oracle.parse_state(w)["counters"][2]) for w in pair.g.get_state()) == 0
+
+
+def test_masked_rollout_six_resources():
+    _masked_rollout("config3_resources", 3, 60)
+
+
+def test_masked_rollout_full_size_sampled_envs():
+    cfg = inputs.configs()["headline"]
+    _masked_rollout("headline", cfg["E"], 40, env_ids=[0, 1500, cfg["E"] - 1], seed=cfg["seed"])
