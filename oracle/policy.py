@@ -52,24 +52,30 @@ def mlp_logits(net: dict, obs_rows) -> np.ndarray:
     return h2 @ w3.T + b3
 
 
-def softmax_cdf(logits_head) -> np.ndarray:
-    """Cumulative softmax probabilities of one head (binary64), last entry exactly 1."""
+def softmax_cdf(logits_head, mask=None) -> np.ndarray:
+    """Cumulative softmax probabilities of one head (binary64), 1 from the last available entry on.
+    mask (f1): actions with mask == 0 get probability exactly 0 -- they are left out
+    of the maximum and of the normalising sum, i.e. their logit is -inf."""
     l = np.asarray(logits_head, np.float64)
-    p = np.exp(l - l.max())
+    ok = np.ones(l.shape, bool) if mask is None else np.asarray(mask).astype(bool)
+    p = np.where(ok, np.exp(l - l[ok].max()), 0.0)
     c = np.cumsum(p / p.sum())
-    c[-1] = 1.0
+    c[np.flatnonzero(ok)[-1]:] = 1.0
     return c
 
 
-def sample(logits_head, u: float) -> int:
-    """First index a with u < CDF[a] (G33)."""
-    return int(np.searchsorted(softmax_cdf(logits_head), u, side="right"))
+def sample(logits_head, u: float, mask=None) -> int:
+    """First index a with u < CDF[a] (G33); an unavailable action has an empty interval."""
+    return int(np.searchsorted(softmax_cdf(logits_head, mask), u, side="right"))
 
 
-def sample_consistent(logits_head, u: float, action: int, eps: float) -> bool:
+def sample_consistent(logits_head, u: float, action: int, eps: float, mask=None) -> bool:
     """True if `action` is what `sample` returns for some u' within eps of u: u lies in the action's
-    CDF interval widened by eps (the teacher-forced acceptance test of G33)."""
-    c = softmax_cdf(logits_head)
+    CDF interval widened by eps (the teacher-forced acceptance test of G33).  Under a mask an
+    unavailable action is never consistent."""
+    if mask is not None and not mask[action]:
+        return False
+    c = softmax_cdf(logits_head, mask)
     lo = 0.0 if action == 0 else c[action - 1]
     return bool(lo - eps <= u < c[action] + eps)
 

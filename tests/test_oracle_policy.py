@@ -119,3 +119,35 @@ def test_philox_u_uses_the_pinned_generator():
     # T11 known answer: counter = key = 0 -> 6627e8d5 e169c58d bc57ac4c 9b00dbd8
     assert P.philox_u(0, 0, 0, 0, 0, 0) == (0x6627e8d5 >> 8) / 16777216.0
     assert P.philox_u(0, 0, 0, 0, 0, 3) == (0x9b00dbd8 >> 8) / 16777216.0
+
+
+# ---- f1: masked categorical ----
+
+def test_masked_softmax_hand_values_and_library():
+    from scipy.special import softmax
+    l = np.array([0.0, 5.0, 0.0, -1.0, 0.0])
+    m = np.array([1, 0, 1, 0, 1])
+    c = P.softmax_cdf(l, m)
+    assert np.allclose(c, [1 / 3, 1 / 3, 2 / 3, 2 / 3, 1.0], atol=1e-15)      # the dominant logit is unavailable
+    assert P.sample(l, 0.33, m) == 0 and P.sample(l, 0.34, m) == 2 and P.sample(l, 0.999, m) == 4
+    rng = np.random.default_rng(0)
+    for _ in range(50):
+        l = rng.normal(0, 2, 17)
+        m = rng.random(17) < 0.5
+        m[rng.integers(17)] = True
+        c = P.softmax_cdf(l, m)
+        p = np.diff(np.concatenate([[0.0], c]))
+        assert np.all(p[~m] == 0.0)
+        idx = np.flatnonzero(m)
+        assert np.allclose(p[idx][:-1], softmax(l[idx])[:-1], atol=1e-12)     # = softmax over the available sub-vector
+        for u in rng.random(20):
+            a = P.sample(l, float(u), m)
+            assert m[a] and P.sample_consistent(l, float(u), a, 0.0, m)
+
+
+def test_mask_of_ones_changes_nothing():
+    rng = np.random.default_rng(1)
+    l = rng.normal(0, 1, 44)
+    assert np.array_equal(P.softmax_cdf(l), P.softmax_cdf(l, np.ones(44, np.uint8)))
+    for u in rng.random(30):
+        assert P.sample(l, float(u)) == P.sample(l, float(u), np.ones(44, np.uint8))
