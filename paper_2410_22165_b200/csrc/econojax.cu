@@ -322,6 +322,15 @@ int launch_policy(ej_env* h, const float* obs, int32_t* actions, int32_t* gov_ac
     PolicyLaunch pl;
     memset(&pl, 0, sizeof(pl));
     fill_job(h, pl.job[0], h->pop_net, obs, c.D_pop, c.E * c.N, c.N, -1, 0u, actions, pop_logits);
+    if (h->masking) {  // f1: the population head samples among the available actions
+        PolicyMask& k = pl.job[0].mask;
+        k.on = 1;
+        k.o_coin = c.o_coin; k.o_mask = c.o_mask; k.o_inv = c.o_inv; k.NS = c.N4;
+        k.R = c.R; k.P = c.P; k.M = c.M; k.craft_mode = c.craft_mode; k.craft_units = c.craft_units;
+        k.craft_distinct = c.craft_distinct; k.base_buy = c.base_buy; k.base_sell = c.base_sell; k.A = c.A;
+        k.allow_noop = c.allow_noop;
+        for (int i = 0; i < EJ_MAX_PRICES; ++i) k.prices[i] = c.prices[i];
+    }
     int smem = policy_smem_bytes(h->pop_net, c.D_pop), gov_ctas = 0;
     if (gov_actions) {
         fill_job(h, pl.job[1], h->gov_net, obs + c.gov_obs_offset, c.D_gov_pad, c.E, 1, c.N, 1u, gov_actions, gov_logits);

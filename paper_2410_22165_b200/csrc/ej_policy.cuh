@@ -35,8 +35,18 @@ struct PolicyNet {
     int nch;               // 16-column chunks a head's logits span at most (register-resident sampler if <= 5)
 };
 
+// f1: what the masked sampler needs to rebuild a row's action mask from the env state blob
+// (same rules as ej_mask_kernel).
+struct PolicyMask {
+    int on;
+    int o_coin, o_mask, o_inv, NS;  // blob-relative byte offsets, stride of the per-agent arrays
+    int R, P, M, craft_mode, craft_units, craft_distinct, base_buy, base_sell, A, allow_noop;
+    int prices[EJ_MAX_PRICES];
+};
+
 struct PolicyArgs {
     PolicyNet net;
+    PolicyMask mask;         // population job only
     const float* obs;        // first row
     int row_stride;          // floats between rows
     int rows;                // number of rows
@@ -302,6 +312,89 @@ __device__ __forceinline__ int sample_head_sweeps(uint32_t taddr_row, const floa
     return pick;
 }
 
+// f1 masked categorical for a single-head row: unavailable actions are left out of
+// the maximum, the sum and the running sum (their probability is exactly 0).  Out of line and
+// sweep-based: the unmasked samplers keep their registers; this path is an option, not the headline.
+__device__ __noinline__ int sample_head_masked(uint32_t taddr_row, const float* b3, int n_logits, float u, float* logits_row,
+                                               const PolicyMask& k, const uint8_t* blob, int agent) {
+    unsigned long long av[4] = {0ull, 0ull, 0ull, 0ull};
+    auto set = [&](int a) {
+        const unsigned long long bit = 1ull << (a & 63);
+        const int w = a >> 6;
+        av[0] |= w == 0 ? bit : 0ull; av[1] |= w == 1 ? bit : 0ull; av[2] |= w == 2 ? bit : 0ull; av[3] |= w == 3 ? bit : 0ull;
+    };
+    const float coin = ((const float*)(blob + k.o_coin))[agent];
+    const bool room = __popc(((const uint32_t*)(blob + k.o_mask))[agent]) < k.M;
+    const int* inv = (const int*)(blob + k.o_inv);
+    int enough = 0;
+    for (int r = 0; r < k.R; ++r) {
+        set(r);  // gather: always
+        enough += inv[r * k.NS + agent] >= k.craft_units;
+    }
+    if (k.craft_mode == EJ_CRAFT_PER_RESOURCE) {
+        for (int r = 0; r < k.R; ++r)
+            if (inv[r * k.NS + agent] >= k.craft_units) set(k.R + r);
+    } else if (enough >= k.craft_distinct) {
+        set(k.R);
+    }
+    if (room) {
+        for (int r = 0; r < k.R; ++r) {
+            const bool has = inv[r * k.NS + agent] >= 1;
+            for (int p = 0; p < k.P; ++p) {
+                if (coin >= (float)k.prices[p]) set(k.base_buy + r * k.P + p);
+                if (has) set(k.base_sell + r * k.P + p);
+            }
+        }
+    }
+    if (k.allow_noop) set(k.A - 1);
+    auto ok = [&](int col) {
+        const int w = col >> 6;
+        const unsigned long long word = w == 0 ? av[0] : w == 1 ? av[1] : w == 2 ? av[2] : av[3];
+        return ((word >> (col & 63)) & 1ull) != 0ull;
+    };
+    float mx = -INFINITY;
+    for (int c = 0; c < n_logits; c += 16) {
+        float v[16];
+        tmem_ld16(taddr_row + c, v);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int col = c + j;
+            if (col < n_logits) {
+                const float l = v[j] + b3[col];
+                if (logits_row) logits_row[col] = l;
+                if (ok(col)) mx = fmaxf(mx, l);
+            }
+        }
+    }
+    float s = 0.0f;
+    for (int c = 0; c < n_logits; c += 16) {
+        float v[16];
+        tmem_ld16(taddr_row + c, v);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int col = c + j;
+            if (col < n_logits && ok(col)) s += __expf(v[j] + b3[col] - mx);
+        }
+    }
+    const float target = u * s;
+    float cum = 0.0f;
+    int pick = -1, last_ok = 0;
+    for (int c = 0; c < n_logits; c += 16) {
+        float v[16];
+        tmem_ld16(taddr_row + c, v);
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+            const int col = c + j;
+            if (col < n_logits && ok(col)) {
+                cum += __expf(v[j] + b3[col] - mx);
+                last_ok = col;
+                if (pick < 0 && target < cum) pick = col;
+            }
+        }
+    }
+    return pick >= 0 ? pick : last_ok;
+}
+
 __device__ __forceinline__ void group_sync(int grp) { asm volatile("bar.sync %0, %1;\n" ::"r"(grp + 1), "r"(PTILE) : "memory"); }
 
 // 1-D TMA bulk copy global -> shared, completion on an mbarrier (bytes and both addresses multiples of 16).
@@ -435,6 +528,9 @@ __global__ void __launch_bounds__(PGROUPS* PTILE, 1) ej_policy_kernel(const __gr
             const int lo = h * n.head, hi = lo + n.head;
             float* lrow = (a.logits && live) ? a.logits + (size_t)row * n.n_out : nullptr;
             int pick;
+            if (a.mask.on) {  // f1: single-head population job (uniform over the CTA)
+                pick = sample_head_masked(taddr_row, b3, n.n_out, u, lrow, a.mask, a.state + (size_t)env * a.blob_stride, agent);
+            } else
             switch (n.nch) {
                 case 1: pick = sample_head<1>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
                 case 2: pick = sample_head<2>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;

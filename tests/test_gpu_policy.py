@@ -236,3 +236,46 @@ def _teacher_step(pair, acts_sel, gov_sel):
     """Step the 1-env oracles of a sampled-env Pair with already-selected action rows."""
     outs = [o.step(acts_sel[k:k + 1], gov_sel[k:k + 1]) for k, o in enumerate(pair.o)]
     return tuple(np.concatenate([x[j] for x in outs]) for j in range(4))
+
+
+def test_masked_policy_rollout_teacher_forced():
+    """f1 with the policy head: under ej_set_action_masking every sampled population
+    action is available in the oracle's mask of the state before the step, is eps-consistent with
+    the oracle's MASKED categorical, and the env never counts an invalid action."""
+    import torch
+
+    cfg = inputs.configs()["config5_policy"]
+    N, R, E, T = cfg["N"], cfg["R"], 4, 48
+    params = dict(cfg["params"], tax_period=16)
+    pair = Pair(E, N, R, params, cfg["seed"])
+    g = pair.g
+    pop, gov = inputs.policy_weights(cfg, seed=3, std=0.3, bias_std=0.1)
+    g.set_policy(pop, gov)
+    g.set_action_masking(True)
+    act_ring = torch.zeros((T, E, N), dtype=torch.int32, device="cuda")
+    gov_ring = torch.zeros((T, E, g.B), dtype=torch.int32, device="cuda")
+    pl_ring = torch.zeros((T, E * N, g.A), dtype=torch.float32, device="cuda")
+    g.rollout(T, ring_depth=T, actions_ring=act_ring, gov_actions_ring=gov_ring, pop_logits_ring=pl_ring)
+    torch.cuda.synchronize()
+    a_out, g_out = act_ring.cpu().numpy(), gov_ring.cpu().numpy()
+    pl = pl_ring.cpu().numpy().reshape(T, E, N, -1)
+    o_pop, o_gov = pair.o[0].observe()
+    amb = tot = masked_out = 0
+    for t in range(T):
+        mask = pair.o[0].action_mask()
+        masked_out += int((mask == 0).sum())
+        ol_pop = OP.mlp_logits(pop, o_pop.reshape(E * N, -1)).reshape(E, N, -1)
+        check_logits(pl[t], ol_pop, "t=%d population logits (reported unmasked)" % t)
+        for e in range(E):
+            for i in range(N):
+                a = int(a_out[t, e, i])
+                assert mask[e, i, a] == 1, "t=%d env %d agent %d: unavailable action %d sampled" % (t, e, i, a)
+                if t % 6 == 0:
+                    u = OP.philox_u(cfg["seed"], e, i, t, 0, 0)
+                    assert OP.sample_consistent(ol_pop[e, i], u, a, EPS_CDF, mask[e, i]), "t=%d env %d agent %d action %d u=%g" % (t, e, i, a, u)
+                    amb += OP.sample(ol_pop[e, i], u, mask[e, i]) != a
+                    tot += 1
+        o_pop, o_gov, _, _ = pair.o[0].step(a_out[t], g_out[t])
+    compare_state(pair.g_state(), pair.o_state(), "masked policy rollout final state")
+    assert masked_out > 0 and amb <= max(2, 0.01 * tot)
+    assert sum(int(oracle.parse_state(w)["counters"][2]) for w in pair.g.get_state()) == 0
