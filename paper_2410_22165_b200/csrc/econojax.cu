@@ -149,6 +149,7 @@ void build_layout(DevCfg& c) {
     } else {
         c.o_mb = take(R * NP * 4);
         c.o_ma = take(R * NP * 4);
+        c.o_coltab = take(3 * c.D_pop * 4);  // column table of the unstaged observation loop
         c.o_stage = o;
     }
     c.smem_bytes = o;
@@ -162,32 +163,39 @@ void select_step_kernel(ej_env* h) {
     const DevCfg& c = h->c;
     h->step_fn = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0>;
     h->step_RT = h->step_PT = 0;
-    auto pick = [&](auto rt, auto pt, auto nt, auto bt) {
+    // pf = 1 also fixes the paper's mechanics (Table 2; PF in ej_device.cuh)
+    auto pick = [&](auto rt, auto pt, auto nt, auto bt, auto pf) {
         constexpr int RT = decltype(rt)::value, PT = decltype(pt)::value, NT = decltype(nt)::value, BT = decltype(bt)::value;
-        // NT > 0 variants also fix the paper's mechanics (PF = 1 in ej_device.cuh)
+        constexpr int PF = decltype(pf)::value;
         const bool paper = c.M == 15 && c.Mp_log2 == 4 && c.K == 0 && c.craft_mode == EJ_CRAFT_SINGLE && c.craft_units == 2 &&
                            c.craft_distinct == 2 && c.allow_noop == 1 && c.stage_obs == 1;
-        if (c.R == RT && c.P == PT && (NT == 0 || (c.N == NT && c.B == BT && paper))) {
-            h->step_fn = ej_step_kernel<MT, NS, RT, PT, NT, BT, (NT > 0)>;
+        if (c.R == RT && c.P == PT && (NT == 0 || (c.N == NT && c.B == BT)) && (PF == 0 || paper)) {
+            h->step_fn = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF>;
             h->step_RT = RT; h->step_PT = PT;
         }
     };
-    using std::integral_constant;
+    using I0 = std::integral_constant<int, 0>;
+    using I1 = std::integral_constant<int, 1>;
+    using I2 = std::integral_constant<int, 2>;
+    using I7 = std::integral_constant<int, 7>;
+    using I10 = std::integral_constant<int, 10>;
     if constexpr (MT == 128) {
-        // BASELINE.json's N = 100 shapes: R, P, N and B are compile-time constants
+        // BASELINE.json's N = 100 shapes: R, P, N, B and the mechanics are compile-time constants
         if constexpr (NS == tight_stride(128)) {
-            pick(integral_constant<int, 2>(), integral_constant<int, 10>(), integral_constant<int, 100>(), integral_constant<int, 7>());
+            using I100 = std::integral_constant<int, 100>;
+            pick(I2(), I10(), I100(), I7(), I1());
 #ifndef EJ_DEV_ONLY_128
-            pick(integral_constant<int, 3>(), integral_constant<int, 10>(), integral_constant<int, 100>(), integral_constant<int, 7>());
-            pick(integral_constant<int, 6>(), integral_constant<int, 10>(), integral_constant<int, 100>(), integral_constant<int, 7>());
+            pick(std::integral_constant<int, 3>(), I10(), I100(), I7(), I1());
+            pick(std::integral_constant<int, 6>(), I10(), I100(), I7(), I1());
 #endif
         }
 #ifndef EJ_DEV_ONLY_128
-        if (h->step_RT == 0) pick(integral_constant<int, 2>(), integral_constant<int, 5>(), integral_constant<int, 0>(), integral_constant<int, 0>());
+        if (h->step_RT == 0) pick(I2(), std::integral_constant<int, 5>(), I0(), I0(), I0());
 #endif
     }
     if constexpr (MT == 1024 && NS == 1024) {
-        pick(integral_constant<int, 2>(), integral_constant<int, 10>(), integral_constant<int, 0>(), integral_constant<int, 0>());
+        // configs[3]: N = 1000 with a book cap (mechanics stay runtime)
+        pick(I2(), I10(), std::integral_constant<int, 1000>(), I7(), I0());
     }
 }
 

@@ -65,7 +65,7 @@ struct DevCfg {
     int o_blob, o_scratch1;  // absolute: blob start (= Lay<Npad>::blob), first byte after the blob
     // scratch section offsets (bytes from the shared-memory base; all after the blob)
     int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma, o_bucket, o_sorted;
-    int o_gcnt, o_goff, o_resq, o_shrow, o_govrow, o_misc, o_cdf, o_stage;
+    int o_gcnt, o_goff, o_resq, o_shrow, o_govrow, o_misc, o_cdf, o_coltab, o_stage;
     int smem_bytes;
     unsigned long long gov_obs_offset, obs_floats;
 };
@@ -160,6 +160,7 @@ struct Sm {
     __device__ __forceinline__ int* goff() const { return at<int>(c.o_goff); }
     __device__ __forceinline__ uint32_t* cdf() const { return at<uint32_t>(c.o_cdf); }
     __device__ __forceinline__ float* stage() const { return at<float>(c.o_stage); }
+    __device__ __forceinline__ uint32_t* coltab() const { return at<uint32_t>(c.o_coltab); }
 };
 
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), G30.
@@ -608,20 +609,18 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
     }
     // ---- population rows when they cannot go out as one bulk store: coalesced loop ----
     if (obs && !staged) {
-        const int D = D_pop, priv = 3 * R + 4, total = N * D;
+        // element (i, k) = scale_k * value of column k's source array at agent i: the column table
+        // (build_coltab) replaces a chain of ten compares per element
+        extern __shared__ __align__(16) uint8_t ej_smem[];
+        const int D = D_pop, total = N * D;
+        const uint32_t* tab = m.coltab();
         float* dst = obs + (size_t)e * total;
         for (int idx = tid; idx < total; idx += NPAD) {
             const int i = idx / D, k = idx - i * D;
-            float v;
-            if (k >= priv) v = m.shrow()[k - priv];
-            else if (k == 0) v = __fmul_rn(m.coin()[i], c.s_coin);
-            else if (k <= R) v = __fmul_rn((float)m.inv()[(k - 1) * N4 + i], c.s_count);
-            else if (k == R + 1) v = __fmul_rn((float)m.esc_coin()[i], c.s_coin);
-            else if (k <= 2 * R + 1) v = __fmul_rn((float)m.esc_res()[(k - R - 2) * N4 + i], c.s_count);
-            else if (k <= 3 * R + 1) v = m.SG()[(k - 2 * R - 2) * N4 + i];
-            else if (k == 3 * R + 2) v = m.SC()[i];
-            else v = __fmul_rn(m.labor()[i], c.s_labor);
-            dst[idx] = v;
+            const uint32_t base = tab[k], st = tab[D + k];
+            const uint32_t w = *reinterpret_cast<const uint32_t*>(ej_smem + base + (uint32_t)i * (st & 4u));
+            const float f = (st >> 31) ? (float)(int)w : __uint_as_float(w);
+            dst[idx] = __fmul_rn(f, __uint_as_float(tab[2 * D + k]));  // scale 1 for the unscaled columns: exact
         }
         __syncthreads();  // the loop reads other agents' state: the next step must not start updating it
     }
@@ -676,6 +675,32 @@ __device__ __noinline__ int masked_draw(const DevCfg& c, const Sm<NS>& m, int ti
         target = ((unsigned long long)x0 * S) >> 32;  // S <= 2^32: no overflow
     }
     return pick >= 0 ? pick : first_ok;
+}
+
+// Column table of the population observation row (G25) for shapes whose tile does not fit
+// the staging buffer: per column k the byte offset of its source array in shared memory, the
+// per-agent stride (4, or 0 for the env-wide tail) with bit 31 = integer source, and the scale.
+template <int NS>
+__device__ __forceinline__ void build_coltab(const DevCfg& c, const Sm<NS>& m, int tid, int nthreads) {
+    extern __shared__ __align__(16) uint8_t ej_smem[];
+    if (c.stage_obs) return;
+    const int R = c.R, D = c.D_pop, priv = 3 * R + 4;
+    auto off = [&](const void* p) { return (uint32_t)((const uint8_t*)p - ej_smem); };
+    for (int k = tid; k < D; k += nthreads) {
+        uint32_t base, st = 4u;
+        float sc = 1.0f;
+        if (k >= priv) { base = off(m.shrow() + (k - priv)); st = 0u; }
+        else if (k == 0) { base = off(m.coin()); sc = c.s_coin; }
+        else if (k <= R) { base = off(m.inv() + (k - 1) * NS); st |= 0x80000000u; sc = c.s_count; }
+        else if (k == R + 1) { base = off(m.esc_coin()); st |= 0x80000000u; sc = c.s_coin; }
+        else if (k <= 2 * R + 1) { base = off(m.esc_res() + (k - R - 2) * NS); st |= 0x80000000u; sc = c.s_count; }
+        else if (k <= 3 * R + 1) base = off(m.SG() + (k - 2 * R - 2) * NS);
+        else if (k == 3 * R + 2) base = off(m.SC());
+        else { base = off(m.labor()); sc = c.s_labor; }
+        m.coltab()[k] = base;
+        m.coltab()[D + k] = st;
+        m.coltab()[2 * D + k] = __float_as_uint(sc);
+    }
 }
 
 // Inputs and outputs of step `s` of a launch (ring slot `slot`), resolved where they are used:
@@ -1114,6 +1139,7 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
         for (int l = tid; l < c.n_levels; l += NPAD) m.ahead()[l] = NIL;
     if (!io.actions)
         for (int i = tid; i < c.A; i += NPAD) m.cdf()[i] = io.cdf[i];
+    build_coltab<NS>(c, m, tid, NPAD);
     __syncthreads();
     StepPtrs p{io, c, 0, 0};
 #pragma unroll 1
@@ -1138,6 +1164,7 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
     __syncthreads();
     const int t = m.hdr()->t;
+    build_coltab<NS>(c, m, tid, NPAD);
     if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
     if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
     if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
