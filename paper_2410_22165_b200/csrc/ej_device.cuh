@@ -893,7 +893,9 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             }
         }
         __syncthreads();
-        const unsigned long long mine = ((unsigned long long)x2 << 32) | (unsigned long long)tid;
+        // arrival key | agent | level: ordered by (key, agent) (G11); the level rides along so that the
+        // ranking loop needs no second, dependent load
+        const unsigned long long mine = ((unsigned long long)x2 << 32) | ((unsigned long long)tid << 16) | (unsigned long long)(lvl >= 0 ? lvl : 0);
         if (lvl >= 0) m.bucket()[m.goff()[grp] + pos] = mine;
         __syncthreads();
         int before = 0, gbase = 0, gn = 0;
@@ -903,7 +905,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
             int brank = 0;
             for (int k = 0; k < gn; ++k) {
                 const unsigned long long o = m.bucket()[gbase + k];
-                const int lj = m.cinfo()[(int)(o & 0xFFFFFFFFu)];
+                const int lj = (int)(o & 0xFFFFu);
                 const bool earlier = o < mine, same = lj == lvl;
                 brank += earlier;
                 lrank += same && earlier;
