@@ -335,8 +335,8 @@ def main():
             pass
     if world == 1 and not args.no_cpu_baseline:
         cores = max(1, min(os.cpu_count() or 1, 32))
-        per, osteps = 48, min(1000, T)
-        # ~10-30 s of CPU work: (cores x 48 envs + 48 envs on one core) x 1000 steps, after a short warm-up
+        per, osteps = 160, min(1000, T)
+        # ~10-30 s of CPU work: (cores x 160 envs + 160 envs on one core) x 1000 steps, after a short warm-up
         oracle_sample(cfg, per, 5, cores, cfg["seed"])
         v, dt = oracle_sample(cfg, per, osteps, cores, cfg["seed"])
         v1, dt1 = oracle_sample(cfg, per, osteps, 1, cfg["seed"])

@@ -40,5 +40,11 @@ if __name__ == "__main__":
     env = run("config5_policy", 2, 4, tax_period=3)
     env.set_policy(*inputs.policy_weights(cfg, seed=1, std=0.3))
     env.rollout(4)
+    env.set_action_masking(True)   # f1: masked policy sampler, mask kernel, masked table generator
+    env.rollout(3)
+    env.action_mask()
+    env2 = run("config2_paper", 2, 3)
+    env2.set_action_masking(True)
+    env2.rollout(6)
     torch.cuda.synchronize()
     print("driver done")
