@@ -169,7 +169,14 @@ void select_step_kernel(ej_env* h) {
         constexpr int PF = decltype(pf)::value;
         const bool paper = c.M == 15 && c.Mp_log2 == 4 && c.K == 0 && c.craft_mode == EJ_CRAFT_SINGLE && c.craft_units == 2 &&
                            c.craft_distinct == 2 && c.allow_noop == 1 && c.stage_obs == 1;
-        if (c.R == RT && c.P == PT && (NT == 0 || (c.N == NT && c.B == BT)) && (PF == 0 || paper)) {
+        bool lay_ok = true;
+        if constexpr (PF == 1) {  // the kernel's compile-time layout must be the one build_layout() made
+            using S = StaticLay<NS, RT, PT, NT>;
+            lay_ok = c.o_esc_res == S::esc_res && c.o_SG == S::SG && c.o_head == S::head && c.o_tail == S::tail && c.o_cnt == S::cnt &&
+                     c.o_pool == S::pool && c.blob_bytes == S::blob_bytes && c.o_ahead == S::ahead && c.o_cdf == S::cdf &&
+                     c.o_stage == S::stage && c.o_mb == S::mb && c.o_ma == S::ma;
+        }
+        if (c.R == RT && c.P == PT && (NT == 0 || (c.N == NT && c.B == BT)) && (PF == 0 || (paper && lay_ok))) {
             h->step_fn = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF>;
             h->step_RT = RT; h->step_PT = PT;
         }

@@ -117,9 +117,33 @@ struct Lay {
     static_assert(blob % 16 == 0 && inv % 16 == 0, "16-byte alignment");
 };
 
-template <int NP>
+// Offsets of the R-, P-, N-dependent sections when those are compile-time constants and the
+// paper's mechanics hold (16 pool slots per agent, no book cap: PF = 1 in the step kernel): the
+// same arithmetic as build_layout() in econojax.cu, which checks the two against each other
+// before it selects a kernel that relies on this.
+constexpr int lay_align16(int x) { return (x + 15) & ~15; }
+template <int NP, int R, int P, int N>
+struct StaticLay {
+    static constexpr int nl = 2 * R * P, A = 2 * R * P + R + 2;
+    static constexpr int esc_res = lay_align16(Lay<NP>::inv + R * NP * 4);
+    static constexpr int SG = lay_align16(esc_res + R * NP * 4);
+    static constexpr int head = lay_align16(SG + R * NP * 4);
+    static constexpr int tail = lay_align16(head + nl * 2);
+    static constexpr int cnt = lay_align16(tail + nl * 2);
+    static constexpr int pool = lay_align16(cnt + 2 * nl * 4);
+    static constexpr int blob_bytes = lay_align16(pool + (N << 4) * 4);
+    static constexpr int ahead = Lay<NP>::blob + blob_bytes;  // absolute from here on
+    static constexpr int cdf = lay_align16(ahead + nl * 4);
+    static constexpr int stage = lay_align16(cdf + A * 4);
+    static constexpr int mb = stage, ma = stage + R * NP * 4;
+};
+
+// View of one economy's shared memory.  SR > 0: static layout (StaticLay<NP, SR, SP, SN>).
+template <int NP, int SR = 0, int SP = 0, int SN = 0>
 struct Sm {
     using L = Lay<NP>;
+    using S = StaticLay<NP, (SR > 0 ? SR : 1), (SP > 0 ? SP : 1), (SN > 0 ? SN : 1)>;
+    static constexpr bool ST = SR > 0;
     const DevCfg& c;
     template <class T>
     __device__ __forceinline__ static T* at(int off) {
@@ -135,12 +159,12 @@ struct Sm {
     __device__ __forceinline__ uint32_t* mask() const { return at<uint32_t>(L::blob + L::mask); }
     __device__ __forceinline__ double* cf() const { return at<double>(L::blob + L::cf); }
     __device__ __forceinline__ int* inv() const { return at<int>(L::blob + L::inv); }
-    __device__ __forceinline__ int* esc_res() const { return at<int>(L::blob + c.o_esc_res); }
-    __device__ __forceinline__ float* SG() const { return at<float>(L::blob + c.o_SG); }
-    __device__ __forceinline__ uint16_t* head() const { return at<uint16_t>(L::blob + c.o_head); }
-    __device__ __forceinline__ uint16_t* tail() const { return at<uint16_t>(L::blob + c.o_tail); }
-    __device__ __forceinline__ int* cnt() const { return at<int>(L::blob + c.o_cnt); }  // [2][n_levels]: buffer (t & 1) is current
-    __device__ __forceinline__ uint32_t* pool() const { return at<uint32_t>(L::blob + c.o_pool); }
+    __device__ __forceinline__ int* esc_res() const { return at<int>(L::blob + (ST ? S::esc_res : c.o_esc_res)); }
+    __device__ __forceinline__ float* SG() const { return at<float>(L::blob + (ST ? S::SG : c.o_SG)); }
+    __device__ __forceinline__ uint16_t* head() const { return at<uint16_t>(L::blob + (ST ? S::head : c.o_head)); }
+    __device__ __forceinline__ uint16_t* tail() const { return at<uint16_t>(L::blob + (ST ? S::tail : c.o_tail)); }
+    __device__ __forceinline__ int* cnt() const { return at<int>(L::blob + (ST ? S::cnt : c.o_cnt)); }  // [2][n_levels]: buffer (t & 1) is current
+    __device__ __forceinline__ uint32_t* pool() const { return at<uint32_t>(L::blob + (ST ? S::pool : c.o_pool)); }
     __device__ __forceinline__ uint32_t* key() const { return at<uint32_t>(L::key); }
     __device__ __forceinline__ uint32_t* cslot() const { return at<uint32_t>(L::cslot); }
     __device__ __forceinline__ uint32_t* anext() const { return at<uint32_t>(L::anext); }
@@ -151,15 +175,15 @@ struct Sm {
     __device__ __forceinline__ float* shrow() const { return at<float>(L::shrow); }
     __device__ __forceinline__ float* govrow() const { return at<float>(L::govrow); }
     __device__ __forceinline__ unsigned long long* misc() const { return at<unsigned long long>(L::misc); }  // [0] tax pool in 2^-20 coin
-    __device__ __forceinline__ uint32_t* ahead() const { return at<uint32_t>(c.o_ahead); }
-    __device__ __forceinline__ uint32_t* mb() const { return at<uint32_t>(c.o_mb); }
-    __device__ __forceinline__ uint32_t* ma() const { return at<uint32_t>(c.o_ma); }
+    __device__ __forceinline__ uint32_t* ahead() const { return at<uint32_t>(ST ? S::ahead : c.o_ahead); }
+    __device__ __forceinline__ uint32_t* mb() const { return at<uint32_t>(ST ? S::mb : c.o_mb); }
+    __device__ __forceinline__ uint32_t* ma() const { return at<uint32_t>(ST ? S::ma : c.o_ma); }
     __device__ __forceinline__ unsigned long long* bucket() const { return at<unsigned long long>(c.o_bucket); }
     __device__ __forceinline__ uint32_t* sorted() const { return at<uint32_t>(c.o_sorted); }
     __device__ __forceinline__ int* gcnt() const { return at<int>(c.o_gcnt); }
     __device__ __forceinline__ int* goff() const { return at<int>(c.o_goff); }
-    __device__ __forceinline__ uint32_t* cdf() const { return at<uint32_t>(c.o_cdf); }
-    __device__ __forceinline__ float* stage() const { return at<float>(c.o_stage); }
+    __device__ __forceinline__ uint32_t* cdf() const { return at<uint32_t>(ST ? S::cdf : c.o_cdf); }
+    __device__ __forceinline__ float* stage() const { return at<float>(ST ? S::stage : c.o_stage); }
     __device__ __forceinline__ uint32_t* coltab() const { return at<uint32_t>(c.o_coltab); }
 };
 
@@ -376,8 +400,8 @@ __device__ __forceinline__ void bit_select(const uint32_t (&key)[EPL], int r0, i
     hi = r1 >= __reduce_add_sync(FULL, b) ? __reduce_min_sync(FULL, mn) : res;
 }
 
-template <int NP, int NT>
-__device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm<NP>& m, int k, double mean, double var, float lo, float hi,
+template <int NP, int NT, class SM>
+__device__ __forceinline__ void gov_triple(const DevCfg& c, const SM& m, int k, double mean, double var, float lo, float hi,
                                            float scale) {
     const int N = NT > 0 ? NT : c.N;
     const float sd = __fsqrt_rn((float)var);
@@ -395,8 +419,8 @@ __device__ __forceinline__ void gov_triple(const DevCfg& c, const Sm<NP>& m, int
 // instance of this code per kernel (the caller loops over k without unrolling): the unrolled
 // network is most of the kernel's instruction footprint.
 //   mode 0 = step, 1 = finished env (reward 0), 2 = observe only
-template <int EPL, int NS, int NT>
-__device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, int k, int lane, int mode, int e, float* rew) {
+template <int EPL, int NS, int NT, class SM>
+__device__ __forceinline__ void metric_stats(const DevCfg& c, const SM& m, int k, int lane, int mode, int e, float* rew) {
     const int N = NT > 0 ? NT : c.N;  // NT > 0: population size known at compile time
     const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
     const float* farr = k == 0 ? m.coin() : k == 1 ? m.labor() : m.income();
@@ -463,8 +487,8 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const Sm<NS>& m, i
 // sum of squares are exact integers (REDUX), so mean and variance (N sum x^2 - (sum x)^2) / N^2
 // need no second pass; the median walks from last step's value on the integer keys, with the
 // bitwise search as fall-back.
-template <int EPL, int NS, int NT>
-__device__ __forceinline__ void int_metric_stats(const DevCfg& c, const Sm<NS>& m, int r, int lane) {
+template <int EPL, int NS, int NT, class SM>
+__device__ __forceinline__ void int_metric_stats(const DevCfg& c, const SM& m, int r, int lane) {
     const int N = NT > 0 ? NT : c.N;
     const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
     const int* iarr = m.inv() + r * NS;
@@ -507,8 +531,8 @@ __device__ __forceinline__ void int_metric_stats(const DevCfg& c, const Sm<NS>& 
 }
 
 // Shared tail of the population rows: market statistics of the post-step books.
-template <int PT, int NP>
-__device__ __forceinline__ void write_market_row(const DevCfg& c, const Sm<NP>& m, int r, const int* cnt) {
+template <int PT, class SM>
+__device__ __forceinline__ void write_market_row(const DevCfg& c, const SM& m, int r, const int* cnt) {
     const int P = PT > 0 ? PT : c.P;
     int best_bid = 0, best_ask = 0, nb = 0, na = 0;
     for (int p = 0; p < P; ++p) {
@@ -525,8 +549,8 @@ __device__ __forceinline__ void write_market_row(const DevCfg& c, const Sm<NP>& 
     o[3] = __fmul_rn((float)na, c.s_count);
     o[4] = __fmul_rn((float)m.hdr()->last_price[r], c.s_price);
 }
-template <int NP>
-__device__ __forceinline__ void write_timers(const DevCfg& c, const Sm<NP>& m, int tq, int tq_in_period) {
+template <class SM>
+__device__ __forceinline__ void write_timers(const DevCfg& c, const SM& m, int tq, int tq_in_period) {
     m.shrow()[5 * c.R + c.B] = __fdiv_rn((float)tq_in_period, (float)c.period);
     m.shrow()[5 * c.R + c.B + 1] = __fdiv_rn((float)tq, (float)c.T);
 }
@@ -536,8 +560,8 @@ __device__ __forceinline__ void write_timers(const DevCfg& c, const Sm<NP>& m, i
 //   mode     0 = step, 1 = finished env (rewards 0), 2 = observe only
 //   rows     0 = rewrite only the columns that change every step, 1 = also the tax rates,
 //            2 = every column (first step of a launch: skills)
-template <int NPAD, int NS, int RT, int NT, int BT, int PF>
-__device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
+template <int NPAD, int NS, int RT, int NT, int BT, int PF, class SM>
+__device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
                         double cf_pre, float* obs, float* rew) {
     constexpr int NW = NPAD / 32, EPL = NPAD / 32;
     // RT, NT, BT > 0: resource count, population size, bracket count known at compile time
@@ -628,8 +652,8 @@ __device__ void outputs(const DevCfg& c, const Sm<NS>& m, int tid, int e, int mo
 
 // f1 masked sampling, the table generator.  Out of line: the unmasked hot path
 // keeps its registers and instruction footprint.
-template <int NS>
-__device__ __noinline__ int masked_draw(const DevCfg& c, const Sm<NS>& m, int tid, uint32_t x0, int R, int P, int M, int craft_mode,
+template <int NS, class SM>
+__device__ __noinline__ int masked_draw(const DevCfg& c, const SM& m, int tid, uint32_t x0, int R, int P, int M, int craft_mode,
                             int craft_units, int craft_distinct, int base_buy, int base_sell, int A) {
     constexpr int N4 = NS;
     // f1: the table restricted to this agent's available actions, renormalised with
@@ -680,8 +704,8 @@ __device__ __noinline__ int masked_draw(const DevCfg& c, const Sm<NS>& m, int ti
 // Column table of the population observation row (G25) for shapes whose tile does not fit
 // the staging buffer: per column k the byte offset of its source array in shared memory, the
 // per-agent stride (4, or 0 for the env-wide tail) with bit 31 = integer source, and the scale.
-template <int NS>
-__device__ __forceinline__ void build_coltab(const DevCfg& c, const Sm<NS>& m, int tid, int nthreads) {
+template <int NS, class SM>
+__device__ __forceinline__ void build_coltab(const DevCfg& c, const SM& m, int tid, int nthreads) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
     if (c.stage_obs) return;
     const int R = c.R, D = c.D_pop, priv = 3 * R + 4;
@@ -722,8 +746,8 @@ struct StepPtrs {
 // Phases P1-P4 of one environment step on the state in shared memory (G1: actions -> match ->
 // expire -> tax); returns the pre-step values the rewards need.  `first` = first step of this
 // launch (full observation rows).
-template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF>
-__device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int tid, int e, const StepPtrs& io, bool first, int t,
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, class SM>
+__device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid, int e, const StepPtrs& io, bool first, int t,
                                           float& coin_pre, float& labor_pre, double& cf_pre, int& rows) {
     // RT, PT > 0: resource and price counts known at compile time (shape-specialised variants)
     const int N = NT > 0 ? NT : c.N, B = BT > 0 ? BT : c.B, R = RT > 0 ? RT : c.R, P = PT > 0 ? PT : c.P, nl = (RT > 0 && PT > 0) ? 2 * RT * PT : c.n_levels;
@@ -1100,8 +1124,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const Sm<NS>& m, int 
 
 // One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
 // observations.  outputs() has this single call site (instruction footprint).
-template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF>
-__device__ void env_step(const DevCfg& c, const Sm<NS>& m, int tid, int e, const StepPtrs& io, bool first) {
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, class SM>
+__device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const StepPtrs& io, bool first) {
     const int t = m.hdr()->t;
     // the previous step's bulk stores must have read the staging tile before it is rewritten
     if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
@@ -1131,7 +1155,7 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
     extern __shared__ __align__(16) uint8_t ej_smem[];
     uint8_t* const sblob = ej_smem + Lay<NS>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
-    const Sm<NS> m{c};
+    const Sm<NS, (PF ? RT : 0), (PF ? PT : 0), (PF ? NT : 0)> m{c};
     uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
     for (int i = tid; i < Lay<NS>::blob / 16; i += NPAD) ((uint4*)ej_smem)[i] = make_uint4(0u, 0u, 0u, 0u);
