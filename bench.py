@@ -271,6 +271,28 @@ def main():
         step_ms = e0.elapsed_time(e1) / ks
         run_steps.t += ks + min(3, ks)
 
+    # ---- f2: the same rollout with factored observations (private block + env-wide block), reported beside it ----
+    fx = None
+    if not use_policy and (N * (3 * R + 4)) % 4 == 0 and N * env.D_pop * 4 <= 64 * 1024:
+        priv, shared, govr = env.new_factored_obs(depth)
+        env.reset(cfg["seed"])
+        kf = min(K, chunk)
+        for _ in range(2):
+            env.rollout(min(W, chunk), ring_depth=depth, actions_in=acts, gov_actions_in=gov, rew_ring=rew_ring, done_ring=done_ring,
+                        obs_priv_ring=priv, obs_shared_ring=shared, obs_gov_ring=govr)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        env.rollout(kf, ring_depth=depth, actions_in=acts, gov_actions_in=gov, rew_ring=rew_ring, done_ring=done_ring,
+                    obs_priv_ring=priv, obs_shared_ring=shared, obs_gov_ring=govr)
+        e1.record()
+        torch.cuda.synchronize()
+        f_ms = e0.elapsed_time(e1) / kf
+        fx_bytes = 4 * N + 4 * B + 4 * N * env.D_priv + 4 * env.D_shared + 4 * env.D_gov + 4 * (N + 1) + 4
+        fx = {"api": "ej_rollout with obs_priv_ring / obs_shared_ring (SURVEY 8(f) f2)", "ms_per_step": f_ms,
+              "value": E * N / (f_ms * 1e-3), "unit": UNIT, "bytes_per_env_step": fx_bytes, "steps": kf}
+        del priv, shared, govr
+
     # ---- e2e: ej_step_host, pinned host buffers, H2D + D2H inside the timed region ----
     e2e = None
     if not args.no_e2e:
@@ -323,6 +345,8 @@ def main():
                             "ms_per_step": step_ms, "value": E * N / (step_ms * 1e-3), "unit": UNIT},
         "clocks": clocks,
     }
+    if fx:
+        line["factored_obs"] = fx
     traffic_path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_path):
         try:

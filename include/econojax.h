@@ -116,6 +116,16 @@ typedef struct ej_rollout_io {
     int32_t* gov_actions_ring;        /* [ring_depth][E][B] */
     float* pop_logits_ring;           /* policy mode only: [ring_depth][E*N][A] logits the actions were sampled from */
     float* gov_logits_ring;           /* policy mode only: [ring_depth][E][B*L] */
+    /* f2, factored observations: the last 5R + B + 2 entries of a population row (market statistics,
+     * tax rates, timers: P:424) are the same for every agent of an env, so the observation of a step
+     * can leave as an agent-private block and one env-wide block.  Column k < 3R + 4 of obs row
+     * (e, i) = priv[e][i][k]; column 3R + 4 + k = shared[e][k].  Set priv and shared together and
+     * leave obs_ring NULL; needs N * (3R + 4) to be a multiple of 4 and a shape whose full tile is
+     * staged in shared memory (N * D_pop * 4 bytes <= ~70 KB), not available in policy mode:
+     * EJ_ERR_PARAM otherwise. */
+    float* obs_priv_ring;             /* [ring_depth][E][N][3R + 4] */
+    float* obs_shared_ring;           /* [ring_depth][E][ceil4(5R + B + 2)] */
+    float* obs_gov_ring;              /* [ring_depth][E][D_gov_pad] government rows (optional) */
 } ej_rollout_io;
 
 /* One tanh MLP  in_dim -> 128 -> 128 -> out_dim  (Table 2; BASELINE.json

@@ -57,6 +57,7 @@ class EjRolloutIO(C.Structure):
         ("obs_ring", C.c_void_p), ("rew_ring", C.c_void_p), ("done_ring", C.c_void_p),
         ("actions_ring", C.c_void_p), ("gov_actions_ring", C.c_void_p),
         ("pop_logits_ring", C.c_void_p), ("gov_logits_ring", C.c_void_p),
+        ("obs_priv_ring", C.c_void_p), ("obs_shared_ring", C.c_void_p), ("obs_gov_ring", C.c_void_p),
     ]
 
 
@@ -348,7 +349,8 @@ class Env:
         return actions, gov_actions
 
     def rollout(self, T, ring_depth=1, actions_in=None, gov_actions_in=None, obs_ring=None, rew_ring=None,
-                done_ring=None, actions_ring=None, gov_actions_ring=None, pop_logits_ring=None, gov_logits_ring=None):
+                done_ring=None, actions_ring=None, gov_actions_ring=None, pop_logits_ring=None, gov_logits_ring=None,
+                obs_priv_ring=None, obs_shared_ring=None, obs_gov_ring=None):
         io = EjRolloutIO()
         io.struct_size = C.sizeof(EjRolloutIO)
         io.ring_depth = ring_depth
@@ -356,7 +358,26 @@ class Env:
         io.obs_ring, io.rew_ring, io.done_ring = _dp(obs_ring), _dp(rew_ring), _dp(done_ring)
         io.actions_ring, io.gov_actions_ring = _dp(actions_ring), _dp(gov_actions_ring)
         io.pop_logits_ring, io.gov_logits_ring = _dp(pop_logits_ring), _dp(gov_logits_ring)
+        io.obs_priv_ring, io.obs_shared_ring, io.obs_gov_ring = _dp(obs_priv_ring), _dp(obs_shared_ring), _dp(obs_gov_ring)
         ej_rollout(self.h, T, io)
+
+    # f2, factored observations (shapes of the three rings of one step)
+    @property
+    def D_priv(self):
+        return 3 * self.R + 4
+
+    @property
+    def D_shared(self):
+        return 5 * self.R + self.B + 2
+
+    @property
+    def D_shared_pad(self):
+        return (self.D_shared + 3) // 4 * 4
+
+    def new_factored_obs(self, depth=1):
+        t = self.torch
+        z = lambda *shape: t.zeros(shape, dtype=t.float32, device=self.device)
+        return z(depth, self.E, self.N, self.D_priv), z(depth, self.E, self.D_shared_pad), z(depth, self.E, self.D_gov_pad)
 
     def set_action_cdf(self, cdf: np.ndarray):
         cdf = np.ascontiguousarray(cdf, np.uint32)

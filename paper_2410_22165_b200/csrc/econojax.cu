@@ -49,6 +49,7 @@ struct ej_env {
     int n_sms = 148;
     // the step kernel variant of this handle's shape (CTA size, array stride, specialised R / P)
     void (*step_fn)(const DevCfg, uint8_t*, const StepIO) = nullptr;
+    void (*step_fn_fx)(const DevCfg, uint8_t*, const StepIO) = nullptr;  // f2: factored observations
     int step_RT = 0, step_PT = 0;
 };
 
@@ -162,6 +163,7 @@ template <int MT, int NS>
 void select_step_kernel(ej_env* h) {
     const DevCfg& c = h->c;
     h->step_fn = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0>;
+    h->step_fn_fx = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0, 1>;
     h->step_RT = h->step_PT = 0;
     // pf = 1 also fixes the paper's mechanics (Table 2; PF in ej_device.cuh)
     auto pick = [&](auto rt, auto pt, auto nt, auto bt, auto pf) {
@@ -178,6 +180,7 @@ void select_step_kernel(ej_env* h) {
         }
         if (c.R == RT && c.P == PT && (NT == 0 || (c.N == NT && c.B == BT)) && (PF == 0 || (paper && lay_ok))) {
             h->step_fn = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF>;
+            if constexpr (PF == 1 && RT == 2) h->step_fn_fx = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF, 1>;  // headline shape
             h->step_RT = RT; h->step_PT = PT;
         }
     };
@@ -208,7 +211,7 @@ void select_step_kernel(ej_env* h) {
 
 int launch_step(ej_env* h, const StepIO& io) {
     const DevCfg& c = h->c;
-    h->step_fn<<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, io);
+    (io.obs_priv ? h->step_fn_fx : h->step_fn)<<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, io);
     h->launches++;
     EJ_CUDA(h, cudaGetLastError(), "ej_step_kernel launch");
     return EJ_OK;
@@ -220,6 +223,7 @@ int set_smem_attr(ej_env* h) {
         constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
         select_step_kernel<MT, NS>(h);
         EJ_CUDA(h, cudaFuncSetAttribute(h->step_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step)");
+        EJ_CUDA(h, cudaFuncSetAttribute(h->step_fn_fx, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step, factored)");
         EJ_CUDA(h, cudaFuncSetAttribute(ej_observe_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (observe)");
         EJ_CUDA(h, cudaFuncSetAttribute(ej_reset_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (reset)");
         return EJ_OK;
@@ -641,6 +645,14 @@ int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* rio) {
         io.actions = rio->actions_in; io.gov_actions = rio->gov_actions_in;
         io.obs = rio->obs_ring; io.rew = rio->rew_ring; io.done = rio->done_ring;
         io.actions_out = rio->actions_ring; io.gov_out = rio->gov_actions_ring;
+        if (rio->obs_priv_ring || rio->obs_shared_ring || rio->obs_gov_ring) {  // f2: factored observations
+            const DevCfg& c = h->c;
+            if (!rio->obs_priv_ring || !rio->obs_shared_ring) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring / io.obs_shared_ring (set both)");
+            if (rio->obs_ring) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_ring (must be NULL with factored observations)");
+            if (!c.stage_obs || (c.N * (3 * c.R + 4)) % 4 != 0) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring (shape cannot stage factored observations)");
+            if (h->has_policy && !rio->actions_in) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring (not available in policy mode)");
+            io.obs_priv = rio->obs_priv_ring; io.obs_shared = rio->obs_shared_ring; io.obs_gov = rio->obs_gov_ring;
+        }
     }
     if (h->has_policy && !io.actions) return rollout_with_policy(h, T, rio, io);
     return launch_step(h, io);

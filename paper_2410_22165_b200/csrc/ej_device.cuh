@@ -81,6 +81,9 @@ struct StepIO {
     const uint32_t* cdf;         // [A] device
     int n_steps, ring_depth;
     int masked;                  // f1: the generator draws among the available actions only
+    float* obs_priv;             // f2 rings (factored observations): [E][N][3R+4], [E][ceil4(5R+B+2)], [E][D_gov_pad]
+    float* obs_shared;
+    float* obs_gov;
 };
 
 // Shared-memory layout of one economy.  Everything whose size depends only on the CTA size NP
@@ -560,9 +563,12 @@ __device__ __forceinline__ void write_timers(const DevCfg& c, const SM& m, int t
 //   mode     0 = step, 1 = finished env (rewards 0), 2 = observe only
 //   rows     0 = rewrite only the columns that change every step, 1 = also the tax rates,
 //            2 = every column (first step of a launch: skills)
-template <int NPAD, int NS, int RT, int NT, int BT, int PF, class SM>
+//   FX       f2, factored observations: the staging tile holds only the 3R + 4 agent-private columns
+//            (-> priv), the env-wide tail leaves once per env from m.shrow() (-> shared), the
+//            government row goes to govp
+template <int NPAD, int NS, int RT, int NT, int BT, int PF, int FX, class SM>
 __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, int rows, float coin_pre, float labor_pre,
-                        double cf_pre, float* obs, float* rew) {
+                        double cf_pre, float* obs, float* rew, float* priv = nullptr, float* shared = nullptr, float* govp = nullptr) {
     constexpr int NW = NPAD / 32, EPL = NPAD / 32;
     // RT, NT, BT > 0: resource count, population size, bracket count known at compile time
     const int N = NT > 0 ? NT : c.N, R = RT > 0 ? RT : c.R, B = BT > 0 ? BT : c.B;
@@ -570,7 +576,9 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
     constexpr int N4 = NS;  // stride of the per-agent arrays
     const bool act = tid < N;
     const int lane = tid & 31, warp = tid >> 5;
-    const bool staged = (PF || c.stage_obs) && obs;
+    const bool staged = FX ? priv != nullptr : ((PF || c.stage_obs) && obs);
+    const bool any_obs = FX ? (priv != nullptr || govp != nullptr) : obs != nullptr;
+    const int DP = FX ? 3 * R + 4 : D_pop;  // row stride of the staging tile
     const int stage_alias_bytes = PF ? 2 * R * NS * 4 : c.stage_alias_bytes, n_metrics = RT > 0 ? 3 + RT : c.n_metrics;
 
     if (act) {
@@ -588,20 +596,22 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
         }
         // ---- this agent's observation row (G25) in the staging tile ----
         if (staged) {
-            float* o = m.stage() + tid * D_pop;
+            float* o = m.stage() + tid * DP;
             o[0] = __fmul_rn(coin, c.s_coin);
             for (int r = 0; r < R; ++r) o[1 + r] = __fmul_rn((float)m.inv()[r * N4 + tid], c.s_count);
             o[R + 1] = __fmul_rn((float)m.esc_coin()[tid], c.s_coin);
             for (int r = 0; r < R; ++r) o[R + 2 + r] = __fmul_rn((float)m.esc_res()[r * N4 + tid], c.s_count);
             o[3 * R + 3] = __fmul_rn(labor, c.s_labor);
-            float* tl = o + 3 * R + 4;
-            for (int k = 0; k < 5 * R; ++k) tl[k] = m.shrow()[k];
-            tl[5 * R + B] = m.shrow()[5 * R + B];
-            tl[5 * R + B + 1] = m.shrow()[5 * R + B + 1];
             // rows whose bytes the matched-order lists reuse are rewritten in full every step
-            const int rows_eff = (tid * D_pop * 4 < stage_alias_bytes) ? 2 : rows;
-            if (rows_eff >= 1)
-                for (int b = 0; b < B; ++b) tl[5 * R + b] = m.shrow()[5 * R + b];
+            const int rows_eff = (tid * DP * 4 < stage_alias_bytes) ? 2 : rows;
+            if (!FX) {
+                float* tl = o + 3 * R + 4;
+                for (int k = 0; k < 5 * R; ++k) tl[k] = m.shrow()[k];
+                tl[5 * R + B] = m.shrow()[5 * R + B];
+                tl[5 * R + B + 1] = m.shrow()[5 * R + B + 1];
+                if (rows_eff >= 1)
+                    for (int b = 0; b < B; ++b) tl[5 * R + b] = m.shrow()[5 * R + b];
+            }
             if (rows_eff >= 2) {
                 for (int r = 0; r < R; ++r) o[2 * R + 2 + r] = m.SG()[r * N4 + tid];
                 o[3 * R + 2] = m.SC()[tid];
@@ -617,22 +627,31 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
     for (int r = NW - 1 - warp; r < R; r += NW) int_metric_stats<EPL, NS, NT>(c, m, r, lane);
     if (tid < B + 2) m.govrow()[3 * n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
 
-    if (obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (any_obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
 
-    if (obs && tid == 0) {  // bulk stores: the env's contiguous [N][D_pop] tile and its government row
+    if (any_obs && tid == 0) {  // bulk stores: the env's contiguous tile, (f2) its env-wide tail, its government row
         if (staged) {
-            float* dst = obs + (uint32_t)(e * N * D_pop);
+            float* dst = FX ? priv + (uint32_t)(e * N * DP) : obs + (uint32_t)(e * N * D_pop);
             const uint32_t src = (uint32_t)__cvta_generic_to_shared(m.stage());
-            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(N * D_pop * 4) : "memory");
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(N * DP * 4) : "memory");
         }
-        float* gdst = obs + (uint32_t)((uint32_t)c.gov_obs_offset + (uint32_t)(e * c.D_gov_pad));
-        const uint32_t gsrc = (uint32_t)__cvta_generic_to_shared(m.govrow());
-        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(gsrc), "r"(c.D_gov_pad * 4) : "memory");
+        if (FX && shared) {
+            const int dsp = (5 * R + B + 2 + 3) & ~3;
+            float* sdst = shared + (uint32_t)(e * dsp);
+            const uint32_t ssrc = (uint32_t)__cvta_generic_to_shared(m.shrow());
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(sdst), "r"(ssrc), "r"(dsp * 4) : "memory");
+        }
+        float* gdst = FX ? (govp ? govp + (uint32_t)(e * c.D_gov_pad) : nullptr)
+                         : obs + (uint32_t)((uint32_t)c.gov_obs_offset + (uint32_t)(e * c.D_gov_pad));
+        if (gdst) {
+            const uint32_t gsrc = (uint32_t)__cvta_generic_to_shared(m.govrow());
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(gsrc), "r"(c.D_gov_pad * 4) : "memory");
+        }
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     }
     // ---- population rows when they cannot go out as one bulk store: coalesced loop ----
-    if (obs && !staged) {
+    if (!FX && obs && !staged) {
         // element (i, k) = scale_k * value of column k's source array at agent i: the column table
         // (build_coltab) replaces a chain of ten compares per element
         extern __shared__ __align__(16) uint8_t ej_smem[];
@@ -737,6 +756,9 @@ struct StepPtrs {
     __device__ __forceinline__ const int32_t* actions() const { return io.actions ? io.actions + (uint32_t)s * (uint32_t)(c.E * c.N) : nullptr; }
     __device__ __forceinline__ const int32_t* gov_actions() const { return io.gov_actions ? io.gov_actions + (uint32_t)s * (uint32_t)(c.E * c.B) : nullptr; }
     __device__ __forceinline__ float* obs() const { return io.obs ? io.obs + (uint32_t)slot * (uint32_t)c.obs_floats : nullptr; }
+    __device__ __forceinline__ float* priv() const { return io.obs_priv ? io.obs_priv + (uint32_t)slot * (uint32_t)(c.E * c.N * (3 * c.R + 4)) : nullptr; }
+    __device__ __forceinline__ float* shared() const { return io.obs_shared ? io.obs_shared + (uint32_t)slot * (uint32_t)(c.E * ((5 * c.R + c.B + 2 + 3) & ~3)) : nullptr; }
+    __device__ __forceinline__ float* govp() const { return io.obs_gov ? io.obs_gov + (uint32_t)slot * (uint32_t)(c.E * c.D_gov_pad) : nullptr; }
     __device__ __forceinline__ float* rew() const { return io.rew ? io.rew + (uint32_t)slot * (uint32_t)(c.E * (c.N + 1)) : nullptr; }
     __device__ __forceinline__ uint8_t* done() const { return io.done ? io.done + (uint32_t)slot * (uint32_t)c.E : nullptr; }
     __device__ __forceinline__ int32_t* actions_out() const { return io.actions_out ? io.actions_out + (uint32_t)slot * (uint32_t)(c.E * c.N) : nullptr; }
@@ -1124,7 +1146,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
 
 // One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
 // observations.  outputs() has this single call site (instruction footprint).
-template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, class SM>
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX, class SM>
 __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const StepPtrs& io, bool first) {
     const int t = m.hdr()->t;
     // the previous step's bulk stores must have read the staging tile before it is rewritten
@@ -1142,14 +1164,15 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
         step_body<NPAD, NS, RT, PT, NT, BT, PF>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
     }
     // ---------------- P5 rewards, P6 observations ----------------
-    outputs<NPAD, NS, RT, NT, BT, PF>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs(), io.rew());
+    outputs<NPAD, NS, RT, NT, BT, PF, FX>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs(), io.rew(), FX ? io.priv() : nullptr,
+                                          FX ? io.shared() : nullptr, FX ? io.govp() : nullptr);
     if (mode == 1) {
         if (tid == 0 && io.io.done) io.done()[e] = 1;
         __syncthreads();  // shrow is rewritten at the very start of the next finished step
     }
 }
 
-template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF>
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX = 0>
 __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const __grid_constant__ StepIO io) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
@@ -1171,7 +1194,7 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
 #pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
         p.s = s;
-        env_step<NPAD, NS, RT, PT, NT, BT, PF>(c, m, tid, e, p, s == 0);
+        env_step<NPAD, NS, RT, PT, NT, BT, PF, FX>(c, m, tid, e, p, s == 0);
         p.slot = (p.slot + 1 == io.ring_depth) ? 0 : p.slot + 1;
     }
     __syncthreads();
@@ -1195,7 +1218,7 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
     if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
     __syncthreads();
-    outputs<NPAD, NS, 0, 0, 0, 0>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
+    outputs<NPAD, NS, 0, 0, 0, 0, 0>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 

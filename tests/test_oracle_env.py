@@ -429,3 +429,20 @@ def test_book_cap_by_arrival_order():
     # next step: book already holds 2 -> everything rejected
     env.step([[a.buy(0, 0)] * 4], gov0(env))
     assert st(env)["counters"][1] == 2
+
+
+def test_env_wide_tail_of_the_population_rows_is_identical_for_all_agents():
+    """f2 rests on this (market statistics are global; rates and timers are per env): columns
+    3R + 4 .. of the population observation do not depend on the agent."""
+    cfg = inputs.configs()["tiny_dense"]
+    E, N, R = 4, cfg["N"], cfg["R"]
+    o = oracle.OracleEnv(E, N, R, cfg["params"])
+    o.reset(2)
+    acts, gov = inputs.action_stream(cfg, 40, seed=2, E=E)
+    varied = 0
+    for t in range(40):
+        pop, _, _, _ = o.step(acts[t], gov[t])
+        tail = pop[:, :, 3 * R + 4:]
+        assert (tail == tail[:, :1, :]).all()
+        varied += int((pop[:, :, :3 * R + 4] != pop[:, :1, :3 * R + 4]).any())
+    assert varied > 0  # while the private block does differ between agents
