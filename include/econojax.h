@@ -121,7 +121,7 @@ typedef struct ej_rollout_io {
      * can leave as an agent-private block and one env-wide block.  Column k < 3R + 4 of obs row
      * (e, i) = priv[e][i][k]; column 3R + 4 + k = shared[e][k].  Set priv and shared together and
      * leave obs_ring NULL; needs N * (3R + 4) to be a multiple of 4 and a shape whose full tile is
-     * staged in shared memory (N * D_pop * 4 bytes <= ~70 KB), not available in policy mode:
+     * staged in shared memory (N <= 256 and N * D_pop * 4 bytes <= ~70 KB), not available in policy mode:
      * EJ_ERR_PARAM otherwise. */
     float* obs_priv_ring;             /* [ring_depth][E][N][3R + 4] */
     float* obs_shared_ring;           /* [ring_depth][E][ceil4(5R + B + 2)] */

@@ -163,7 +163,8 @@ template <int MT, int NS>
 void select_step_kernel(ej_env* h) {
     const DevCfg& c = h->c;
     h->step_fn = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0>;
-    h->step_fn_fx = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0, 1>;
+    h->step_fn_fx = nullptr;  // f2 variants exist for CTAs of up to 256 threads (build time)
+    if constexpr (MT <= 256) h->step_fn_fx = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0, 1>;
     h->step_RT = h->step_PT = 0;
     // pf = 1 also fixes the paper's mechanics (Table 2; PF in ej_device.cuh)
     auto pick = [&](auto rt, auto pt, auto nt, auto bt, auto pf) {
@@ -223,7 +224,7 @@ int set_smem_attr(ej_env* h) {
         constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
         select_step_kernel<MT, NS>(h);
         EJ_CUDA(h, cudaFuncSetAttribute(h->step_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step)");
-        EJ_CUDA(h, cudaFuncSetAttribute(h->step_fn_fx, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step, factored)");
+        if (h->step_fn_fx) EJ_CUDA(h, cudaFuncSetAttribute(h->step_fn_fx, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step, factored)");
         EJ_CUDA(h, cudaFuncSetAttribute(ej_observe_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (observe)");
         EJ_CUDA(h, cudaFuncSetAttribute(ej_reset_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (reset)");
         return EJ_OK;
@@ -649,7 +650,7 @@ int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* rio) {
             const DevCfg& c = h->c;
             if (!rio->obs_priv_ring || !rio->obs_shared_ring) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring / io.obs_shared_ring (set both)");
             if (rio->obs_ring) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_ring (must be NULL with factored observations)");
-            if (!c.stage_obs || (c.N * (3 * c.R + 4)) % 4 != 0) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring (shape cannot stage factored observations)");
+            if (!h->step_fn_fx || !c.stage_obs || (c.N * (3 * c.R + 4)) % 4 != 0) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring (shape cannot stage factored observations)");
             if (h->has_policy && !rio->actions_in) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring (not available in policy mode)");
             io.obs_priv = rio->obs_priv_ring; io.obs_shared = rio->obs_shared_ring; io.obs_gov = rio->obs_gov_ring;
         }
