@@ -82,6 +82,10 @@ typedef struct ej_params {
     uint32_t env_id_base;                   /* global id of local env 0: every random draw is keyed by
                                                the global env id, so results do not depend on E or on
                                                how envs are sharded over GPUs (multi-GPU: DESIGN.md 7) */
+    float skill_growth_rate;                /* f3: 0 = skills fixed.  > 0: after a valid gather r (craft) the
+                                               skill SG[r] (SC) becomes min(skill_max, s + s * (rate * (1 - s / skill_max))),
+                                               one binary32 rounding per operation (G41); the action itself uses the old skill */
+    float skill_max;                        /* > 0 when skill_growth_rate > 0 (5) */
 } ej_params;
 
 typedef struct ej_env ej_env;

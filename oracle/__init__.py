@@ -41,6 +41,7 @@ class OrcParams(C.Structure):
         ("obs_scale_coin", C.c_float), ("obs_scale_count", C.c_float),
         ("obs_scale_price", C.c_float), ("obs_scale_labor", C.c_float),
         ("env_id_base", C.c_uint32),
+        ("skill_growth_rate", C.c_float), ("skill_max", C.c_float),
     ]
 
 
@@ -127,7 +128,7 @@ def make_params(d: dict) -> OrcParams:
         setattr(p, name, int(d[name]))
     for name in ("starting_coin", "labor_craft", "labor_gather", "labor_trade", "eta", "omega", "craft_scale",
                  "skill_clip_lo", "skill_clip_hi", "obs_scale_coin", "obs_scale_count", "obs_scale_price",
-                 "obs_scale_labor"):
+                 "obs_scale_labor", "skill_growth_rate", "skill_max"):
         setattr(p, name, float(d[name]))
     return p
 

@@ -482,12 +482,16 @@ static void step_env(const orc_sim* s, orc_env* v, uint32_t gid, const int32_t* 
             int32_t amt = orc_gather_amount(v->SG[i * R + a], orc_u01(x[1]));
             v->inv[i * R + a] += amt;
             v->labor[i] = v->labor[i] + p->labor_gather;
+            if (p->skill_growth_rate > 0.0f) /* f3: the amount above used the skill before the increase */
+                v->SG[i * R + a] = orc_progress_skill(v->SG[i * R + a], p->skill_growth_rate, p->skill_max);
         } else if (a < base_buy) { /* craft */
             if (orc_craft_consume(&v->inv[i * R], R, p->craft_units, p->craft_distinct, p->craft_mode, a - R)) {
                 float pay = v->SC[i] * p->craft_scale;
                 v->coin[i] = v->coin[i] + pay;
                 v->income[i] = v->income[i] + pay;
                 v->labor[i] = v->labor[i] + p->labor_craft;
+                if (p->skill_growth_rate > 0.0f) /* f3: the payout above used the skill before the increase */
+                    v->SC[i] = orc_progress_skill(v->SC[i], p->skill_growth_rate, p->skill_max);
             } else {
                 v->n_invalid++;
             }
@@ -643,6 +647,17 @@ void orc_step(orc_sim* s, int32_t env_begin, int32_t env_count, const int32_t* a
                  obs_pop ? obs_pop + (size_t)k * N * Dp : NULL, obs_gov ? obs_gov + (size_t)k * Dg : NULL,
                  rew ? rew + (size_t)k * (N + 1) : NULL, done ? done + k : NULL);
     }
+}
+
+/* f3 (G41): one correctly rounded binary32 operation per step of the formula. */
+float orc_progress_skill(float skill, float rate, float max) {
+    const float frac = skill / max;
+    const float room = 1.0f - frac;
+    const float g = rate * room;
+    const float inc = skill * g;
+    float out = skill + inc;
+    if (out > max) out = max;
+    return out;
 }
 
 /* Rollout-mode action generator (G30): Philox stream 0 word 0 through the caller's CDF

@@ -70,7 +70,15 @@ typedef struct orc_params {
     float skill_clip_lo, skill_clip_hi;     /* PARETO_CLIP bounds */
     float obs_scale_coin, obs_scale_count, obs_scale_price, obs_scale_labor; /* G25 */
     uint32_t env_id_base;                   /* global id of local env 0 (Philox counter word 0) */
+    float skill_growth_rate;                /* f3: 0 = skills fixed (default); section 5 uses 0.005 */
+    float skill_max;                        /* f3: "maximum skill level of 5" */
 } orc_params;
+
+/* f3, skill growth ("Whenever an agent gathers or crafts, the respective skill is increased
+ * by 0.5%.  This 0.5% bonus shrinks as the agent approaches the maximum skill level of 5"; the
+ * paper gives no formula: linear damping after S:101, G41):
+ *   skill' = min(max, skill + skill * (rate * (1 - skill / max))), each operation rounded to binary32. */
+float orc_progress_skill(float skill, float rate, float max);
 
 typedef struct orc_sim orc_sim;
 

@@ -49,6 +49,8 @@ def default_params() -> dict:
         skill_clip_lo=1.0, skill_clip_hi=10.0,
         obs_scale_coin=0.01, obs_scale_count=0.1, obs_scale_price=0.1, obs_scale_labor=0.01,  # G25
         env_id_base=0,
+        skill_growth_rate=0.0,            # f3: 0 = fixed skills; section 5 uses 0.005
+        skill_max=5.0,
     )
 
 

@@ -317,3 +317,48 @@ def test_matching_brute_force_on_tiny_books():
             assert max(b[0] for b in rb) < min(a[0] for a in ra)  # uncrossed afterwards
         assert len(rb) == len(bids) - q and len(ra) == len(asks) - q
         assert sorted(rb + [b for b in bids if b not in rb]) == sorted(bids)
+
+
+# ---- f3: skill growth (G41) ----
+
+def _progress(skill, rate=0.005, mx=5.0):
+    import ctypes as C
+    L = oracle.lib()
+    L.orc_progress_skill.restype = C.c_float
+    L.orc_progress_skill.argtypes = [C.c_float, C.c_float, C.c_float]
+    return float(L.orc_progress_skill(skill, rate, mx))
+
+
+def test_skill_growth_closed_form_and_limits():
+    # 0.5 % at skill << max, shrinking linearly to 0 at the maximum skill level of 5
+    assert abs(_progress(1.0) - 1.004) < 1e-6            # 1 + 1 * 0.005 * (1 - 1/5), also S:104
+    assert _progress(5.0) == 5.0 and _progress(0.0) == 0.0
+    assert abs(_progress(2.5) - (2.5 + 2.5 * 0.005 * 0.5)) < 1e-6
+    assert abs(_progress(1e-3) / 1e-3 - 1.005) < 1e-5    # the full 0.5 % far from the cap
+    xs = np.linspace(0.0, 5.0, 2001, dtype=np.float32)
+    ys = np.array([_progress(float(x)) for x in xs])
+    assert np.all(ys >= xs) and np.all(ys <= 5.0)        # never decreases, never passes the cap
+    gain = ys[1:-1] / xs[1:-1] - 1.0
+    assert np.all(np.diff(gain) <= 1e-6)                  # "this bonus shrinks as the agent approaches the maximum"
+    assert _progress(1.0, rate=0.0) == 1.0
+
+
+def test_skill_growth_in_the_step(small_params):
+    from conftest import Act
+    act = Act(2, 10)
+    gov = np.zeros((1, 3), np.int32)
+    for rate in (0.0, 0.005):
+        p = dict(small_params, skill_growth_rate=rate, skill_max=5.0)
+        o = oracle.OracleEnv(1, 3, 2, p)
+        o.reset(0)
+        o.set_agent(0, 0, 0.0, [0, 0], [1.0, 2.0], 3.0)
+        o.set_agent(0, 1, 0.0, [2, 2], [1.0, 2.0], 3.0)
+        o.set_agent(0, 2, 0.0, [0, 0], [1.0, 2.0], 3.0)
+        o.step(np.array([[act.gather(1), act.craft(), act.craft()]], np.int32), gov)   # agent 2's craft is invalid
+        s = oracle.parse_state(o.get_state()[0])
+        g = lambda x: _progress(x) if rate else x
+        assert s["SG"][0].tolist() == [1.0, np.float32(g(2.0))]      # only the gathered resource's skill grows
+        assert s["SC"][0] == 3.0 and s["SG"][1].tolist() == [1.0, 2.0]
+        assert s["SC"][1] == np.float32(g(3.0))                       # craft: the crafting skill
+        assert s["coin"][1] == 30.0                                   # payout used the skill BEFORE the increase
+        assert s["SC"][2] == 3.0                                      # an invalid craft teaches nothing
