@@ -22,7 +22,7 @@ _LIB = os.path.join(_HERE, "liborc.so")
 
 MAX_PRICES, MAX_BRACKETS, MAX_RATE_LEVELS = 16, 16, 32
 CRAFT_SINGLE, CRAFT_PER_RESOURCE = 0, 1
-SKILL_UNIFORM01, SKILL_PARETO_CLIP = 0, 1
+SKILL_UNIFORM01, SKILL_PARETO_CLIP, SKILL_NORMAL_CLIP = 0, 1, 2
 
 
 class OrcParams(C.Structure):
@@ -42,6 +42,7 @@ class OrcParams(C.Structure):
         ("obs_scale_price", C.c_float), ("obs_scale_labor", C.c_float),
         ("env_id_base", C.c_uint32),
         ("skill_growth_rate", C.c_float), ("skill_max", C.c_float),
+        ("skill_mean", C.c_float), ("skill_std", C.c_float),
     ]
 
 
@@ -128,7 +129,7 @@ def make_params(d: dict) -> OrcParams:
         setattr(p, name, int(d[name]))
     for name in ("starting_coin", "labor_craft", "labor_gather", "labor_trade", "eta", "omega", "craft_scale",
                  "skill_clip_lo", "skill_clip_hi", "obs_scale_coin", "obs_scale_count", "obs_scale_price",
-                 "obs_scale_labor", "skill_growth_rate", "skill_max"):
+                 "obs_scale_labor", "skill_growth_rate", "skill_max", "skill_mean", "skill_std"):
         setattr(p, name, float(d[name]))
     return p
 

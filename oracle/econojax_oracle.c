@@ -315,9 +315,15 @@ static void draw(const orc_sim* s, uint32_t env_gid, uint32_t agent, uint32_t t,
     orc_philox4x32_10(ctr, key, x);
 }
 
-/* Skill draw number d of an agent: Philox stream 16, "t" field = d/4, word d%4 (G30). */
+/* Skill draw number d of an agent: Philox stream 16, "t" field = d/4, word d%4 (G30).
+ * NORMAL_CLIP (f3, G42): stream 17, "t" fields 3d, 3d+1, 3d+2 give the twelve words of draw d. */
 static float skill_draw(const orc_sim* s, uint32_t env_gid, uint32_t agent, int32_t d) {
     uint32_t x[4];
+    if (s->p.skill_init == ORC_SKILL_NORMAL_CLIP) {
+        uint32_t w[12];
+        for (int32_t j = 0; j < 3; ++j) draw(s, env_gid, agent, (uint32_t)(3 * d + j), 17u, &w[4 * j]);
+        return orc_normal_skill(w, s->p.skill_mean, s->p.skill_std, s->p.skill_clip_lo, s->p.skill_clip_hi);
+    }
     draw(s, env_gid, agent, (uint32_t)(d / 4), 16u, x);
     float u = orc_u01(x[d % 4]);
     if (s->p.skill_init == ORC_SKILL_UNIFORM01) return u;
@@ -658,6 +664,18 @@ float orc_progress_skill(float skill, float rate, float max) {
     float out = skill + inc;
     if (out > max) out = max;
     return out;
+}
+
+/* f3 (G42): sum of twelve 24-bit uniforms minus 6 as the standard normal. */
+float orc_normal_skill(const uint32_t words[12], float mean, float std, float lo, float hi) {
+    int64_t sum = 0;
+    for (int32_t k = 0; k < 12; ++k) sum += (int64_t)(words[k] >> 8);
+    const double z = (double)sum * (1.0 / 16777216.0) - 6.0; /* exact: |sum - 6 * 2^24| < 2^27 */
+    const double scaled = (double)std * z;                   /* exact: 24 x 27 significant bits */
+    float x = (float)((double)mean + scaled);
+    if (x < lo) x = lo;
+    if (x > hi) x = hi;
+    return x;
 }
 
 /* Rollout-mode action generator (G30): Philox stream 0 word 0 through the caller's CDF

@@ -42,6 +42,8 @@ extern "C" {
 #define ORC_CRAFT_PER_RESOURCE 1 /* BASELINE.json's "convert r" variant (G3) */
 #define ORC_SKILL_UNIFORM01 0
 #define ORC_SKILL_PARETO_CLIP 1  /* Pareto(alpha=4) clipped, BASELINE.json configs 2-5 (G29) */
+#define ORC_SKILL_NORMAL_CLIP 2  /* f3, section 5: "a normal distribution around 1.0 with a standard deviation of 1.0"
+                                    (P:345), clipped to [lo, hi] (G42) */
 
 /* Environment parameters; defaults are Table 2 unless BASELINE.json overrides. */
 typedef struct orc_params {
@@ -72,7 +74,15 @@ typedef struct orc_params {
     uint32_t env_id_base;                   /* global id of local env 0 (Philox counter word 0) */
     float skill_growth_rate;                /* f3: 0 = skills fixed (default); section 5 uses 0.005 */
     float skill_max;                        /* f3: "maximum skill level of 5" */
+    float skill_mean, skill_std;            /* f3: NORMAL_CLIP parameters (1.0 and 1.0) */
 } orc_params;
+
+/* f3, normal skill draw (G42).  The paper names the distribution, not a generator.  To stay a pure
+ * function of the Philox words with no transcendental function in it, the standard normal is the classical
+ * sum of twelve uniforms: z = sum_{k<12} u_k - 6 with u_k = (word_k >> 8) * 2^-24 (mean 0, variance 1 up to the
+ * 2^-24 lattice, support [-6, 6)); the sum is an exact integer, z and std * z are exact in binary64, then
+ *   skill = clip((float)(mean + std * z), lo, hi). */
+float orc_normal_skill(const uint32_t words[12], float mean, float std, float lo, float hi);
 
 /* f3, skill growth ("Whenever an agent gathers or crafts, the respective skill is increased
  * by 0.5%.  This 0.5% bonus shrinks as the agent approaches the maximum skill level of 5"; the

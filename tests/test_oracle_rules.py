@@ -362,3 +362,63 @@ def test_skill_growth_in_the_step(small_params):
         assert s["SC"][1] == np.float32(g(3.0))                       # craft: the crafting skill
         assert s["coin"][1] == 30.0                                   # payout used the skill BEFORE the increase
         assert s["SC"][2] == 3.0                                      # an invalid craft teaches nothing
+
+
+# ---- f3: normal skill initialisation (G42) ----
+
+def _normal_skill(words, mean=1.0, std=1.0, lo=-1e30, hi=1e30):
+    import ctypes as C
+    L = oracle.lib()
+    L.orc_normal_skill.restype = C.c_float
+    L.orc_normal_skill.argtypes = [C.POINTER(C.c_uint32)] + [C.c_float] * 4
+    w = (C.c_uint32 * 12)(*[int(x) for x in words])
+    return float(L.orc_normal_skill(w, mean, std, lo, hi))
+
+
+def test_normal_skill_hand_values_and_exact_recomputation():
+    from fractions import Fraction
+    half = [1 << 31] * 12                       # every uniform 0.5: z = 0, the skill is the mean
+    assert _normal_skill(half) == 1.0 and _normal_skill(half, mean=2.5, std=3.0) == 2.5
+    assert _normal_skill([0] * 12) == -5.0      # z = -6, the lower end of the support
+    assert _normal_skill([0] * 12, lo=0.0, hi=5.0) == 0.0                    # clipped below
+    assert _normal_skill([0xFFFFFFFF] * 12, lo=0.0, hi=5.0) == 5.0           # z -> 6: clipped above
+    assert _normal_skill([0xFF] * 12) == -5.0   # the low 8 bits of a word are not used (24-bit uniforms, as orc_u01)
+    one = [1 << 31] * 11 + [(1 << 31) + (1 << 8)]                            # one lattice step above the mean
+    assert _normal_skill(one, mean=0.0) == 2.0 ** -24
+    rng = np.random.default_rng(5)
+    for _ in range(300):                        # rational arithmetic, one rounding to binary32 at the end
+        w = rng.integers(0, 1 << 32, 12, dtype=np.uint64)
+        mean, std = np.float32(rng.normal(1, 1)), np.float32(abs(rng.normal(1, 1)))
+        z = Fraction(sum(int(x) >> 8 for x in w), 1 << 24) - 6
+        exact = Fraction(float(mean)) + Fraction(float(std)) * z
+        got = _normal_skill(w, float(mean), float(std))
+        assert abs(Fraction(got) - exact) <= abs(exact) * Fraction(1, 1 << 23) + Fraction(1, 1 << 140)
+        assert got == float(np.float32(float(exact)))   # float(Fraction) is correctly rounded; the sum fits binary64 here
+
+
+def test_normal_skill_distribution():
+    from scipy import stats
+    rng = np.random.default_rng(11)
+    w = rng.integers(0, 1 << 32, (40000, 12), dtype=np.uint64)
+    z = np.array([_normal_skill(r, mean=0.0, std=1.0) for r in w], np.float64)
+    assert abs(z.mean()) < 0.02 and abs(z.std() - 1.0) < 0.02
+    assert stats.kstest(z, "norm").statistic < 0.012    # a sample of 40 000 from N(0,1) itself gives ~0.004-0.008
+    assert abs(stats.skew(z)) < 0.05 and abs(stats.kurtosis(z) + 0.1) < 0.08   # the twelve-uniform sum has excess kurtosis -0.1
+
+
+def test_normal_skill_at_reset(small_params):
+    p = dict(small_params, skill_init=oracle.SKILL_NORMAL_CLIP, skill_mean=1.0, skill_std=1.0, skill_clip_lo=0.0, skill_clip_hi=5.0)
+    o = oracle.OracleEnv(40, 50, 2, p)
+    o.reset(3)
+    st = [oracle.parse_state(w) for w in o.get_state()]
+    sk = np.concatenate([np.concatenate([s["SG"].ravel(), s["SC"].ravel()]) for s in st]).astype(np.float64)
+    assert sk.size == 40 * 50 * 3 and sk.min() >= 0.0 and sk.max() <= 5.0
+    # N(1,1) clipped at 0: P(skill = 0) = Phi(-1) = 0.1587; mean of max(0, X) = Phi(1) + phi(1) = 1.0833
+    assert abs((sk == 0.0).mean() - 0.1587) < 0.015 and abs(sk.mean() - 1.0833) < 0.03
+    o2 = oracle.OracleEnv(40, 50, 2, p)
+    o2.reset(3)
+    assert all((a == b).all() for a, b in zip(o.get_state(), o2.get_state()))          # deterministic
+    o2.reset(4)
+    assert any((a != b).any() for a, b in zip(o.get_state(), o2.get_state()))          # keyed by the seed
+    # draws of different agents / skills / envs are different words (no stream reuse): nearly all values distinct
+    assert np.unique(sk[sk > 0]).size > 0.99 * (sk > 0).sum()
