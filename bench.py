@@ -47,7 +47,7 @@ def workload_desc(name, cfg, E):
     p = cfg["params"]
     return "%s: E=%d N=%d R=%d prices=%d brackets=%d T=%d tax_period=%d actions=%s skills=%s" % (
         name, E, cfg["N"], cfg["R"], len(p["prices"]), len(p["thresholds"]) + 1, cfg["T"], p["tax_period"],
-        cfg["action_mix"], "pareto4_clip" if p["skill_init"] else "uniform01")
+        cfg["action_mix"], ("uniform01", "pareto4_clip", "normal_clip+growth" if p["skill_growth_rate"] else "normal_clip")[p["skill_init"]])
 
 
 def algorithmic_bytes_per_env_step(N, B, D_pop, D_gov):

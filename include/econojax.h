@@ -51,6 +51,9 @@ extern "C" {
 #define EJ_CRAFT_PER_RESOURCE 1  /* "convert r" variant of BASELINE.json (G3) */
 #define EJ_SKILL_UNIFORM01 0
 #define EJ_SKILL_PARETO_CLIP 1   /* Pareto(alpha=4) clipped to [lo, hi] (G29) */
+#define EJ_SKILL_NORMAL_CLIP 2   /* f3, section 5 ("a normal distribution around 1.0 with a standard deviation of
+                                    1.0"): skill_mean + skill_std * z clipped to [lo, hi], z = sum of twelve 24-bit
+                                    Philox uniforms - 6 (G42) */
 
 /* Environment parameters (Table 2, unless noted).  POD, versioned by struct_size. */
 typedef struct ej_params {
@@ -86,6 +89,7 @@ typedef struct ej_params {
                                                skill SG[r] (SC) becomes min(skill_max, s + s * (rate * (1 - s / skill_max))),
                                                one binary32 rounding per operation (G41); the action itself uses the old skill */
     float skill_max;                        /* > 0 when skill_growth_rate > 0 (5) */
+    float skill_mean, skill_std;            /* EJ_SKILL_NORMAL_CLIP only (1.0, 1.0); skill_std >= 0 */
 } ej_params;
 
 typedef struct ej_env ej_env;

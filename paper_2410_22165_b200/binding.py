@@ -37,6 +37,7 @@ class EjParams(C.Structure):
         ("obs_scale_price", C.c_float), ("obs_scale_labor", C.c_float),
         ("env_id_base", C.c_uint32),
         ("skill_growth_rate", C.c_float), ("skill_max", C.c_float),
+        ("skill_mean", C.c_float), ("skill_std", C.c_float),
     ]
 
 
@@ -138,7 +139,7 @@ def make_params(d: dict) -> EjParams:
         setattr(p, name, int(d[name]))
     for name in ("starting_coin", "labor_craft", "labor_gather", "labor_trade", "eta", "omega", "craft_scale",
                  "skill_clip_lo", "skill_clip_hi", "obs_scale_coin", "obs_scale_count", "obs_scale_price",
-                 "obs_scale_labor", "skill_growth_rate", "skill_max"):
+                 "obs_scale_labor", "skill_growth_rate", "skill_max", "skill_mean", "skill_std"):
         setattr(p, name, float(d[name]))
     return p
 

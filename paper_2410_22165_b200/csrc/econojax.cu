@@ -440,7 +440,12 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     if (p->order_expiry < 1) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "order_expiry");
     if (p->max_active_orders < 1 || p->max_active_orders > EJ_MAX_ACTIVE_ORDERS) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "max_active_orders");
     if (p->book_cap < 0) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "book_cap");
-    if (p->skill_init != EJ_SKILL_UNIFORM01 && p->skill_init != EJ_SKILL_PARETO_CLIP) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "skill_init");
+    if (p->skill_init != EJ_SKILL_UNIFORM01 && p->skill_init != EJ_SKILL_PARETO_CLIP && p->skill_init != EJ_SKILL_NORMAL_CLIP)
+        return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "skill_init");
+    if (p->skill_init == EJ_SKILL_NORMAL_CLIP && !(p->skill_std >= 0.0f && p->skill_clip_lo <= p->skill_clip_hi))
+        return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "skill_std / skill_clip_lo / skill_clip_hi");
+    if (!(p->skill_growth_rate >= 0.0f)) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "skill_growth_rate");
+    if (p->skill_growth_rate > 0.0f && !(p->skill_max > 0.0f)) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "skill_max");
     int mp_log2 = 0;
     while ((1 << mp_log2) < p->max_active_orders) ++mp_log2;
     if (((int64_t)N << mp_log2) >= 65535) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "max_active_orders (N * M too large)");
@@ -484,6 +489,8 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     c.starting_coin = p->starting_coin; c.labor_craft = p->labor_craft; c.labor_gather = p->labor_gather;
     c.labor_trade = p->labor_trade; c.eta = p->eta; c.omega = p->omega; c.craft_scale = p->craft_scale;
     c.clip_lo = p->skill_clip_lo; c.clip_hi = p->skill_clip_hi;
+    c.skill_rate = p->skill_growth_rate; c.skill_max = p->skill_max;
+    c.skill_mean = p->skill_mean; c.skill_std = p->skill_std;
     c.s_coin = p->obs_scale_coin; c.s_count = p->obs_scale_count; c.s_price = p->obs_scale_price; c.s_labor = p->obs_scale_labor;
     c.env_id_base = p->env_id_base;
     c.gov_obs_offset = ((unsigned long long)E * N * c.D_pop + 3ull) & ~3ull;

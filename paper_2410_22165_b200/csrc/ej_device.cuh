@@ -56,6 +56,8 @@ struct DevCfg {
     float rate_table[EJ_MAX_RATE_LEVELS];
     float starting_coin, labor_craft, labor_gather, labor_trade, eta, omega, craft_scale;
     float clip_lo, clip_hi, s_coin, s_count, s_price, s_labor;
+    float skill_rate, skill_max;  // f3: skill_rate == 0 keeps the skills fixed
+    float skill_mean, skill_std;  // f3: EJ_SKILL_NORMAL_CLIP
     double inv_n;  // 1 / N
     double ua, inv_ua;  // 1 - eta and its reciprocal (Eq.1)
     uint32_t env_id_base, seed_lo, seed_hi;
@@ -189,6 +191,14 @@ struct Sm {
     __device__ __forceinline__ float* stage() const { return at<float>(ST ? S::stage : c.o_stage); }
     __device__ __forceinline__ uint32_t* coltab() const { return at<uint32_t>(c.o_coltab); }
 };
+
+// f3, skill growth ("the respective skill is increased by 0.5%.  This 0.5% bonus shrinks as the agent
+// approaches the maximum skill level of 5"; linear damping, G41): min(max, s + s * (rate * (1 - s / max))),
+// every operation one correctly rounded binary32 operation.
+__device__ __forceinline__ float progress_skill(float s, float rate, float mx) {
+    const float room = __fsub_rn(1.0f, __fdiv_rn(s, mx));
+    return fminf(__fadd_rn(s, __fmul_rn(s, __fmul_rn(rate, room))), mx);
+}
 
 // Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11), G30.
 __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3, uint32_t k0,
@@ -562,7 +572,7 @@ __device__ __forceinline__ void write_timers(const DevCfg& c, const SM& m, int t
 // Called after a block barrier that made the state (and m.shrow()) final.
 //   mode     0 = step, 1 = finished env (rewards 0), 2 = observe only
 //   rows     0 = rewrite only the columns that change every step, 1 = also the tax rates,
-//            2 = every column (first step of a launch: skills)
+//            2 = every column (first step of a launch, every step under skill growth: skills)
 //   FX       f2, factored observations: the staging tile holds only the 3R + 4 agent-private columns
 //            (-> priv), the env-wide tail leaves once per env from m.shrow() (-> shared), the
 //            government row goes to govp
@@ -837,6 +847,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
             const float s = __fadd_rn(m.SG()[a * N4 + tid], rho);
             m.inv()[a * N4 + tid] += (int)floorf(s);
             m.labor()[tid] = __fadd_rn(labor_pre, c.labor_gather);
+            if (c.skill_rate > 0.0f)  // f3: the amount above used the skill before the increase
+                m.SG()[a * N4 + tid] = progress_skill(m.SG()[a * N4 + tid], c.skill_rate, c.skill_max);
         } else if (a < base_buy) {  // craft
             bool ok;
             if (craft_mode == EJ_CRAFT_PER_RESOURCE) {
@@ -866,6 +878,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
                 m.coin()[tid] = __fadd_rn(coin_pre, pay);
                 m.income()[tid] = __fadd_rn(m.income()[tid], pay);
                 m.labor()[tid] = __fadd_rn(labor_pre, c.labor_craft);
+                if (c.skill_rate > 0.0f)  // f3: the payout above used the skill before the increase
+                    m.SC()[tid] = progress_skill(m.SC()[tid], c.skill_rate, c.skill_max);
             } else {
                 invalid = true;
             }
@@ -1141,7 +1155,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
         if (io.io.done) io.done()[e] = (uint8_t)(t + 1 == c.T);
     }
 
-    rows = first ? 2 : (boundary ? 1 : 0);
+    // f3: growing skills change the skill columns of the staged rows at any step
+    rows = (first || c.skill_rate > 0.0f) ? 2 : (boundary ? 1 : 0);
 }
 
 // One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
@@ -1240,7 +1255,20 @@ __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ 
             if ((d & 3) == 0) philox4x32_10(gid, (uint32_t)tid, (uint32_t)(d >> 2), 16u, c.seed_lo, c.seed_hi, x[0], x[1], x[2], x[3]);
             const uint32_t w = (d & 3) == 0 ? x[0] : (d & 3) == 1 ? x[1] : (d & 3) == 2 ? x[2] : x[3];
             float v = u01(w);
-            if (c.skill_init == EJ_SKILL_PARETO_CLIP) {  // Pareto(4) by inversion: 1/sqrt(sqrt(1-u))
+            if (c.skill_init == EJ_SKILL_NORMAL_CLIP) {
+                // f3 (G42): z = sum of twelve 24-bit uniforms - 6 (stream 17, "t" fields 3d .. 3d+2); the
+                // sum is an integer, z and std * z are exact in binary64, one rounding to binary32, then the clip
+                long long sum = 0;
+                for (int j = 0; j < 3; ++j) {
+                    uint32_t y0, y1, y2, y3;
+                    philox4x32_10(gid, (uint32_t)tid, (uint32_t)(3 * d + j), 17u, c.seed_lo, c.seed_hi, y0, y1, y2, y3);
+                    sum += (long long)(y0 >> 8) + (long long)(y1 >> 8) + (long long)(y2 >> 8) + (long long)(y3 >> 8);
+                }
+                const double z = __dsub_rn(__dmul_rn((double)sum, 1.0 / 16777216.0), 6.0);
+                v = __double2float_rn(__dadd_rn((double)c.skill_mean, __dmul_rn((double)c.skill_std, z)));
+                if (v < c.clip_lo) v = c.clip_lo;
+                if (v > c.clip_hi) v = c.clip_hi;
+            } else if (c.skill_init == EJ_SKILL_PARETO_CLIP) {  // Pareto(4) by inversion: 1/sqrt(sqrt(1-u))
                 float rr = __fsqrt_rn(__fsub_rn(1.0f, v));
                 rr = __fsqrt_rn(rr);
                 v = __fdiv_rn(1.0f, rr);

@@ -16,7 +16,7 @@ import math
 import numpy as np
 
 CRAFT_SINGLE, CRAFT_PER_RESOURCE = 0, 1
-SKILL_UNIFORM01, SKILL_PARETO_CLIP = 0, 1
+SKILL_UNIFORM01, SKILL_PARETO_CLIP, SKILL_NORMAL_CLIP = 0, 1, 2
 
 
 def rate_table(levels: int) -> list:
@@ -50,6 +50,7 @@ def default_params() -> dict:
         obs_scale_coin=0.01, obs_scale_count=0.1, obs_scale_price=0.1, obs_scale_labor=0.01,  # G25
         env_id_base=0,
         skill_growth_rate=0.0,            # f3: 0 = fixed skills; section 5 uses 0.005
+        skill_mean=1.0, skill_std=1.0,    # f3: SKILL_NORMAL_CLIP parameters
         skill_max=5.0,
     )
 
@@ -86,7 +87,18 @@ def configs() -> dict:
         "config4_population": _cfg(256, 1000, 2, 1000, 1234, action_mix="market70", book_cap=1000, **big),
         # configs[4]: on-GPU rollout with the MLP policy (R=3)
         "config5_policy": _cfg(2048, 100, 3, 1000, 1234, action_mix="policy", **big),
+        # f3, the paper's section-5 workload: r = 4 / 12 resources (30 / 86 actions), prices {3,6,9}, taxes
+        # off, skills ~ N(1,1) that grow by 0.5 % per gather / craft toward 5 (clip [0,5]: G42), R_d = floor(log2 r) (G43)
+        "section5_r4": _cfg(4096, 100, 4, 1000, 1234, **section5(4)),
+        "section5_r12": _cfg(2048, 100, 12, 1000, 1234, **section5(12)),
     }
+
+
+def section5(R: int) -> dict:
+    """Parameter overrides of the paper's section-5 experiments for R resources."""
+    return dict(prices=[3, 6, 9], taxes_enabled=0, skill_init=SKILL_NORMAL_CLIP, skill_mean=1.0, skill_std=1.0,
+                skill_clip_lo=0.0, skill_clip_hi=5.0, skill_growth_rate=0.005, skill_max=5.0,
+                craft_distinct=max(1, int(math.floor(math.log2(R)))))
 
 
 def num_actions(R: int, P: int, craft_mode: int, allow_noop: int) -> int:

@@ -49,6 +49,12 @@ def test_factored_six_resources():
     _run("config3_resources", 3, 60, dict(tax_period=20))
 
 
+def test_factored_with_growing_skills():
+    # f3 under f2: the skill columns of the private block change at any step
+    _run("config2_paper", 4, 80, dict(tax_period=25, skill_growth_rate=0.005, skill_max=5.0))
+    _run("section5_r4", 3, 60)
+
+
 def test_factored_errors():
     import torch
 

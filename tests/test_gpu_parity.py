@@ -152,6 +152,71 @@ def test_shapes_of_generic_and_specialised_kernels(N, R, prices):
         pair.step_and_compare(acts[t], gov[t], "shape N=%d R=%d P=%d t=%d" % (N, R, len(prices), t), check_state=(t % 10 == 0 or t == 59))
 
 
+# ---------------- f3: skill growth (G41) ----------------
+GROWTH = dict(skill_growth_rate=0.005, skill_max=5.0)
+
+
+def test_skill_growth_step_parity():
+    # uniform skills in [0,1) grow toward 5; Pareto skills clipped to [1,10] start partly ABOVE the maximum, where the
+    # damped bonus is negative until the cap applies: both branches of the rule, state (skills included) bit-exact
+    grown = run_episode("tiny_dense", 6, 50, **GROWTH)
+    fixed = run_episode("tiny_dense", 6, 50)
+    assert (grown.g_state() != fixed.g_state()).any(), "growth left the skills unchanged"
+    run_episode("config2_paper", 5, 220, state_every=20, **GROWTH)
+    run_episode("config3_resources", 3, 120, state_every=10, craft_mode=inputs.CRAFT_PER_RESOURCE, **GROWTH)
+    run_episode("config2_paper", 3, 150, state_every=25, skill_growth_rate=0.25, skill_max=2.0)
+
+
+@pytest.mark.parametrize("R", [4, 12])
+def test_skill_growth_section5_shapes(R):
+    # the paper's section-5 workload: r = 4 / 12 resources, prices {3,6,9}, skills that grow
+    p = inputs.default_params()
+    p.update(prices=[3, 6, 9], episode_length=80, tax_period=20, thresholds=inputs.THRESHOLDS_7, craft_distinct=2, **GROWTH)
+    cfg = dict(E=4, N=100, R=R, T=80, seed=11, action_mix="uniform", params=p)
+    pair = Pair(4, 100, R, p, 11)
+    acts, gov = inputs.action_stream(cfg, 80, seed=11, E=4)
+    for t in range(80):
+        pair.step_and_compare(acts[t], gov[t], "growth R=%d t=%d" % (R, t), check_state=(t % 10 == 0 or t == 79))
+
+
+def test_normal_skill_init_and_section5_workload():
+    # EJ_SKILL_NORMAL_CLIP at reset (bit-exact skills), then the section-5 presets through the persistent rollout
+    for name, E in (("section5_r4", 5), ("section5_r12", 3)):
+        cfg = inputs.configs()[name]
+        assert binding_A(cfg) == {4: 30, 12: 86}[cfg["R"]]
+        pair = Pair(E, cfg["N"], cfg["R"], cfg["params"], 21)
+        compare_state(pair.g_state(), pair.o_state(), name + " reset")
+        sk = np.concatenate([oracle_skills(w) for w in pair.g_state()])
+        assert sk.min() >= 0.0 and sk.max() <= 5.0 and 0.9 < sk.mean() < 1.25 and (sk == 0.0).mean() > 0.1
+        _rollout_vs_oracle(name, E, 90)
+    _rollout_vs_oracle("section5_r4", 4096, 50, env_ids=[0, 1999, 4095], ring=2)
+    _rollout_vs_oracle("section5_r12", 2048, 40, env_ids=[0, 2047], ring=2)
+    run_episode("tiny_dense", 4, 50, skill_init=inputs.SKILL_NORMAL_CLIP, skill_mean=2.0, skill_std=0.5, skill_clip_lo=0.25,
+                skill_clip_hi=3.0)
+
+
+def binding_A(cfg):
+    p = cfg["params"]
+    return inputs.num_actions(cfg["R"], len(p["prices"]), p["craft_mode"], p["allow_noop"])
+
+
+def oracle_skills(words):
+    from oracle import parse_state
+    s = parse_state(words)
+    return np.concatenate([np.asarray(s["SG"], np.float64).ravel(), np.asarray(s["SC"], np.float64).ravel()])
+
+
+def test_skill_growth_rollout_and_bad_params():
+    from paper_2410_22165_b200 import binding
+
+    _rollout_vs_oracle("config2_paper", 6, 130, **GROWTH)
+    _rollout_vs_oracle("headline", 4096, 60, env_ids=[0, 2049, 4095], ring=2, **GROWTH)
+    cfg = inputs.configs()["config1_tiny"]
+    for bad in (dict(skill_growth_rate=-0.1, skill_max=5.0), dict(skill_growth_rate=0.005, skill_max=0.0)):
+        with pytest.raises(binding.EjError):
+            binding.Env(1, cfg["N"], cfg["R"], dict(cfg["params"], **bad))
+
+
 # ---------------- scripted worked examples, seeded into the GPU through the canonical dump ----------------
 def _scripted(N, R, params, setup, steps):
     """setup(oracle_env) scripts the oracle; its dump is loaded into the GPU env; both then step."""
