@@ -196,6 +196,20 @@ int ej_step(ej_env* h, const int32_t* actions, const int32_t* gov_actions, float
 int ej_step_host(ej_env* h, const int32_t* actions, const int32_t* gov_actions, float* obs_out, float* rew_out,
                  uint8_t* done_out);
 
+/* f2: the same step with HOST buffers and FACTORED observations.  Every value of the dense
+ * observation leaves once: the 3R + 4 agent-private columns per agent, the 5R + B + 2 env-wide columns (market
+ * statistics, tax rates, timers: P:424) once per env instead of N times, so the device->host copy carries
+ * 4 N (3R + 4) + 4 ceil4(5R + B + 2) instead of 4 N D_pop bytes per env (2.5x fewer at the headline shape).
+ *  actions, gov_actions  host, as ej_step
+ *  priv_out     host [E][N][3R + 4] float: columns 0 .. 3R + 3 of the dense population rows
+ *  shared_out   host [E][ceil4(5R + B + 2)] float: columns 3R + 4 .. D_pop - 1 of every row of the env
+ *  gov_obs_out  host [E][D_gov_pad] float, or NULL
+ *  rew_out      host [E][N+1] float, or NULL;  done_out  host [E] uint8, or NULL
+ * Shapes whose rows cannot be staged (see ej_rollout_io.obs_priv_ring) and policy mode: EJ_ERR_PARAM.
+ * Synchronises the stream before returning; staging buffers are library-owned. */
+int ej_step_host_factored(ej_env* h, const int32_t* actions, const int32_t* gov_actions, float* priv_out,
+                          float* shared_out, float* gov_obs_out, float* rew_out, uint8_t* done_out);
+
 /* T steps in ONE persistent launch: each env's state stays in shared memory for the whole
  * call.  Actions come from io->actions_in / gov_actions_in or, when NULL, from the Philox/CDF
  * generator (ej_set_action_cdf; uniform over the A actions by default).  io may be NULL

@@ -72,7 +72,7 @@ class EjMlp(C.Structure):
 
 
 EXPORTS = ("ej_create", "ej_destroy", "ej_set_stream", "ej_layout", "ej_last_error", "ej_reset", "ej_observe",
-           "ej_step", "ej_step_host", "ej_rollout", "ej_set_action_cdf", "ej_get_state", "ej_set_state",
+           "ej_step", "ej_step_host", "ej_step_host_factored", "ej_rollout", "ej_set_action_cdf", "ej_get_state", "ej_set_state",
            "ej_launch_count", "ej_set_policy", "ej_policy_act", "ej_action_mask", "ej_set_action_masking")
 
 _lib = None
@@ -98,6 +98,7 @@ def lib():
         L.ej_set_action_masking.argtypes = [vp, C.c_int32]
         L.ej_step.argtypes = [vp, vp, vp, vp, vp, vp]
         L.ej_step_host.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.ej_step_host_factored.argtypes = [vp] * 8
         L.ej_rollout.argtypes = [vp, C.c_int32, C.POINTER(EjRolloutIO)]
         L.ej_set_action_cdf.argtypes = [vp, vp, C.c_int32]
         L.ej_get_state.argtypes = [vp, C.c_int32, C.c_int32, vp, C.c_size_t]
@@ -197,6 +198,11 @@ def ej_step(h, actions: int, gov_actions: int, obs_out: int | None, rew_out: int
 
 def ej_step_host(h, actions: int, gov_actions: int, obs_out: int | None, rew_out: int | None, done_out: int | None):
     _check(h, lib().ej_step_host(h, actions, gov_actions, obs_out, rew_out, done_out))
+
+
+def ej_step_host_factored(h, actions: int, gov_actions: int, priv_out: int, shared_out: int, gov_obs_out: int | None,
+                          rew_out: int | None, done_out: int | None):
+    _check(h, lib().ej_step_host_factored(h, actions, gov_actions, priv_out, shared_out, gov_obs_out, rew_out, done_out))
 
 
 def ej_rollout(h, T: int, io: EjRolloutIO | None):
@@ -336,6 +342,12 @@ class Env:
         ej_step_host(self.h, actions.ctypes.data, gov_actions.ctypes.data,
                      None if obs is None else obs.ctypes.data, None if rew is None else rew.ctypes.data,
                      None if done is None else done.ctypes.data)
+
+    def step_host_factored(self, actions: np.ndarray, gov_actions: np.ndarray, priv: np.ndarray, shared: np.ndarray,
+                           gov_obs: np.ndarray | None = None, rew: np.ndarray | None = None, done: np.ndarray | None = None):
+        p = lambda a: None if a is None else a.ctypes.data
+        ej_step_host_factored(self.h, actions.ctypes.data, gov_actions.ctypes.data, priv.ctypes.data, shared.ctypes.data,
+                              p(gov_obs), p(rew), p(done))
 
     def set_policy(self, pop_net: dict | None, gov_net: dict | None):
         if pop_net is None and gov_net is None:

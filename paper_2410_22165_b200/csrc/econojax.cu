@@ -40,6 +40,9 @@ struct ej_env {
     int32_t *d_act = nullptr, *d_gov = nullptr;
     float *d_obs = nullptr, *d_rew = nullptr;
     uint8_t* d_done = nullptr;
+    // staging for ej_step_host_factored: one allocation, byte offsets of its sections
+    uint8_t* d_fx = nullptr;
+    size_t fx_act = 0, fx_gov = 0, fx_priv = 0, fx_shared = 0, fx_govrow = 0, fx_rew = 0, fx_done = 0;
     // a12: installed policies and the buffers the policy-driven rollout chains through
     bool has_policy = false;
     PolicyNet pop_net{}, gov_net{};
@@ -526,7 +529,7 @@ int ej_destroy(ej_env* h) {
     if (!h) return EJ_OK;
     cudaStreamSynchronize(h->stream);
     cudaFree(h->d_state); cudaFree(h->d_cdf);
-    cudaFree(h->d_act); cudaFree(h->d_gov); cudaFree(h->d_obs); cudaFree(h->d_rew); cudaFree(h->d_done);
+    cudaFree(h->d_act); cudaFree(h->d_gov); cudaFree(h->d_obs); cudaFree(h->d_rew); cudaFree(h->d_done); cudaFree(h->d_fx);
     cudaFree(h->d_pop_blob); cudaFree(h->d_gov_blob); cudaFree(h->d_pobs); cudaFree(h->d_pact); cudaFree(h->d_pgov);
     delete h;
     return EJ_OK;
@@ -631,6 +634,44 @@ int ej_step_host(ej_env* h, const int32_t* actions, const int32_t* gov_actions, 
     if (rew_out) EJ_CUDA(h, cudaMemcpyAsync(rew_out, h->d_rew, (EN + c.E) * 4, cudaMemcpyDeviceToHost, h->stream), "D2H rewards");
     if (done_out) EJ_CUDA(h, cudaMemcpyAsync(done_out, h->d_done, (size_t)c.E, cudaMemcpyDeviceToHost, h->stream), "D2H done");
     EJ_CUDA(h, cudaStreamSynchronize(h->stream), "ej_step_host sync");
+    return EJ_OK;
+}
+
+int ej_step_host_factored(ej_env* h, const int32_t* actions, const int32_t* gov_actions, float* priv_out, float* shared_out,
+                          float* gov_obs_out, float* rew_out, uint8_t* done_out) {
+    if (!h) return EJ_ERR_PARAM;
+    if (!actions) return fail(h, EJ_ERR_PARAM, "bad field: %s", "actions");
+    if (!gov_actions) return fail(h, EJ_ERR_PARAM, "bad field: %s", "gov_actions");
+    if (!priv_out || !shared_out) return fail(h, EJ_ERR_PARAM, "bad field: %s", "priv_out / shared_out (set both)");
+    const DevCfg& c = h->c;
+    const size_t EN = (size_t)c.E * c.N, EB = (size_t)c.E * c.B;
+    const size_t n_priv = EN * (size_t)(3 * c.R + 4), n_shared = (size_t)c.E * (size_t)((5 * c.R + c.B + 2 + 3) & ~3);
+    const size_t n_gov = (size_t)c.E * c.D_gov_pad;
+    if (!h->d_fx) {  // one allocation: actions | gov actions | priv | shared | gov rows | rewards | done
+        size_t off = 0;
+        auto take = [&off](size_t bytes) { const size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
+        h->fx_act = take(EN * 4); h->fx_gov = take(EB * 4); h->fx_priv = take(n_priv * 4); h->fx_shared = take(n_shared * 4);
+        h->fx_govrow = take(n_gov * 4); h->fx_rew = take((EN + c.E) * 4); h->fx_done = take((size_t)c.E);
+        if (cudaMalloc(&h->d_fx, off) != cudaSuccess) { cudaGetLastError(); h->d_fx = nullptr; return fail(h, EJ_ERR_NOMEM, "%s", "staging allocation failed"); }
+    }
+    uint8_t* const d = h->d_fx;
+    EJ_CUDA(h, cudaMemcpyAsync(d + h->fx_act, actions, EN * 4, cudaMemcpyHostToDevice, h->stream), "H2D actions");
+    EJ_CUDA(h, cudaMemcpyAsync(d + h->fx_gov, gov_actions, EB * 4, cudaMemcpyHostToDevice, h->stream), "H2D gov_actions");
+    ej_rollout_io rio;
+    memset(&rio, 0, sizeof(rio));
+    rio.struct_size = sizeof(rio); rio.ring_depth = 1;
+    rio.actions_in = (const int32_t*)(d + h->fx_act); rio.gov_actions_in = (const int32_t*)(d + h->fx_gov);
+    rio.obs_priv_ring = (float*)(d + h->fx_priv); rio.obs_shared_ring = (float*)(d + h->fx_shared);
+    rio.obs_gov_ring = gov_obs_out ? (float*)(d + h->fx_govrow) : nullptr;
+    rio.rew_ring = rew_out ? (float*)(d + h->fx_rew) : nullptr; rio.done_ring = done_out ? d + h->fx_done : nullptr;
+    const int rc = ej_rollout(h, 1, &rio);
+    if (rc != EJ_OK) return rc;
+    EJ_CUDA(h, cudaMemcpyAsync(priv_out, d + h->fx_priv, n_priv * 4, cudaMemcpyDeviceToHost, h->stream), "D2H private block");
+    EJ_CUDA(h, cudaMemcpyAsync(shared_out, d + h->fx_shared, n_shared * 4, cudaMemcpyDeviceToHost, h->stream), "D2H env-wide block");
+    if (gov_obs_out) EJ_CUDA(h, cudaMemcpyAsync(gov_obs_out, d + h->fx_govrow, n_gov * 4, cudaMemcpyDeviceToHost, h->stream), "D2H government rows");
+    if (rew_out) EJ_CUDA(h, cudaMemcpyAsync(rew_out, d + h->fx_rew, (EN + c.E) * 4, cudaMemcpyDeviceToHost, h->stream), "D2H rewards");
+    if (done_out) EJ_CUDA(h, cudaMemcpyAsync(done_out, d + h->fx_done, (size_t)c.E, cudaMemcpyDeviceToHost, h->stream), "D2H done");
+    EJ_CUDA(h, cudaStreamSynchronize(h->stream), "ej_step_host_factored sync");
     return EJ_OK;
 }
 

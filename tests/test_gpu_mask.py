@@ -142,3 +142,16 @@ def test_masked_rollout_six_resources():
 def test_masked_rollout_full_size_sampled_envs():
     cfg = inputs.configs()["headline"]
     _masked_rollout("headline", cfg["E"], 40, env_ids=[0, 1500, cfg["E"] - 1], seed=cfg["seed"])
+
+
+def test_masked_rollout_section5_growing_skills():
+    # the paper's section-5 workload as its agents meet it: masked draws over 30 / 86 actions while the
+    # skills grow; the mask of the reached state, byte for byte
+    import oracle
+    import torch
+    for name, E in (("section5_r4", 4), ("section5_r12", 2)):
+        pair = _masked_rollout(name, E, 70)
+        assert sum(int(oracle.parse_state(w)["counters"][2]) for w in pair.g.get_state()) == 0
+        mg = pair.g.action_mask()
+        torch.cuda.synchronize()
+        assert np.array_equal(mg.cpu().numpy(), pair.o[0].action_mask()), name

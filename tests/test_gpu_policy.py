@@ -91,12 +91,13 @@ def test_policy_act_logits_and_samples(std, bias_std, E):
     assert an.min() >= 0 and an.max() < g.A and len(np.unique(an)) > 5
 
 
-def test_policy_rollout_teacher_forced():
+@pytest.mark.parametrize("over", [{}, dict(skill_growth_rate=0.005, skill_max=5.0)], ids=["fixed_skills", "growing_skills"])
+def test_policy_rollout_teacher_forced(over):
     import torch
 
     cfg = inputs.configs()["config5_policy"]
     N, R, E, T = cfg["N"], cfg["R"], 5, 64
-    params = dict(cfg["params"], tax_period=16)
+    params = dict(cfg["params"], tax_period=16, **over)   # f3: the policy observes skills that grow
     pair = Pair(E, N, R, params, cfg["seed"])
     g = pair.g
     pop, gov = inputs.policy_weights(cfg, seed=0, std=0.3, bias_std=0.1)  # non-uniform action distributions
