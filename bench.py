@@ -320,6 +320,30 @@ def main():
                "d2h_bytes_per_step": int(4 * env.obs_floats + 4 * E * (N + 1) + E),
                "steps": Ke, "ms_per_step": e_ms / Ke, "api": "ej_step_host (pinned host buffers)"}
 
+        # the same through ej_step_host_factored (f2): every observation value once, env-wide columns once per env
+        if fx is not None:
+            dpv, dsh = 3 * cfg["R"] + 4, (5 * cfg["R"] + B + 2 + 3) // 4 * 4
+            h_priv = torch.zeros((E, N, dpv), dtype=torch.float32).pin_memory()
+            h_shared = torch.zeros((E, dsh), dtype=torch.float32).pin_memory()
+            h_govr = torch.zeros((E, env.D_gov_pad), dtype=torch.float32).pin_memory()
+            env.reset(cfg["seed"])
+            step_fx = lambda t: lib.ej_step_host_factored(env.h, h_acts[t].data_ptr(), h_gov[t].data_ptr(), h_priv.data_ptr(),
+                                                          h_shared.data_ptr(), h_govr.data_ptr(), h_rew.data_ptr(), h_done.data_ptr())
+            for t in range(3):
+                step_fx(t)
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for t in range(Ke):
+                step_fx(t)
+            e1.record()
+            barrier()
+            f_ms = sharding.max_over_ranks(e0.elapsed_time(e1), dist, dev)
+            e2e["factored"] = {"value": world * E * N * Ke / (f_ms * 1e-3), "unit": UNIT, "ms_per_step": f_ms / Ke,
+                               "h2d_bytes_per_step": int(4 * E * N + 4 * E * B),
+                               "d2h_bytes_per_step": int(4 * E * (N * dpv + dsh + env.D_gov_pad) + 4 * E * (N + 1) + E),
+                               "api": "ej_step_host_factored (pinned host buffers; same observation values, env-wide columns once per env)"}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()

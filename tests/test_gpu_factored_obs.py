@@ -55,6 +55,38 @@ def test_factored_with_growing_skills():
     _run("section5_r4", 3, 60)
 
 
+def test_step_host_factored_against_the_oracle():
+    # ej_step_host_factored: host buffers in and out, one step per call; every column against the oracle's dense rows
+    from parity import Pair, close, compare_state, exact
+
+    for name, E, over in (("config2_paper", 4, dict(tax_period=10)), ("section5_r4", 3, {})):
+        cfg = inputs.configs()[name]
+        params = dict(cfg["params"], **over)
+        pair = Pair(E, cfg["N"], cfg["R"], params, 8)
+        g = pair.g
+        acts, gov = inputs.action_stream(dict(cfg, params=params), 35, seed=8, E=E)
+        priv = np.zeros((E, cfg["N"], g.D_priv), np.float32)
+        shared = np.zeros((E, g.D_shared_pad), np.float32)
+        govr = np.zeros((E, g.D_gov_pad), np.float32)
+        rew = np.zeros((E, cfg["N"] + 1), np.float32)
+        done = np.zeros(E, np.uint8)
+        for t in range(35):
+            if t % 2:
+                g.step_host_factored(acts[t], gov[t], priv, shared, govr, rew, done)
+            else:   # optional outputs left out
+                g.step_host_factored(acts[t], gov[t], priv, shared)
+            o_pop, o_gov, o_rew, o_done = pair.o[0].step(acts[t], gov[t])
+            exact(priv, o_pop[:, :, : g.D_priv], "%s t=%d private block" % (name, t))
+            exact(shared[:, : g.D_shared], o_pop[:, 0, g.D_priv:], "%s t=%d env-wide block" % (name, t))
+            if t % 2:
+                close(govr[:, : g.D_gov], o_gov, "%s t=%d government rows" % (name, t))
+                close(rew, o_rew, "%s t=%d rewards" % (name, t))
+                exact(done, o_done.astype(np.uint8), "%s t=%d done" % (name, t))
+        compare_state(pair.g_state(), pair.o_state(), name + " state after host factored steps")
+        with pytest.raises(binding.EjError):
+            binding.ej_step_host_factored(g.h, acts[0].ctypes.data, gov[0].ctypes.data, priv.ctypes.data, None, None, None, None)
+
+
 def test_factored_errors():
     import torch
 
