@@ -201,10 +201,14 @@ void select_step_kernel(ej_env* h) {
 #ifndef EJ_DEV_ONLY_128
             pick(std::integral_constant<int, 3>(), I10(), I100(), I7(), I1());
             pick(std::integral_constant<int, 6>(), I10(), I100(), I7(), I1());
+            // f3, the paper's section-5 shapes: prices {3,6,9}, 3 brackets; r = 4 keeps Table 2's mechanics
+            // (R_d = floor(log2 4) = 2), r = 12 has R_d = 3 and gets R and P only
+            pick(std::integral_constant<int, 4>(), std::integral_constant<int, 3>(), I100(), std::integral_constant<int, 3>(), I1());
 #endif
         }
 #ifndef EJ_DEV_ONLY_128
         if (h->step_RT == 0) pick(I2(), std::integral_constant<int, 5>(), I0(), I0(), I0());
+        if (h->step_RT == 0) pick(std::integral_constant<int, 12>(), std::integral_constant<int, 3>(), I0(), I0(), I0());
 #endif
     }
     if constexpr (MT == 1024 && NS == 1024) {
