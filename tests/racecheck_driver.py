@@ -1,5 +1,5 @@
 """Small driver for compute-sanitizer (racecheck / memcheck): a few steps of ej_step, a short
-ej_rollout with generated actions, and a policy-driven rollout, on shapes that exercise the
+ej_rollout with generated actions, a policy-driven rollout, masked sampling, factored observations and the section-5 variants, on shapes that exercise the
 specialised kernel, the generic kernel and the book-cap path.  Not collected by pytest.
 
     compute-sanitizer --tool racecheck python tests/racecheck_driver.py
@@ -46,5 +46,18 @@ if __name__ == "__main__":
     env2 = run("config2_paper", 2, 3)
     env2.set_action_masking(True)
     env2.rollout(6)
+    # f2 / f3: factored rings, growing skills, normal skill init, the section-5 kernel variants, host factored step
+    for name, E in (("section5_r4", 2), ("section5_r12", 1)):
+        env3 = run(name, E, 5)
+        c3 = inputs.configs()[name]
+        if name == "section5_r4":
+            priv, shared, govr = env3.new_factored_obs(2)
+            env3.rollout(4, ring_depth=2, obs_priv_ring=priv, obs_shared_ring=shared, obs_gov_ring=govr)
+            a3, g3 = inputs.action_stream(c3, 2, seed=4, E=E)
+            hp = np.zeros((E, c3["N"], env3.D_priv), np.float32)
+            hs = np.zeros((E, env3.D_shared_pad), np.float32)
+            for t in range(2):
+                env3.step_host_factored(a3[t], g3[t], hp, hs)
+    run("config2_paper", 2, 6, tax_period=3, skill_growth_rate=0.005, skill_max=5.0)
     torch.cuda.synchronize()
     print("driver done")
