@@ -123,3 +123,62 @@ class Pair:
                         o_done, what)
         if check_state:
             compare_state(self.g_state(), self.o_state(), what + " state")
+
+
+def check_dump_invariants(w, cfg, steps):
+    """What the rules fix at any size, checked vectorised on the canonical dump `w`
+    (int32 [E][state_words]) of envs that ran `steps` steps: escrow = sum of the agent's live orders, live-order
+    counts and cap, ages below the expiry, books in priority order and uncrossed,
+    prices on the grid, nothing negative, clock and counters consistent."""
+    E, N, R, p = w.shape[0], cfg["N"], cfg["R"], cfg["params"]
+    B, P, M = len(p["thresholds"]) + 1, len(p["prices"]), p["max_active_orders"]
+    cap = int(w[0, 5])
+    assert (w[:, 0] == steps).all() and (w[:, 1] == N).all() and (w[:, 2] == R).all() and (w[:, 3] == B).all() and (w[:, 4] == P).all()
+    q = 13 + B + R
+    rec = 6 + 3 * R
+    ag = w[:, q:q + N * rec].reshape(E, N, rec)
+    q += N * rec
+    f32 = lambda a: np.ascontiguousarray(a, np.int32).view(np.float32)
+    coin, labor = f32(ag[:, :, 0]), f32(ag[:, :, 3])
+    esc_coin, n_live = ag[:, :, 1], ag[:, :, 5]
+    inv, esc_res = ag[:, :, 6:6 + R], ag[:, :, 6 + R:6 + 2 * R]
+    assert (coin >= 0).all() and np.isfinite(coin).all() and (labor >= 0).all()
+    assert (inv >= 0).all() and (esc_res >= 0).all() and (esc_coin >= 0).all()
+    live = np.zeros((E, N), np.int64)
+    want_coin = np.zeros((E, N), np.int64)
+    want_res = np.zeros((E, N, R), np.int64)
+    env_idx = np.repeat(np.arange(E), cap).reshape(E, cap)
+    best = {}
+    n_orders = 0
+    for b in range(2 * R):
+        n = w[:, q]
+        book = w[:, q + 1:q + 1 + 3 * cap].reshape(E, cap, 3)
+        q += 1 + 3 * cap
+        assert (n >= 0).all() and (n <= cap).all()
+        valid = np.arange(cap)[None, :] < n[:, None]
+        price, owner, placed = book[:, :, 0][valid], book[:, :, 1][valid], book[:, :, 2][valid]
+        e_of = env_idx[valid]
+        n_orders += int(valid.sum())
+        assert np.isin(price, p["prices"]).all() and (owner >= 0).all() and (owner < N).all()
+        age = (steps - 1) - placed
+        assert (age >= 0).all() and (age < p["order_expiry"]).all()
+        np.add.at(live, (e_of, owner), 1)
+        if b % 2 == 0:
+            np.add.at(want_coin, (e_of, owner), price.astype(np.int64))
+        else:
+            np.add.at(want_res, (e_of, owner, b // 2), 1)
+        # priority order: bids by falling price, asks by rising price; among equal prices the older order first
+        pr = np.where(valid, book[:, :, 0], np.int32(-1 if b % 2 == 0 else 1 << 20))
+        d = np.diff(pr, axis=1)
+        assert (d <= 0).all() if b % 2 == 0 else (d >= 0).all()
+        both = valid[:, 1:] & valid[:, :-1] & (d == 0)
+        assert (np.diff(book[:, :, 2], axis=1)[both] >= 0).all()
+        best[b] = np.where(n > 0, book[:, 0, 0], -1)
+    assert q == w.shape[1]
+    assert (want_coin == esc_coin).all() and (want_res == esc_res).all()            # escrow = sum of live orders
+    assert (live == n_live).all() and live.max() <= M                                # P:277
+    for r in range(R):                                                               # uncrossed after matching
+        bb, ab = best[2 * r], best[2 * r + 1]
+        both = (bb >= 0) & (ab >= 0)
+        assert (bb[both] < ab[both]).all()
+    return n_orders

@@ -453,3 +453,36 @@ def test_government_statistics_on_adversarial_states(name):
         close(gov.cpu().numpy(), o_gov, "%s round %d (%s) gov obs" % (name, rnd, shape))
         acts = np.full((E, N), A - 1, np.int32)  # everyone idles: the step kernel's statistics of the same state
         pair.step_and_compare(acts, np.zeros((E, pair.g.B), np.int32), "%s round %d (%s) noop step" % (name, rnd, shape))
+
+
+# ---------------- properties that hold at any size, checked on EVERY env of the full-size launches ----------------
+def _check_invariants_all_envs(name, steps):
+    """Full-size rollout as bench.py launches it; parity.check_dump_invariants on the dump of all E envs."""
+    import torch
+    from paper_2410_22165_b200 import binding
+    from parity import check_dump_invariants
+
+    cfg = inputs.configs()[name]
+    E = cfg["E"]
+    env = binding.Env(E, cfg["N"], cfg["R"], cfg["params"])
+    env.reset(cfg["seed"])
+    env.set_action_cdf(inputs.action_cdf(cfg))
+    env.rollout(steps)
+    torch.cuda.synchronize()
+    w = np.concatenate([env.get_state(b, min(512, E - b)) for b in range(0, E, 512)])   # int32 [E][state_words]
+    assert w.shape[0] == E
+    check_dump_invariants(w, cfg, steps)
+    trades = w[:, 6]
+    assert (trades > 0).mean() > 0.99                                                 # the workload really trades
+    assert len(np.unique(w[:, 6:11], axis=0)) > E // 4                                # envs are keyed by their id
+
+
+def test_full_size_invariants_on_every_env_headline():
+    _check_invariants_all_envs("headline", 75)
+
+
+def test_full_size_invariants_on_every_env_other_workloads():
+    _check_invariants_all_envs("config3_resources", 45)
+    _check_invariants_all_envs("section5_r4", 45)
+    _check_invariants_all_envs("section5_r12", 40)
+    _check_invariants_all_envs("config4_population", 35)     # N = 1000, book cap K = N (G15)

@@ -446,3 +446,23 @@ def test_env_wide_tail_of_the_population_rows_is_identical_for_all_agents():
         assert (tail == tail[:, :1, :]).all()
         varied += int((pop[:, :, :3 * R + 4] != pop[:, :1, :3 * R + 4]).any())
     assert varied > 0  # while the private block does differ between agents
+
+
+@pytest.mark.parametrize("name,E,steps", [("config2_paper", 5, 60), ("tiny_dense", 8, 50), ("section5_r4", 3, 40)])
+def test_dump_invariant_checker_accepts_the_oracle_and_rejects_a_broken_dump(name, E, steps):
+    # parity.check_dump_invariants is what the GPU tests run on every env of the full-size launches
+    from parity import check_dump_invariants
+    cfg = inputs.configs()[name]
+    o = oracle.OracleEnv(E, cfg["N"], cfg["R"], cfg["params"])
+    o.reset(2)
+    cdf = inputs.action_cdf(cfg)
+    for _ in range(steps):
+        a, g = o.draw_actions(cdf)
+        o.step(a, g, want_obs=False)
+    w = np.asarray(o.get_state())
+    check_dump_invariants(w, cfg, steps)
+    B = len(cfg["params"]["thresholds"]) + 1
+    bad = w.copy()
+    bad[0, 13 + B + cfg["R"] + 1] += 1          # agent 0's escrowed coin no longer equals its live bids
+    with pytest.raises(AssertionError):
+        check_dump_invariants(bad, cfg, steps)
