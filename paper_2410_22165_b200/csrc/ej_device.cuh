@@ -1194,17 +1194,34 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
     uint8_t* const sblob = ej_smem + Lay<NS>::blob;
     const int e = blockIdx.x, tid = threadIdx.x;
     const Sm<NS, (PF ? RT : 0), (PF ? PT : 0), (PF ? NT : 0)> m{c};
-    uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
-    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
+    uint8_t* const blob = state + (size_t)e * c.blob_bytes;
+    // The state blob comes in as ONE 1-D TMA bulk copy that completes on an mbarrier (misc()[1]) while the CTA
+    // clears its scratch and builds its tables, and leaves as one bulk store: with one launch per step (ej_step)
+    // the blob traffic is as large as the outputs, and a copy loop costs issue slots the step itself needs.
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&m.misc()[1]);
     for (int i = tid; i < Lay<NS>::blob / 16; i += NPAD) ((uint4*)ej_smem)[i] = make_uint4(0u, 0u, 0u, 0u);
     for (int i = tid; i < (c.o_stage - c.o_scratch1) / 16; i += NPAD) ((uint4*)(ej_smem + c.o_scratch1))[i] = make_uint4(0u, 0u, 0u, 0u);
     __syncthreads();
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar) : "memory");
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(c.blob_bytes) : "memory");
+        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                         (uint32_t)__cvta_generic_to_shared(sblob)),
+                     "l"(blob), "r"(c.blob_bytes), "r"(bar)
+                     : "memory");
+    }
     if (c.K == 0)
         for (int l = tid; l < c.n_levels; l += NPAD) m.ahead()[l] = NIL;
     if (!io.actions)
         for (int i = tid; i < c.A; i += NPAD) m.cdf()[i] = io.cdf[i];
     build_coltab<NS>(c, m, tid, NPAD);
-    __syncthreads();
+    __syncthreads();  // the tables above, and the mbarrier's initialisation, for every thread
+    asm volatile(
+        "{\n\t.reg .pred p;\n\tEJ_BLOB_WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], 0;\n\t"
+        "@p bra EJ_BLOB_DONE_%=;\n\tbra EJ_BLOB_WAIT_%=;\n\tEJ_BLOB_DONE_%=:\n\t}" ::"r"(bar)
+        : "memory");
     StepPtrs p{io, c, 0, 0};
 #pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
@@ -1212,9 +1229,15 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
         env_step<NPAD, NS, RT, PT, NT, BT, PF, FX>(c, m, tid, e, p, s == 0);
         p.slot = (p.slot + 1 == io.ring_depth) ? 0 : p.slot + 1;
     }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // this thread's state writes, for the bulk store below
     __syncthreads();
-    for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)sblob)[i];
-    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    if (tid == 0) {
+        asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(blob), "r"((uint32_t)__cvta_generic_to_shared(sblob)),
+                     "r"(c.blob_bytes)
+                     : "memory");
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    }
 }
 
 template <int NPAD, int NS>
