@@ -15,7 +15,8 @@
  *  - Every function returns 0 (EJ_OK) or a negative EJ_ERR_* code; ej_last_error() gives a
  *    static/handle-owned string naming the offending field.  No exceptions, no errno.
  *  - "device pointer" = memory of the CUDA device that was current at ej_create; it is owned
- *    by the caller, must be 16-byte aligned, is not retained after the call returns, but must
+ *    by the caller, must be 16-byte aligned (observation buffers and rings: checked, EJ_ERR_PARAM;
+ *    int32 / float arrays: 4-byte aligned at least), is not retained after the call returns, but must
  *    stay alive until the handle's stream has executed the call (calls are asynchronous on
  *    the stream set by ej_set_stream, default stream 0).  "host pointer" = ordinary memory.
  *  - There is no CPU fallback: every step of the path runs in the sm_100a kernels of
@@ -109,6 +110,9 @@ typedef struct ej_layout_info {
     size_t device_state_bytes;  /* library-owned device bytes per env */
     size_t smem_bytes;          /* dynamic shared memory per CTA of the step kernel */
     int32_t threads_per_env;    /* CTA size */
+    int32_t D_priv;             /* f2: 3R + 4 agent-private columns of a population row */
+    int32_t D_shared;           /* f2: 5R + B + 2 env-wide columns (market statistics, rates, timers: P:424) */
+    int32_t D_shared_pad;       /* D_shared rounded up to a multiple of 4 (row stride of obs_shared_ring) */
 } ej_layout_info;
 
 /* Optional inputs/outputs of ej_rollout; all device pointers, any may be NULL. */
@@ -129,7 +133,7 @@ typedef struct ej_rollout_io {
      * can leave as an agent-private block and one env-wide block.  Column k < 3R + 4 of obs row
      * (e, i) = priv[e][i][k]; column 3R + 4 + k = shared[e][k].  Set priv and shared together and
      * leave obs_ring NULL; needs N * (3R + 4) to be a multiple of 4 and a shape whose full tile is
-     * staged in shared memory (N <= 256 and N * D_pop * 4 bytes <= ~70 KB), not available in policy mode:
+     * staged in shared memory (N <= 256 and state + scratch + N * D_pop * 4 bytes <= 100 KB per CTA), not available in policy mode:
      * EJ_ERR_PARAM otherwise. */
     float* obs_priv_ring;             /* [ring_depth][E][N][3R + 4] */
     float* obs_shared_ring;           /* [ring_depth][E][ceil4(5R + B + 2)] */
@@ -224,7 +228,12 @@ int ej_set_action_cdf(ej_env* h, const uint32_t* cdf, int32_t A);
 
 /* Canonical, representation-free state dump of envs [env_begin, env_begin+env_count) into /
  * from a HOST buffer of env_count*state_words int32 words (layout: DESIGN.md "Canonical state
- * dump").  Both synchronise the stream.  Cold path: used by tests and checkpointing. */
+ * dump").  Both synchronise the stream.  Cold path: used by tests and checkpointing.
+ * The dump holds the state of the economies, not the Philox key: ej_set_state needs a handle that was
+ * reset (EJ_ERR_STATE otherwise), and a restored run continues draw for draw only if that ej_reset used
+ * the seed of the run the dump was taken from.  ej_set_state rejects (EJ_ERR_PARAM) dumps whose books are
+ * crossed (best bid >= best ask: resting books are uncrossed after every step, G13), whose orders are off
+ * the price grid or exceed max_active_orders per agent. */
 int ej_get_state(ej_env* h, int32_t env_begin, int32_t env_count, int32_t* words, size_t n_words);
 int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t* words, size_t n_words);
 

@@ -48,7 +48,7 @@ class EjLayoutInfo(C.Structure):
         ("noop_action", C.c_int32), ("D_pop", C.c_int32), ("D_gov", C.c_int32), ("D_gov_pad", C.c_int32),
         ("gov_obs_offset", C.c_size_t), ("obs_floats", C.c_size_t), ("rew_floats", C.c_size_t),
         ("state_words", C.c_size_t), ("device_state_bytes", C.c_size_t), ("smem_bytes", C.c_size_t),
-        ("threads_per_env", C.c_int32),
+        ("threads_per_env", C.c_int32), ("D_priv", C.c_int32), ("D_shared", C.c_int32), ("D_shared_pad", C.c_int32),
     ]
 
 
@@ -337,17 +337,35 @@ class Env:
         ej_step(self.h, actions.data_ptr(), gov_actions.data_ptr(), _dp(obs), _dp(rew), _dp(done))
         return obs, rew, done
 
+    def _host_in(self, a, n):
+        """Host input as contiguous int32 (numpy's default integer is 64-bit: convert, never reinterpret)."""
+        a = np.ascontiguousarray(a, np.int32)
+        assert a.size == n, "expected %d int32 values, got %d" % (n, a.size)
+        return a
+
+    @staticmethod
+    def _host_out(a, dtype, n, what):
+        """Host output buffer the library writes through a raw pointer: dtype, size and contiguity are checked."""
+        if a is None:
+            return None
+        assert isinstance(a, np.ndarray) and a.dtype == dtype and a.flags["C_CONTIGUOUS"] and a.flags["WRITEABLE"] and a.size >= n, \
+            "%s must be a writable C-contiguous %s array of at least %d elements" % (what, np.dtype(dtype).name, n)
+        return a.ctypes.data
+
     def step_host(self, actions: np.ndarray, gov_actions: np.ndarray, obs: np.ndarray | None, rew: np.ndarray | None,
                   done: np.ndarray | None):
-        ej_step_host(self.h, actions.ctypes.data, gov_actions.ctypes.data,
-                     None if obs is None else obs.ctypes.data, None if rew is None else rew.ctypes.data,
-                     None if done is None else done.ctypes.data)
+        a, g = self._host_in(actions, self.E * self.N), self._host_in(gov_actions, self.E * self.B)
+        ej_step_host(self.h, a.ctypes.data, g.ctypes.data, self._host_out(obs, np.float32, self.obs_floats, "obs"),
+                     self._host_out(rew, np.float32, self.rew_floats, "rew"), self._host_out(done, np.uint8, self.E, "done"))
 
     def step_host_factored(self, actions: np.ndarray, gov_actions: np.ndarray, priv: np.ndarray, shared: np.ndarray,
                            gov_obs: np.ndarray | None = None, rew: np.ndarray | None = None, done: np.ndarray | None = None):
-        p = lambda a: None if a is None else a.ctypes.data
-        ej_step_host_factored(self.h, actions.ctypes.data, gov_actions.ctypes.data, priv.ctypes.data, shared.ctypes.data,
-                              p(gov_obs), p(rew), p(done))
+        a, g = self._host_in(actions, self.E * self.N), self._host_in(gov_actions, self.E * self.B)
+        ej_step_host_factored(self.h, a.ctypes.data, g.ctypes.data,
+                              self._host_out(priv, np.float32, self.E * self.N * self.D_priv, "priv"),
+                              self._host_out(shared, np.float32, self.E * self.D_shared_pad, "shared"),
+                              self._host_out(gov_obs, np.float32, self.E * self.D_gov_pad, "gov_obs"),
+                              self._host_out(rew, np.float32, self.rew_floats, "rew"), self._host_out(done, np.uint8, self.E, "done"))
 
     def set_policy(self, pop_net: dict | None, gov_net: dict | None):
         if pop_net is None and gov_net is None:
@@ -375,19 +393,7 @@ class Env:
         io.obs_priv_ring, io.obs_shared_ring, io.obs_gov_ring = _dp(obs_priv_ring), _dp(obs_shared_ring), _dp(obs_gov_ring)
         ej_rollout(self.h, T, io)
 
-    # f2, factored observations (shapes of the three rings of one step)
-    @property
-    def D_priv(self):
-        return 3 * self.R + 4
-
-    @property
-    def D_shared(self):
-        return 5 * self.R + self.B + 2
-
-    @property
-    def D_shared_pad(self):
-        return (self.D_shared + 3) // 4 * 4
-
+    # f2, factored observations: the three rings of one step (widths from ej_layout)
     def new_factored_obs(self, depth=1):
         t = self.torch
         z = lambda *shape: t.zeros(shape, dtype=t.float32, device=self.device)

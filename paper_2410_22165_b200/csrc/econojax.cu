@@ -8,8 +8,11 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <map>
+#include <mutex>
 #include <new>
 #include <type_traits>
+#include <utility>
 #include <vector>
 
 #include "ej_device.cuh"
@@ -217,12 +220,36 @@ void select_step_kernel(ej_env* h) {
     }
 }
 
+bool misaligned16(const void* p) { return ((uintptr_t)p & 15u) != 0; }
+bool misaligned4(const void* p) { return ((uintptr_t)p & 3u) != 0; }
+
 int launch_step(ej_env* h, const StepIO& io) {
     const DevCfg& c = h->c;
+    // the kernels move observation tiles with 16-byte bulk copies and everything else with 32-bit accesses
+    if (misaligned16(io.obs) || misaligned16(io.obs_priv) || misaligned16(io.obs_shared) || misaligned16(io.obs_gov))
+        return fail(h, EJ_ERR_PARAM, "bad field: %s", "observation pointer (must be 16-byte aligned)");
+    if (misaligned4(io.actions) || misaligned4(io.gov_actions) || misaligned4(io.rew) || misaligned4(io.actions_out) || misaligned4(io.gov_out))
+        return fail(h, EJ_ERR_PARAM, "bad field: %s", "actions / rewards pointer (must be 4-byte aligned)");
     (io.obs_priv ? h->step_fn_fx : h->step_fn)<<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, io);
     h->launches++;
     EJ_CUDA(h, cudaGetLastError(), "ej_step_kernel launch");
     return EJ_OK;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize belongs to the kernel FUNCTION, and handles of different shapes
+// share functions (the generic step kernel, reset, observe, the policy kernel): the attribute is only ever
+// raised, to the largest request any live or past handle of this process has made for that function.
+std::mutex g_smem_mu;
+std::map<std::pair<int, const void*>, int> g_smem_max;  // (device, function) -> bytes
+cudaError_t raise_smem_attr(const void* fn, int bytes) {
+    std::lock_guard<std::mutex> lock(g_smem_mu);
+    int dev = 0;
+    cudaGetDevice(&dev);
+    int& cur = g_smem_max[std::make_pair(dev, fn)];
+    if (bytes <= cur) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) cur = bytes;
+    return e;
 }
 
 int set_smem_attr(ej_env* h) {
@@ -230,10 +257,10 @@ int set_smem_attr(ej_env* h) {
     return for_variant(c.Npad, c.N4, [&](auto mt, auto ns) {
         constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
         select_step_kernel<MT, NS>(h);
-        EJ_CUDA(h, cudaFuncSetAttribute(h->step_fn, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step)");
-        if (h->step_fn_fx) EJ_CUDA(h, cudaFuncSetAttribute(h->step_fn_fx, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (step, factored)");
-        EJ_CUDA(h, cudaFuncSetAttribute(ej_observe_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (observe)");
-        EJ_CUDA(h, cudaFuncSetAttribute(ej_reset_kernel<MT, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize, c.smem_bytes), "smem attr (reset)");
+        EJ_CUDA(h, raise_smem_attr((const void*)h->step_fn, c.smem_bytes), "smem attr (step)");
+        if (h->step_fn_fx) EJ_CUDA(h, raise_smem_attr((const void*)h->step_fn_fx, c.smem_bytes), "smem attr (step, factored)");
+        EJ_CUDA(h, raise_smem_attr((const void*)ej_observe_kernel<MT, NS>, c.smem_bytes), "smem attr (observe)");
+        EJ_CUDA(h, raise_smem_attr((const void*)ej_reset_kernel<MT, NS>, c.smem_bytes), "smem attr (reset)");
         return EJ_OK;
     });
 }
@@ -510,6 +537,7 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     int rc = set_smem_attr(h);
     if (rc != EJ_OK) { memcpy(g_create_err, h->err, 256); delete h; return rc; }
     cudaError_t ce = cudaMalloc(&h->d_state, (size_t)E * c.blob_bytes);
+    if (ce == cudaSuccess) ce = cudaMemset(h->d_state, 0, (size_t)E * c.blob_bytes);
     if (ce == cudaSuccess) ce = cudaMalloc(&h->d_cdf, (size_t)c.A * 4);
     if (ce != cudaSuccess) {
         cudaGetLastError();
@@ -559,6 +587,7 @@ int ej_layout(const ej_env* h, ej_layout_info* o) {
     o->device_state_bytes = (size_t)c.blob_bytes;
     o->smem_bytes = (size_t)c.smem_bytes;
     o->threads_per_env = c.Npad;
+    o->D_priv = 3 * c.R + 4; o->D_shared = 5 * c.R + c.B + 2; o->D_shared_pad = (o->D_shared + 3) & ~3;
     return EJ_OK;
 }
 
@@ -581,6 +610,7 @@ int ej_reset(ej_env* h, uint64_t seed) {
 int ej_observe(ej_env* h, float* obs_out) {
     if (!h || !obs_out) return h ? fail(h, EJ_ERR_PARAM, "bad field: %s", "obs_out") : EJ_ERR_PARAM;
     if (!h->was_reset) return fail(h, EJ_ERR_STATE, "%s", "ej_observe before ej_reset / ej_set_state");
+    if (misaligned16(obs_out)) return fail(h, EJ_ERR_PARAM, "bad field: %s", "obs_out (must be 16-byte aligned)");
     const DevCfg& c = h->c;
     return for_variant(c.Npad, c.N4, [&](auto mt, auto ns) {
         constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
@@ -724,7 +754,7 @@ int ej_set_policy(ej_env* h, const ej_mlp* pop, const ej_mlp* gov) {
     if (rc != EJ_OK) return rc;
     const int sp = policy_smem_bytes(h->pop_net, c.D_pop), sg = policy_smem_bytes(h->gov_net, c.D_gov_pad);
     const int smem = sp > sg ? sp : sg;
-    EJ_CUDA(h, cudaFuncSetAttribute(ej_policy_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem), "smem attr (policy)");
+    EJ_CUDA(h, raise_smem_attr((const void*)ej_policy_kernel, smem), "smem attr (policy)");
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&h->n_sms, cudaDevAttrMultiProcessorCount, dev);
@@ -841,6 +871,9 @@ int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t*
     if (env_begin < 0 || env_count < 0 || env_begin + env_count > c.E) return fail(h, EJ_ERR_PARAM, "bad field: %s", "env range");
     const size_t W = state_words(c);
     if (!words || n_words < W * (size_t)env_count) return fail(h, EJ_ERR_PARAM, "bad field: %s", "words / n_words");
+    // the dump holds no Philox key and may cover only some envs: the handle must have been reset (with the seed
+    // of the run the dump comes from, if that run is to continue draw for draw)
+    if (!h->was_reset) return fail(h, EJ_ERR_STATE, "%s", "ej_set_state before ej_reset (reset with the original seed first)");
     const int N = c.N, R = c.R, B = c.B, P = c.P, cap = c.N * c.M, N4 = c.N4;
     std::vector<uint8_t> blobs((size_t)env_count * c.blob_bytes, 0);
     for (int k = 0; k < env_count; ++k) {
@@ -875,6 +908,7 @@ int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t*
         }
         for (int l = 0; l < c.n_levels; ++l) { head[l] = (uint16_t)NIL; tail[l] = (uint16_t)NIL; }
         cnt += (hd->t & 1) * c.n_levels;  // the buffer current at clock t
+        int best_bid = 0;  // of the resource whose bids were just read
         for (int b = 0; b < 2 * R; ++b) {
             const int n = w[q++];
             if (n < 0 || n > cap) return fail(h, EJ_ERR_PARAM, "bad field: %s", "words (book size)");
@@ -895,13 +929,16 @@ int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t*
                 else head[l] = (uint16_t)slot;
                 tail[l] = (uint16_t)slot;
                 cnt[l]++;
+                // a resting book is uncrossed (G13): the kernels size their matched-order lists by that
+                if ((b & 1) == 0) { if (o == 0 || price > best_bid) best_bid = price; }
+                else if (price <= best_bid) return fail(h, EJ_ERR_PARAM, "bad field: %s", "words (crossed book: best bid >= best ask)");
             }
+            if ((b & 1) == 0 && n == 0) best_bid = 0;
             q += 3 * (size_t)cap;
         }
     }
     EJ_CUDA(h, cudaStreamSynchronize(h->stream), "set_state sync");
     EJ_CUDA(h, cudaMemcpy(h->d_state + (size_t)env_begin * c.blob_bytes, blobs.data(), blobs.size(), cudaMemcpyHostToDevice), "set_state copy");
-    h->was_reset = true;
     return EJ_OK;
 }
 

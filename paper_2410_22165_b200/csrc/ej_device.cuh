@@ -1170,6 +1170,7 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
     double cf_pre = 0.0;
     int mode = 0, rows = 2;
     if (t >= c.T) {  // G28: finished env
+        __syncthreads();  // thread 0 has waited for the previous step's bulk reads of shrow / the staging tile
         if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
         if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
         if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);

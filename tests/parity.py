@@ -182,3 +182,64 @@ def check_dump_invariants(w, cfg, steps):
         both = (bb >= 0) & (ab >= 0)
         assert (bb[both] < ab[both]).all()
     return n_orders
+
+
+class OracleShards:
+    """The oracle on runs of consecutive global env ids, advanced by host threads (economies are independent and
+    keyed by their global id; ctypes releases the GIL while the C oracle steps).  Used by the full-size parity tests:
+    the oracle itself is unchanged, only many copies of it run side by side."""
+
+    def __init__(self, N, R, params, seed, runs, threads=None, per_shard=None):
+        import os
+        from concurrent.futures import ThreadPoolExecutor
+
+        self.N, self.R = N, R
+        self.runs = [(int(lo), int(n)) for lo, n in runs]
+        total = sum(n for _, n in self.runs)
+        self.threads = threads or max(1, min(os.cpu_count() or 1, 32))
+        per = per_shard or max(1, -(-total // (4 * self.threads)))
+        self.shards = []   # (first local index in the concatenated order, oracle env)
+        k = 0
+        base = int(params["env_id_base"])
+        for lo, n in self.runs:
+            for s in range(lo, lo + n, per):
+                cnt = min(per, lo + n - s)
+                o = oracle.OracleEnv(cnt, N, R, dict(params, env_id_base=base + s))
+                o.reset(seed)
+                self.shards.append((k, o))
+                k += cnt
+        self.n = k
+        self.ids = np.concatenate([np.arange(lo, lo + n) for lo, n in self.runs])
+        self.pool = ThreadPoolExecutor(self.threads)
+
+    def _map(self, fn):
+        return list(self.pool.map(fn, self.shards))
+
+    def state(self):
+        return np.concatenate(self._map(lambda s: s[1].get_state()))
+
+    def observe(self):
+        outs = self._map(lambda s: s[1].observe())
+        return np.concatenate([x[0] for x in outs]), np.concatenate([x[1] for x in outs])
+
+    def advance(self, steps, cdf=None, actions=None, gov_actions=None, keep=()):
+        """Step every env `steps` times with actions drawn from `cdf` (rollout-mode generator) or supplied as
+        [steps][n][N] / [steps][n][B] in the concatenated env order.  Returns {s: (acts, gov, pop, govobs, rew, done)}
+        for the step indices s in `keep` (observations are built only there)."""
+        keep = set(keep)
+
+        def work(sh):
+            k, o = sh
+            out = {}
+            for s in range(steps):
+                if actions is None:
+                    a, g = o.draw_actions(cdf)
+                else:
+                    a, g = actions[s][k:k + o.E], gov_actions[s][k:k + o.E]
+                pop, gv, rew, done = o.step(a, g, want_obs=s in keep)
+                if s in keep:
+                    out[s] = (a, g, pop, gv, rew, done)
+            return out
+
+        parts = self._map(work)
+        return {s: tuple(np.concatenate([p[s][j] for p in parts]) for j in range(6)) for s in keep}

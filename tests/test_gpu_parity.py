@@ -183,8 +183,9 @@ def test_normal_skill_init_and_section5_workload():
     # EJ_SKILL_NORMAL_CLIP at reset (bit-exact skills), then the section-5 presets through the persistent rollout
     for name, E in (("section5_r4", 5), ("section5_r12", 3)):
         cfg = inputs.configs()[name]
-        assert binding_A(cfg) == {4: 30, 12: 86}[cfg["R"]]
         pair = Pair(E, cfg["N"], cfg["R"], cfg["params"], 21)
+        assert pair.g.A == {4: 30, 12: 86}[cfg["R"]]                             # P:350, read from ej_layout
+        assert pair.g.noop_action == pair.g.A - 1 and pair.g.base_buy == cfg["R"] + 1 and pair.g.D_pop == 6 + 8 * cfg["R"] + 3
         compare_state(pair.g_state(), pair.o_state(), name + " reset")
         sk = np.concatenate([oracle_skills(w) for w in pair.g_state()])
         assert sk.min() >= 0.0 and sk.max() <= 5.0 and 0.9 < sk.mean() < 1.25 and (sk == 0.0).mean() > 0.1
@@ -193,11 +194,6 @@ def test_normal_skill_init_and_section5_workload():
     _rollout_vs_oracle("section5_r12", 2048, 40, env_ids=[0, 2047], ring=2)
     run_episode("tiny_dense", 4, 50, skill_init=inputs.SKILL_NORMAL_CLIP, skill_mean=2.0, skill_std=0.5, skill_clip_lo=0.25,
                 skill_clip_hi=3.0)
-
-
-def binding_A(cfg):
-    p = cfg["params"]
-    return inputs.num_actions(cfg["R"], len(p["prices"]), p["craft_mode"], p["allow_noop"])
 
 
 def oracle_skills(words):

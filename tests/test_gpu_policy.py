@@ -187,56 +187,59 @@ def test_policy_error_paths():
         env.policy_act(obs)
 
 
-def test_full_size_config5_sampled_envs():
+def test_full_size_config5_envs_0_to_127_teacher_forced():
     """BASELINE.json configs[4] at full size (E=2048, N=100, R=3) in the launch configuration bench.py
-    times (policy kernel + step kernel per step, output rings); sampled envs are teacher-forced through
-    1-env oracles keyed by global env id, their logits and samples re-checked."""
+    times (policy-driven ej_rollout with output rings), 200 steps; envs 0..127 are teacher-forced
+    through the oracle sharded over the host cores: every transition, observation and reward of every step is
+    compared, the logits are recomputed in binary64 every 8th step and the samples re-checked on a sample."""
     import torch
+    from parity import OracleShards
 
     cfg = inputs.configs()["config5_policy"]
-    N, R, E, T, depth = cfg["N"], cfg["R"], cfg["E"], 24, 24
-    ids = [0, 1, 127, 128, 1023, 2046, 2047]
-    pair = Pair(E, N, R, cfg["params"], cfg["seed"], env_ids=ids)
-    g = pair.g
+    N, R, E, T, chunk = cfg["N"], cfg["R"], cfg["E"], 200, 40
+    n_ids = 128
+    g = binding.Env(E, N, R, cfg["params"])
+    g.reset(cfg["seed"])
+    o = OracleShards(N, R, cfg["params"], cfg["seed"], [(0, n_ids)])
     pop, gov = inputs.policy_weights(cfg, seed=cfg["seed"])   # the weights bench.py installs
     g.set_policy(pop, gov)
-    obs_ring, rew_ring, done_ring = g.new_obs(depth), g.new_rew(depth), g.new_done(depth)
-    act_ring = torch.zeros((depth, E, N), dtype=torch.int32, device="cuda")
-    gov_ring = torch.zeros((depth, E, g.B), dtype=torch.int32, device="cuda")
-    pl_ring = torch.zeros((depth, E * N, g.A), dtype=torch.float32, device="cuda")
-    gl_ring = torch.zeros((depth, E, g.B * g.L), dtype=torch.float32, device="cuda")
-    g.rollout(T, ring_depth=depth, obs_ring=obs_ring, rew_ring=rew_ring, done_ring=done_ring, actions_ring=act_ring,
-              gov_actions_ring=gov_ring, pop_logits_ring=pl_ring, gov_logits_ring=gl_ring)
-    torch.cuda.synchronize()
-    pop_obs, gov_obs = g.split_obs(obs_ring)
-    pop_obs, gov_obs = pop_obs[:, ids].cpu().numpy(), gov_obs[:, ids].cpu().numpy()
-    rew, done = rew_ring[:, ids].cpu().numpy(), done_ring[:, ids].cpu().numpy()
-    a_out, g_out = act_ring[:, ids].cpu().numpy(), gov_ring[:, ids].cpu().numpy()
-    pl = pl_ring.reshape(depth, E, N, g.A)[:, ids].cpu().numpy()
-    gl = gl_ring[:, ids].cpu().numpy()
-    outs = [o.observe() for o in pair.o]
-    o_pop, o_gov = np.concatenate([x[0] for x in outs]), np.concatenate([x[1] for x in outs])
+    obs_ring, rew_ring, done_ring = g.new_obs(chunk), g.new_rew(chunk), g.new_done(chunk)
+    act_ring = torch.zeros((chunk, E, N), dtype=torch.int32, device="cuda")
+    gov_ring = torch.zeros((chunk, E, g.B), dtype=torch.int32, device="cuda")
+    pl_ring = torch.zeros((chunk, E * N, g.A), dtype=torch.float32, device="cuda")
+    gl_ring = torch.zeros((chunk, E, g.B * g.L), dtype=torch.float32, device="cuda")
+    o_pop, o_gov = o.observe()
     amb = tot = 0
-    for t in range(T):
-        ol_pop = OP.mlp_logits(pop, o_pop.reshape(len(ids) * N, -1)).reshape(len(ids), N, -1)
-        ol_gov = OP.mlp_logits(gov, o_gov.reshape(len(ids), -1))
-        check_logits(pl[t], ol_pop, "t=%d population logits" % t)
-        check_logits(gl[t], ol_gov, "t=%d government logits" % t)
-        if t % 6 == 0 or t == T - 1:
-            a_, t_ = check_samples(cfg["seed"], ids, N, [t] * len(ids), ol_pop, ol_gov, a_out[t], g_out[t], g.B, g.L, "t=%d" % t)
-            amb, tot = amb + a_, tot + t_
-        o_pop, o_gov, o_rew, o_done = _teacher_step(pair, a_out[t], g_out[t])
-        compare_outputs(g, pop_obs[t], gov_obs[t], rew[t], done[t], o_pop, o_gov, o_rew, o_done, "config5 full size t=%d" % t)
-    compare_state(pair.g_state(), pair.o_state(), "config5 full size final state")
-    assert amb <= max(2, 0.01 * tot)
+    worst = 0.0
+    for c0 in range(0, T, chunk):
+        g.rollout(chunk, ring_depth=chunk, obs_ring=obs_ring, rew_ring=rew_ring, done_ring=done_ring, actions_ring=act_ring,
+                  gov_actions_ring=gov_ring, pop_logits_ring=pl_ring, gov_logits_ring=gl_ring)
+        torch.cuda.synchronize()
+        pop_obs, gov_obs = g.split_obs(obs_ring)
+        pop_obs, gov_obs = pop_obs[:, :n_ids].cpu().numpy(), gov_obs[:, :n_ids].cpu().numpy()
+        rew, done = rew_ring[:, :n_ids].cpu().numpy(), done_ring[:, :n_ids].cpu().numpy()
+        a_out, g_out = act_ring[:, :n_ids].cpu().numpy(), gov_ring[:, :n_ids].cpu().numpy()
+        # teacher forcing: the oracle envs consume the GPU's actions; every step's outputs are kept
+        outs = o.advance(chunk, actions=a_out, gov_actions=g_out, keep=range(chunk))
+        for s in range(chunk):
+            t = c0 + s
+            if t % 8 == 0:   # logits from the oracle's own (bit-identical) observation of the state before step t
+                ol_pop = OP.mlp_logits(pop, o_pop.reshape(n_ids * N, -1)).reshape(n_ids, N, -1)
+                ol_gov = OP.mlp_logits(gov, o_gov.reshape(n_ids, -1))
+                pl = pl_ring[s].reshape(E, N, g.A)[:n_ids].cpu().numpy()
+                gl = gl_ring[s][:n_ids].cpu().numpy()
+                worst = max(worst, check_logits(pl, ol_pop, "t=%d population logits" % t), check_logits(gl, ol_gov, "t=%d government logits" % t))
+                if t % 40 == 0:
+                    sel = list(range(0, n_ids, 9))
+                    a_, t_ = check_samples(cfg["seed"], sel, N, [t] * len(sel), ol_pop[sel], ol_gov[sel], a_out[s][sel], g_out[s][sel],
+                                           g.B, g.L, "t=%d" % t)
+                    amb, tot = amb + a_, tot + t_
+            _, _, o_pop, o_gov, o_rew, o_done = outs[s]
+            compare_outputs(g, pop_obs[s], gov_obs[s], rew[s], done[s], o_pop, o_gov, o_rew, o_done, "config5 full size t=%d" % t)
+        compare_state(g.get_state(0, n_ids), o.state(), "config5 full size state at t=%d" % (c0 + chunk))
+    assert amb <= max(2, 0.01 * tot) and worst < 5e-3
     an = act_ring.cpu().numpy()
     assert an.min() >= 0 and an.max() < g.A
-
-
-def _teacher_step(pair, acts_sel, gov_sel):
-    """Step the 1-env oracles of a sampled-env Pair with already-selected action rows."""
-    outs = [o.step(acts_sel[k:k + 1], gov_sel[k:k + 1]) for k, o in enumerate(pair.o)]
-    return tuple(np.concatenate([x[j] for x in outs]) for j in range(4))
 
 
 def test_masked_policy_rollout_teacher_forced():

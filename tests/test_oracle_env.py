@@ -192,6 +192,100 @@ def test_observation_layout_and_market_stats(small_params):
     assert g[3 * 4 + 2] == np.median(s["inv"][:, 1].astype(np.float32)) * f32(0.1)
 
 
+def test_government_row_hand_values(small_params):
+    """Every entry of the government row (Fig.1, "mean, standard deviation, and median"; G26: metric
+    order coin, labor, income, inv[r]; population std; each statistic times the metric's scale; then rates and
+    the two timers, G27) on a 4-agent state built by scripted actions whose coin, labor, income and inventories
+    all differ.  Scales are powers of two so that the hand values are exact in binary32."""
+    import math
+
+    a = Act(2, 10)
+    p = dict(small_params, starting_coin=15.0, craft_units=1, craft_distinct=1, labor_craft=1.0, labor_trade=0.25,
+             obs_scale_coin=0.5, obs_scale_labor=0.25, obs_scale_count=2.0, obs_scale_price=0.125)
+    env = make(1, 4, 2, p)
+    env.set_agent(0, 0, 15.0, inv=[3, 1], SC=1.25)
+    env.set_agent(0, 1, 15.0, inv=[0, 5], SC=0.0)
+    env.set_agent(0, 2, 15.0, inv=[7, 0], SC=0.0)
+    env.set_agent(0, 3, 15.0, inv=[4, 2], SC=0.5)
+    rates = [np.float32(0.1), np.float32(0.3), np.float32(0.5)]
+    env.set_rates(0, rates)
+    # step A: 0 crafts (pay 12.5), 1 bids 4 for r0, 2 idles, 3 crafts (pay 5)
+    env.step([[a.craft(), a.buy(0, 3), a.noop, a.craft()]], gov0(env))
+    # step B: 0 crafts again, 3 asks 3 for r0 -> trades with 1's bid at the later order's price 3 (P:432-433)
+    _, g, _, _ = env.step([[a.craft(), a.noop, a.noop, a.sell(0, 2)]], gov0(env))
+    s = st(env)
+    assert s["coin"].tolist() == [40.0, 12.0, 15.0, 23.0]
+    assert s["labor"].tolist() == [2.0, 0.25, 0.0, 1.25]
+    assert s["income"].tolist() == [25.0, 0.0, 0.0, 8.0]
+    assert s["inv"].tolist() == [[1, 1], [1, 5], [7, 0], [2, 2]]
+    g = g[0]
+    assert g.shape == (3 * (3 + 2) + 3 + 2,)
+    f32 = np.float32
+    want = [
+        # coin, scale 0.5: mean 22.5, variance 473/4, median (15 + 23) / 2
+        f32(22.5 * 0.5), f32(math.sqrt(118.25) * 0.5), f32(19.0 * 0.5),
+        # labor, scale 0.25: mean 0.875, variance 2.5625/4, median (0.25 + 1.25) / 2
+        f32(0.875 * 0.25), f32(math.sqrt(0.640625) * 0.25), f32(0.75 * 0.25),
+        # income, scale 0.5 (a coin amount): mean 8.25, variance 416.75/4, median (0 + 8) / 2
+        f32(8.25 * 0.5), f32(math.sqrt(104.1875) * 0.5), f32(4.0 * 0.5),
+        # inventory of resource 0, scale 2: [1, 1, 7, 2]
+        f32(2.75 * 2.0), f32(math.sqrt(6.1875) * 2.0), f32(1.5 * 2.0),
+        # inventory of resource 1, scale 2: [1, 5, 0, 2]
+        f32(2.0 * 2.0), f32(math.sqrt(3.5) * 2.0), f32(1.5 * 2.0),
+    ]
+    for k, w in enumerate(want):
+        if k % 3 == 1:                                             # std: binary64 sqrt, one rounding to binary32
+            assert abs(float(g[k]) - float(w)) <= 1.2e-7 * float(w), (k, g[k], w)
+        else:
+            assert g[k] == w, (k, g[k], w)
+    assert g[15:18].tolist() == [float(r) for r in rates]          # the rates in force (set_rates), not the action
+    assert g[18] == f32(2) / f32(10) and g[19] == f32(2) / f32(50)  # timers of t' = 2 (G27)
+    # three agents (odd N): the median is the middle value, not a midpoint
+    env3 = make(1, 3, 2, p)
+    for i, (c, inv) in enumerate(((3.0, [9, 0]), (1.0, [2, 4]), (8.0, [5, 1]))):
+        env3.set_agent(0, i, c, inv=inv, SC=0.0)
+    _, g3 = env3.observe()
+    assert g3[0, 2] == f32(3.0 * 0.5) and g3[0, 11] == f32(5 * 2.0) and g3[0, 14] == f32(1 * 2.0)
+    assert g3[0, 0] == f32(4.0 * 0.5) and g3[0, 18] == 0.0 and g3[0, 19] == 0.0
+
+
+def test_government_level_draws_recomputed_from_philox():
+    """Rollout-mode government levels (G30): bracket b takes word b % 4 of Philox(ctr = (global env, N, t,
+    stream 1 + b / 4), key = seed) and level = (x * L) >> 32.  Recomputed here from orc_philox4x32_10 (itself
+    pinned by the Random123 known answers) for B = 7: two counter blocks, every word used once."""
+    import ctypes as C
+
+    L = oracle.lib()
+
+    def philox(ctr, key):
+        c, k, o = (C.c_uint32 * 4)(*ctr), (C.c_uint32 * 2)(*key), (C.c_uint32 * 4)()
+        L.orc_philox4x32_10(c, k, o)
+        return list(o)
+
+    cfg = inputs.configs()["config2_paper"]
+    seed = (0x9E3779B9 << 32) | 0x12345678                          # both key words matter
+    N, nl = cfg["N"], len(cfg["params"]["rate_table"])
+    env = make(3, N, 2, dict(cfg["params"], env_id_base=40), seed=seed)
+    assert env.B == 7 and nl == 21
+    cdf = inputs.action_cdf(cfg)
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    seen = set()
+    for t in range(6):
+        acts, gov = env.draw_actions(cdf)
+        for e in range(3):
+            blocks = [philox([40 + e, N, t, 1], key), philox([40 + e, N, t, 2], key)]
+            want = [(blocks[b // 4][b % 4] * nl) >> 32 for b in range(7)]
+            assert gov[e].tolist() == want, (t, e)
+            seen.update(want)
+            # population action of agent i: smallest a with x0 < cdf[a] on stream 0 (word 0)
+            for i in (0, 57, N - 1):
+                x0 = philox([40 + e, i, t, 0], key)[0]
+                assert acts[e, i] == int(np.searchsorted(cdf.astype(np.uint64), x0, side="right")) or \
+                    (acts[e, i] == env.A - 1 and x0 >= cdf[-2])
+        env.step(acts, gov, want_obs=False)
+    assert len(seen) > 10                                          # the words differ: not one word for every bracket
+
+
 def test_reward_is_utility_delta_and_gov_reward(small_params):
     a = Act(1, 10)
     p = dict(small_params, starting_coin=15.0, craft_units=1, craft_distinct=1)
@@ -466,3 +560,38 @@ def test_dump_invariant_checker_accepts_the_oracle_and_rejects_a_broken_dump(nam
     bad[0, 13 + B + cfg["R"] + 1] += 1          # agent 0's escrowed coin no longer equals its live bids
     with pytest.raises(AssertionError):
         check_dump_invariants(bad, cfg, steps)
+
+
+def test_sharded_oracle_helper_equals_one_oracle():
+    """tests/parity.py's OracleShards (many copies of the oracle on host threads, used by the full-size GPU parity
+    tests) returns exactly what one oracle over the same global env ids returns."""
+    import sys, os
+    sys.path.insert(0, os.path.dirname(__file__))
+    from parity import OracleShards
+
+    cfg = inputs.configs()["config2_paper"]
+    params = dict(cfg["params"], env_id_base=5)
+    cdf = inputs.action_cdf(cfg)
+    runs = [(0, 5), (9, 3)]
+    sh = OracleShards(cfg["N"], cfg["R"], params, 11, runs, threads=3, per_shard=2)
+    ones = [make(n, cfg["N"], cfg["R"], dict(params, env_id_base=5 + lo), seed=11) for lo, n in runs]
+    assert sh.n == 8 and sh.ids.tolist() == [0, 1, 2, 3, 4, 9, 10, 11]
+    outs = sh.advance(12, cdf=cdf, keep=[3, 11])
+    for s in range(12):
+        for k, o in enumerate(ones):
+            a, g = o.draw_actions(cdf)
+            res = o.step(a, g, want_obs=s in (3, 11))
+            if s in (3, 11):
+                lo = 0 if k == 0 else 5
+                for j, ref in enumerate((a, g) + tuple(res)):
+                    assert np.array_equal(outs[s][j][lo:lo + o.E], ref), (s, k, j)
+    assert np.array_equal(sh.state(), np.concatenate([o.get_state() for o in ones]))
+    # supplied actions, every step kept
+    acts, gov = inputs.action_stream(cfg, 4, seed=2, E=8)
+    outs = sh.advance(4, actions=acts, gov_actions=gov, keep=range(4))
+    for s in range(4):
+        for k, o in enumerate(ones):
+            lo = 0 if k == 0 else 5
+            res = o.step(acts[s][lo:lo + o.E], gov[s][lo:lo + o.E])
+            assert np.array_equal(outs[s][4][lo:lo + o.E], res[2])
+    assert np.array_equal(sh.state(), np.concatenate([o.get_state() for o in ones]))
