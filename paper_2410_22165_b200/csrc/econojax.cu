@@ -133,13 +133,13 @@ void build_layout(DevCfg& c) {
     c.o_scratch1 = o;
     c.o_ahead = take(nl * 4);
     c.o_cdf = take(c.A * 4);
-    if (c.K) {  // book-cap path: compaction buckets
-        c.o_bucket = take(NP * 8);
-        c.o_sorted = take(NP * 4);
-        c.o_gcnt = take(c.n_groups * 4);
-        c.o_goff = take(c.n_groups * 4);
+    if (c.K) {  // book-cap path: key bins of this step's candidates, per book and per level
+        c.o_bbh = take(2 * R * BOOK_BINS * 4);
+        c.o_bbc = take(2 * R * BOOK_BINS * 4);
+        c.o_lbh = take(nl * LEVEL_BINS * 4);
+        c.o_lmask = take(nl * 4);
     } else {
-        c.o_bucket = c.o_sorted = c.o_gcnt = c.o_goff = c.o_ahead;  // unused
+        c.o_bbh = c.o_bbc = c.o_lbh = c.o_lmask = c.o_ahead;  // unused
     }
     // staging tile of the population observation rows (not zeroed); the matched-order lists
     // mb | ma alias its head (written after the previous step's bulk store has been read,

@@ -30,6 +30,9 @@
 namespace {
 
 constexpr uint32_t NIL = 0xFFFFu;      // null slot of the order pool
+// Book-cap path: a step's candidates are binned by the top bits of their arrival key (a uniform Philox word, G11):
+// 256 bins per book give the rank of a candidate on its book, 32 bins per level its neighbours on its level.
+constexpr int BOOK_BINS = 256, BOOK_BIN_SHIFT = 24, LEVEL_BINS = 32, LEVEL_BIN_SHIFT = 27;
 constexpr uint32_t FULL = 0xffffffffu;
 
 struct EnvHdr {
@@ -41,6 +44,8 @@ struct EnvHdr {
     int32_t pad1;
     float rates[EJ_MAX_BRACKETS];
     int32_t last_price[EJ_MAX_RESOURCES];
+    uint32_t coin_spl[32];  // last step's coin order statistics of rank (b+1) N / NW (float bits): bucket bounds of the
+                            // block-wide coin sort of large populations; hints like med_prev, not state
 };
 static_assert(sizeof(EnvHdr) % 16 == 0, "EnvHdr must keep 16-byte alignment");
 
@@ -66,8 +71,9 @@ struct DevCfg {
     int o_head, o_tail, o_cnt, o_pool, blob_bytes;
     int o_blob, o_scratch1;  // absolute: blob start (= Lay<Npad>::blob), first byte after the blob
     // scratch section offsets (bytes from the shared-memory base; all after the blob)
-    int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma, o_bucket, o_sorted;
-    int o_gcnt, o_goff, o_resq, o_shrow, o_govrow, o_misc, o_cdf, o_coltab, o_stage;
+    int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma;
+    int o_bbh, o_bbc, o_lbh, o_lmask;  // book-cap path (K > 0): arrival bins per book and per level
+    int o_resq, o_shrow, o_govrow, o_misc, o_cdf, o_coltab, o_stage;
     int smem_bytes;
     unsigned long long gov_obs_offset, obs_floats;
 };
@@ -109,7 +115,13 @@ struct Lay {
     static constexpr int govrow = shrow + shrow_cap * 4;
     static constexpr int govrow_cap = 80;  // >= ceil4(3 (3 + 16) + 16 + 2)
     static constexpr int misc = govrow + govrow_cap * 4;       // u64 [2]: tax pool
-    static constexpr int blob = misc + 16;
+    // block-wide coin sort (CTAs of 8 warps and more): one bucket of coin keys per warp
+    static constexpr bool bucketed = NP >= 416;                 // NP is the array stride (13/16 of the CTA size or the CTA size): CTAs of 512 and 1024 threads
+    static constexpr int bk_cap = 128;                          // keys per bucket (4 per lane at most)
+    static constexpr int bk_cnt = misc + 16;                    // u32 [32] bucket sizes, [32] = overflow flag, [33..34] medians
+    static constexpr int bk_part = bk_cnt + (bucketed ? 36 * 4 : 0);  // f64 [32][3]: gini, sum, sum of squares per bucket
+    static constexpr int bk_keys = bk_part + (bucketed ? 32 * 3 * 8 : 0);
+    static constexpr int blob = bk_keys + (bucketed ? 32 * bk_cap * 4 : 0);
     // blob sections (byte offsets relative to the blob)
     static constexpr int coin = (int)sizeof(EnvHdr);
     static constexpr int labor = coin + NP * 4;
@@ -180,13 +192,17 @@ struct Sm {
     __device__ __forceinline__ float* shrow() const { return at<float>(L::shrow); }
     __device__ __forceinline__ float* govrow() const { return at<float>(L::govrow); }
     __device__ __forceinline__ unsigned long long* misc() const { return at<unsigned long long>(L::misc); }  // [0] tax pool in 2^-20 coin
+    __device__ __forceinline__ uint32_t* bk_cnt() const { return at<uint32_t>(L::bk_cnt); }
+    __device__ __forceinline__ double* bk_part() const { return at<double>(L::bk_part); }
+    __device__ __forceinline__ uint32_t* bk_keys() const { return at<uint32_t>(L::bk_keys); }
     __device__ __forceinline__ uint32_t* ahead() const { return at<uint32_t>(ST ? S::ahead : c.o_ahead); }
     __device__ __forceinline__ uint32_t* mb() const { return at<uint32_t>(ST ? S::mb : c.o_mb); }
     __device__ __forceinline__ uint32_t* ma() const { return at<uint32_t>(ST ? S::ma : c.o_ma); }
-    __device__ __forceinline__ unsigned long long* bucket() const { return at<unsigned long long>(c.o_bucket); }
-    __device__ __forceinline__ uint32_t* sorted() const { return at<uint32_t>(c.o_sorted); }
-    __device__ __forceinline__ int* gcnt() const { return at<int>(c.o_gcnt); }
-    __device__ __forceinline__ int* goff() const { return at<int>(c.o_goff); }
+    // book-cap path: this step's candidates binned by arrival key (G11, G15)
+    __device__ __forceinline__ uint32_t* bbh() const { return at<uint32_t>(c.o_bbh); }    // [2R][BOOK_BINS] chain heads
+    __device__ __forceinline__ uint32_t* bbc() const { return at<uint32_t>(c.o_bbc); }    // [2R][BOOK_BINS] counts -> exclusive prefix
+    __device__ __forceinline__ uint32_t* lbh() const { return at<uint32_t>(c.o_lbh); }    // [levels][LEVEL_BINS] chain heads
+    __device__ __forceinline__ uint32_t* lmask() const { return at<uint32_t>(c.o_lmask); }  // [levels] occupied level bins
     __device__ __forceinline__ uint32_t* cdf() const { return at<uint32_t>(ST ? S::cdf : c.o_cdf); }
     __device__ __forceinline__ float* stage() const { return at<float>(ST ? S::stage : c.o_stage); }
     __device__ __forceinline__ uint32_t* coltab() const { return at<uint32_t>(c.o_coltab); }
@@ -471,6 +487,13 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const SM& m, int k
         lo = warp_pick<EPL>(x, r0);
         hi = warp_pick<EPL>(x, r1);
         if (k != 0 && lane == 0) m.hdr()->med_prev[k - 1] = __float_as_uint(lo);
+        if (k == 0 && SM::L::bucketed) {  // EPL = warps of the CTA: renew the bucket bounds of the block-wide sort
+#pragma unroll 1
+            for (int b = 0; b + 1 < EPL; ++b) {
+                const float v = warp_pick<EPL>(x, ((b + 1) * N) / EPL);
+                if (lane == 0) m.hdr()->coin_spl[b] = __float_as_uint(v);
+            }
+        }
         if (k == 0 && mode != 2) {
             // sum_i sum_j |c_i - c_j| = 2 sum_k (2k - N + 1) c_(k)  =>  gini * prod = gn / N   (G23)
             double g = 0.0;
@@ -541,6 +564,93 @@ __device__ __forceinline__ void int_metric_stats(const DevCfg& c, const SM& m, i
         if (lane == 0) m.hdr()->med_prev[2 + r] = klo;
     }
     if (lane == 0) gov_triple<NS, NT>(c, m, 3 + r, mean, var, (float)(int)klo, (float)(int)khi, c.s_count);
+}
+
+// ---- block-wide coin statistics of large populations (CTAs of 512 / 1024 threads) ----
+// The coin metric needs the sorted order (median, and gini in its sorted-rank form, G23).  One warp sorting 1024
+// values in registers was the longest branch of the N = 1000 step (profiles/r2a: 26 % of the stall samples on the
+// barrier that waits for it).  Here every warp sorts one BUCKET of coin values: bucket b holds the values in
+// [spl[b-1], spl[b]), the bounds being last step's order statistics of rank (b+1) N / NW (coins drift slowly, so the
+// buckets stay near N / NW values); the rank of a value = sizes of the lower buckets + its place in its bucket.
+// Exact for any bounds; if a bucket overflows (start of an episode, a tax redistribution, many equal coins) the
+// step falls back to the single-warp sort, which also renews the bounds.
+
+// Thread `tid` files its agent's final coin of this step; called before the barrier that ends the state update.
+template <int NPAD, class SM>
+__device__ __forceinline__ void coin_bucket_fill(const SM& m, int tid, bool act) {
+    constexpr int NW = NPAD / 32, CAP = SM::L::bk_cap;
+    if (!act) return;
+    const uint32_t key = __float_as_uint(m.coin()[tid]);
+    int lo = 0, hi = NW - 1;  // bucket = number of bounds <= key
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (key < m.hdr()->coin_spl[mid]) hi = mid;
+        else lo = mid + 1;
+    }
+    const uint32_t pos = atomicAdd(&m.bk_cnt()[lo], 1u);
+    if (pos < (uint32_t)CAP && !(key >> 31)) m.bk_keys()[lo * CAP + (int)pos] = key;
+    else m.bk_cnt()[32] = 1u;  // overflow (or a negative value): fall back
+}
+
+// Warp `warp` sorts its bucket (n <= 32 EPL values, blocked layout) and leaves its share of gini, sum and sum of
+// squares; the warp that holds a wanted rank writes that order statistic (medians, next step's bounds).
+template <int EPL, int NPAD, class SM>
+__device__ __forceinline__ void coin_bucket_sort(const SM& m, int warp, int lane, int n, int off, int N) {
+    constexpr int NW = NPAD / 32, CAP = SM::L::bk_cap;
+    float x[EPL];
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) {
+        const int idx = lane * EPL + q;
+        x[q] = idx < n ? __uint_as_float(m.bk_keys()[warp * CAP + idx]) : INFINITY;
+    }
+    warp_sort<EPL>(x, lane);
+    double g = 0.0, s1 = 0.0, s2 = 0.0;
+#pragma unroll
+    for (int q = 0; q < EPL; ++q) {
+        const int idx = lane * EPL + q;
+        const double v = idx < n ? (double)x[q] : 0.0;
+        g += (double)(2 * (off + idx) - N + 1) * v;  // sum_k (2k - N + 1) c_(k)  (G23)
+        s1 += v;
+        s2 += v * v;
+    }
+    g = warp_sum(g); s1 = warp_sum(s1); s2 = warp_sum(s2);
+    if (lane == 0) { m.bk_part()[warp * 3 + 0] = g; m.bk_part()[warp * 3 + 1] = s1; m.bk_part()[warp * 3 + 2] = s2; }
+    // order statistics held by this bucket: lane b < NW - 1 looks for the bound of rank (b+1) N / NW, lanes 30 / 31
+    // ... the two median ranks are handled below (warp-uniform picks)
+    {
+        const int want = lane < NW - 1 ? ((lane + 1) * N) / NW - off : -1;
+        const bool mine = want >= 0 && want < n;
+        const int src = mine ? want : 0;
+        float v = __shfl_sync(FULL, x[0], src / EPL);
+#pragma unroll
+        for (int q = 1; q < EPL; ++q) {
+            const float y = __shfl_sync(FULL, x[q], src / EPL);
+            v = (src % EPL) == q ? y : v;
+        }
+        if (mine) m.hdr()->coin_spl[lane] = __float_as_uint(v);
+    }
+    const int r0 = (N >= 2 ? (N >> 1) - 1 : 0) - off, r1 = (N >> 1) - off;
+    if (r0 >= 0 && r0 < n) { const float v = warp_pick<EPL>(x, r0); if (lane == 0) m.bk_cnt()[33] = __float_as_uint(v); }
+    if (r1 >= 0 && r1 < n) { const float v = warp_pick<EPL>(x, r1); if (lane == 0) m.bk_cnt()[34] = __float_as_uint(v); }
+}
+
+// All warps: sort the own bucket.  Returns false (for every thread) if the buckets overflowed.
+template <int NPAD, class SM>
+__device__ __forceinline__ bool coin_bucket_stats(const SM& m, int warp, int lane, int N) {
+    constexpr int NW = NPAD / 32;
+    if (m.bk_cnt()[32]) return false;
+    const int mine = lane < NW ? (int)m.bk_cnt()[lane] : 0;
+    int incl = mine;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(FULL, incl, o);
+        if (lane >= o) incl += y;
+    }
+    const int n = __shfl_sync(FULL, mine, warp), off = __shfl_sync(FULL, incl - mine, warp);
+    if (n <= 32) coin_bucket_sort<1, NPAD>(m, warp, lane, n, off, N);
+    else if (n <= 64) coin_bucket_sort<2, NPAD>(m, warp, lane, n, off, N);
+    else coin_bucket_sort<4, NPAD>(m, warp, lane, n, off, N);
+    return true;
 }
 
 // Shared tail of the population rows: market statistics of the post-step books.
@@ -631,14 +741,48 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
 
     // ---- government statistics: metric k is owned by one warp (floats from warp 0 up, integer
     // metrics from the last warp down) ----
+    constexpr bool BKT = SM::L::bucketed;  // coin: every warp sorts one bucket (filled before the caller's barrier)
+    bool bk_ok = false;
+    if (BKT) bk_ok = coin_bucket_stats<NPAD>(m, warp, lane, N);
 #pragma unroll 1
-    for (int k = warp; k < 3; k += NW) metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
+    for (int k = warp; k < 3; k += NW)
+        if (!(BKT && k == 0)) metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
 #pragma unroll 1
     for (int r = NW - 1 - warp; r < R; r += NW) int_metric_stats<EPL, NS, NT>(c, m, r, lane);
     if (tid < B + 2) m.govrow()[3 * n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
 
     if (any_obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
+
+    if (BKT && warp == 0) {  // coin triple and welfare from the buckets' shares (or the single-warp sort)
+        if (bk_ok) {
+            double g = 0.0, s1 = 0.0, s2 = 0.0;
+            if (lane < NW) { g = m.bk_part()[lane * 3 + 0]; s1 = m.bk_part()[lane * 3 + 1]; s2 = m.bk_part()[lane * 3 + 2]; }
+            g = warp_sum(g); s1 = warp_sum(s1); s2 = warp_sum(s2);
+            if (lane == 0) {
+                const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
+                const double mean = s1 * inv_n;
+                double var = (s2 - s1 * mean) * inv_n;  // population variance from sum and sum of squares (binary64)
+                if (var < 0.0) var = 0.0;
+                gov_triple<NS, NT>(c, m, 0, mean, var, __uint_as_float(m.bk_cnt()[33]), __uint_as_float(m.bk_cnt()[34]), c.s_coin);
+                if (mode != 2) {
+                    const double ug = s1 - (double)c.omega * (g * inv_n);  // Eq.3-5 as in metric_stats
+                    if (mode == 0) {
+                        if (rew) rew[(uint32_t)(e * (N + 1) + N)] = (float)(ug - m.hdr()->u_g_prev);
+                        m.hdr()->u_g_prev = ug;
+                    } else if (rew) {
+                        rew[(uint32_t)(e * (N + 1) + N)] = 0.0f;
+                    }
+                }
+            }
+        } else {
+            metric_stats<EPL, NS, NT>(c, m, 0, lane, mode, e, rew);
+        }
+        for (int i = lane; i < 36; i += 32) m.bk_cnt()[i] = 0u;  // empty buckets for the next step
+        __syncwarp();
+        if (any_obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        __syncwarp();
+    }
 
     if (any_obs && tid == 0) {  // bulk stores: the env's contiguous tile, (f2) its env-wide tail, its government row
         if (staged) {
@@ -666,14 +810,19 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
         // (build_coltab) replaces a chain of ten compares per element
         extern __shared__ __align__(16) uint8_t ej_smem[];
         const int D = D_pop, total = N * D;
-        const uint32_t* tab = m.coltab();
+        const uint2* tab = reinterpret_cast<const uint2*>(m.coltab());
         float* dst = obs + (size_t)e * total;
+        // idx = i D + k advances by the CTA size: (i, k) follow without a division per element
+        const int dq = NPAD / D, dr = NPAD - dq * D;
+        int i = tid / D, k = tid - i * D;
         for (int idx = tid; idx < total; idx += NPAD) {
-            const int i = idx / D, k = idx - i * D;
-            const uint32_t base = tab[k], st = tab[D + k];
-            const uint32_t w = *reinterpret_cast<const uint32_t*>(ej_smem + base + (uint32_t)i * (st & 4u));
-            const float f = (st >> 31) ? (float)(int)w : __uint_as_float(w);
-            dst[idx] = __fmul_rn(f, __uint_as_float(tab[2 * D + k]));  // scale 1 for the unscaled columns: exact
+            const uint2 col = tab[k];  // source offset | per-agent stride (bit 30) | integer source (bit 31), scale
+            const uint32_t w = *reinterpret_cast<const uint32_t*>(ej_smem + (col.x & 0xFFFFFu) + ((col.x >> 30) & 1u) * (uint32_t)(i * 4));
+            const float f = (col.x >> 31) ? (float)(int)w : __uint_as_float(w);
+            dst[idx] = __fmul_rn(f, __uint_as_float(col.y));  // scale 1 for the unscaled columns: exact
+            i += dq;
+            k += dr;
+            if (k >= D) { k -= D; ++i; }
         }
         __syncthreads();  // the loop reads other agents' state: the next step must not start updating it
     }
@@ -731,8 +880,8 @@ __device__ __noinline__ int masked_draw(const DevCfg& c, const SM& m, int tid, u
 }
 
 // Column table of the population observation row (G25) for shapes whose tile does not fit
-// the staging buffer: per column k the byte offset of its source array in shared memory, the
-// per-agent stride (4, or 0 for the env-wide tail) with bit 31 = integer source, and the scale.
+// the staging buffer: per column k one 64-bit entry = byte offset of its source array in shared memory | bit 30:
+// one value per agent (else the env-wide tail) | bit 31: integer source, and the scale.
 template <int NS, class SM>
 __device__ __forceinline__ void build_coltab(const DevCfg& c, const SM& m, int tid, int nthreads) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
@@ -740,7 +889,7 @@ __device__ __forceinline__ void build_coltab(const DevCfg& c, const SM& m, int t
     const int R = c.R, D = c.D_pop, priv = 3 * R + 4;
     auto off = [&](const void* p) { return (uint32_t)((const uint8_t*)p - ej_smem); };
     for (int k = tid; k < D; k += nthreads) {
-        uint32_t base, st = 4u;
+        uint32_t base, st = 1u << 30;  // bit 30: one value per agent; bit 31: integer source
         float sc = 1.0f;
         if (k >= priv) { base = off(m.shrow() + (k - priv)); st = 0u; }
         else if (k == 0) { base = off(m.coin()); sc = c.s_coin; }
@@ -750,9 +899,8 @@ __device__ __forceinline__ void build_coltab(const DevCfg& c, const SM& m, int t
         else if (k <= 3 * R + 1) base = off(m.SG() + (k - 2 * R - 2) * NS);
         else if (k == 3 * R + 2) base = off(m.SC());
         else { base = off(m.labor()); sc = c.s_labor; }
-        m.coltab()[k] = base;
-        m.coltab()[D + k] = st;
-        m.coltab()[2 * D + k] = __float_as_uint(sc);
+        m.coltab()[2 * k] = base | st;
+        m.coltab()[2 * k + 1] = __float_as_uint(sc);
     }
 }
 
@@ -832,7 +980,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
         if (io.io.gov_out) io.gov_out()[(uint32_t)(e * B + tid)] = gov_lvl;
     }
 
-    int lvl = -1, grp = 0, pos = 0, price_c = 0, r_c = 0, side_c = 0;
+    int lvl = -1, grp = 0, price_c = 0, r_c = 0, side_c = 0;
     uint32_t slot = 0, mymask = 0, old_tail = NIL;
     if (act) {
         coin_pre = m.coin()[tid];
@@ -897,10 +1045,14 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
                 slot = ((uint32_t)tid << MPL) + (uint32_t)(__ffs(~mymask) - 1);
                 m.cslot()[tid] = slot;
                 old_tail = m.tail()[lvl];  // read before anyone links (tails change after barrier #1)
-                if (K) {
+                if (K) {  // book cap: push on the key bins of the level and of the book
                     grp = r_c * 2 + side_c;
-                    pos = atomicAdd(&m.gcnt()[grp], 1);
-                    m.cinfo()[tid] = lvl;
+                    const uint32_t n1 = atomicExch(&m.lbh()[(uint32_t)lvl * LEVEL_BINS + (x2 >> LEVEL_BIN_SHIFT)], (uint32_t)tid);
+                    atomicOr(&m.lmask()[lvl], 1u << (x2 >> LEVEL_BIN_SHIFT));
+                    const uint32_t bb = (uint32_t)grp * BOOK_BINS + (x2 >> BOOK_BIN_SHIFT);
+                    const uint32_t n2 = atomicExch(&m.bbh()[bb], (uint32_t)tid);
+                    atomicAdd(&m.bbc()[bb], 1u);
+                    m.anext()[tid] = n1 | (n2 << 16);  // next candidate of the level bin | of the book bin
                 } else {  // push on the level's arrival stack
                     m.anext()[tid] = atomicExch(&m.ahead()[lvl], (uint32_t)tid);
                 }
@@ -936,53 +1088,69 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
             accepted = true;
         }
     } else {
-        // exclusive scan of the per-book candidate counts (warp 0)
-        if (tid < 32) {
-            int carry = 0;
-            for (int base = 0; base < c.n_groups; base += 32) {
-                const int g = base + tid;
-                const int v = g < c.n_groups ? m.gcnt()[g] : 0;
-                int incl = v;
+        // Book cap (G15): the j-th candidate of a book in arrival order is accepted iff n_rest + j < K.  Rank on the
+        // book = candidates in lower key bins (exclusive prefix of the bin counts) + earlier candidates of the own bin.
+        for (int w = tid >> 5; w < 2 * R; w += NPAD / 32) {  // a warp scans the bins of one book: 8 bins per lane
+            const int lane = tid & 31;
+            uint32_t* cnt = m.bbc() + w * BOOK_BINS + lane * (BOOK_BINS / 32);
+            uint32_t v[BOOK_BINS / 32], sum = 0;
 #pragma unroll
-                for (int o = 1; o < 32; o <<= 1) {
-                    const int y = __shfl_up_sync(FULL, incl, o);
-                    if (tid >= o) incl += y;
-                }
-                if (g < c.n_groups) m.goff()[g] = carry + incl - v;
-                carry += __shfl_sync(FULL, incl, 31);
+            for (int q = 0; q < BOOK_BINS / 32; ++q) { v[q] = cnt[q]; sum += v[q]; }
+            uint32_t incl = sum;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const uint32_t y = __shfl_up_sync(FULL, incl, o);
+                if (lane >= o) incl += y;
             }
+            uint32_t run = incl - sum;
+#pragma unroll
+            for (int q = 0; q < BOOK_BINS / 32; ++q) { cnt[q] = run; run += v[q]; }
         }
         __syncthreads();
-        // arrival key | agent | level: ordered by (key, agent) (G11); the level rides along so that the
-        // ranking loop needs no second, dependent load
-        const unsigned long long mine = ((unsigned long long)x2 << 32) | ((unsigned long long)tid << 16) | (unsigned long long)(lvl >= 0 ? lvl : 0);
-        if (lvl >= 0) m.bucket()[m.goff()[grp] + pos] = mine;
-        __syncthreads();
-        int before = 0, gbase = 0, gn = 0;
+        int succ = -1;
         if (lvl >= 0) {
-            gbase = m.goff()[grp];
-            gn = m.gcnt()[grp];
-            int brank = 0;
-            for (int k = 0; k < gn; ++k) {
-                const unsigned long long o = m.bucket()[gbase + k];
-                const int lj = (int)(o & 0xFFFFu);
-                const bool earlier = o < mine, same = lj == lvl;
-                brank += earlier;
-                lrank += same && earlier;
-                before += (lj < lvl) || (same && earlier);
+            const uint32_t bb = (uint32_t)grp * BOOK_BINS + (x2 >> BOOK_BIN_SHIFT);
+            int brank = (int)m.bbc()[bb];
+            for (uint32_t j = m.bbh()[bb]; j != NIL; j = m.anext()[j] >> 16) {
+                const uint32_t kj = m.key()[j];
+                brank += (kj < x2) || (kj == x2 && (int)j < tid);
             }
             int n_rest = 0;
             for (int p = 0; p < P; ++p) n_rest += cnt_cur[grp * P + p];
             accepted = n_rest + brank < K;
-            m.sorted()[gbase + before] = (uint32_t)tid | (accepted ? 0x10000u : 0u);
+            m.cslot()[tid] = slot | (accepted ? 0x10000u : 0u);
+            // neighbours on the level: an earlier arrival (then this one is not the level's first) and the next one
+            const uint32_t b5 = x2 >> LEVEL_BIN_SHIFT, lmask = m.lmask()[lvl];
+            lrank = (lmask & ((1u << b5) - 1u)) != 0u;
+            uint32_t sk = 0;
+            for (uint32_t j = m.lbh()[(uint32_t)lvl * LEVEL_BINS + b5]; j != NIL; j = m.anext()[j] & 0xFFFFu) {
+                if ((int)j == tid) continue;
+                const uint32_t kj = m.key()[j];
+                const bool later = (kj > x2) || (kj == x2 && (int)j > tid);
+                if (!later) lrank = 1;
+                else if (succ < 0 || kj < sk || (kj == sk && (int)j < succ)) { succ = (int)j; sk = kj; }
+            }
+            const uint32_t above = (lmask >> b5) >> 1;
+            if (succ < 0 && above) {  // the earliest arrival of the next occupied bin
+                const uint32_t b2 = b5 + (uint32_t)__ffs(above);
+                for (uint32_t j = m.lbh()[(uint32_t)lvl * LEVEL_BINS + b2]; j != NIL; j = m.anext()[j] & 0xFFFFu) {
+                    const uint32_t kj = m.key()[j];
+                    if (succ < 0 || kj < sk || (kj == sk && (int)j < succ)) { succ = (int)j; sk = kj; }
+                }
+            }
         }
-        __syncthreads();
-        if (lvl >= 0 && accepted && before + 1 < gn) {
-            const uint32_t s = m.sorted()[gbase + before + 1];
-            const int j = (int)(s & 0xFFFFu);
-            if ((s & 0x10000u) && m.cinfo()[j] == lvl) nxt = m.cslot()[j];
+        __syncthreads();  // acceptance flags of every candidate
+        if (lvl >= 0) {
+            if (accepted && succ >= 0) {  // acceptance is a prefix of the book's arrival order: only the successor can fail
+                const uint32_t cs = m.cslot()[succ];
+                if (cs & 0x10000u) nxt = cs & 0xFFFFu;
+            }
+            // bins ready for the next step (every member of a bin writes the same values)
+            m.lbh()[(uint32_t)lvl * LEVEL_BINS + (x2 >> LEVEL_BIN_SHIFT)] = NIL;
+            m.lmask()[lvl] = 0u;
+            m.bbh()[(uint32_t)grp * BOOK_BINS + (x2 >> BOOK_BIN_SHIFT)] = NIL;
         }
-        for (int g = tid; g < c.n_groups; g += NPAD) m.gcnt()[g] = 0;  // ready for the next step
+        for (int g = tid; g < 2 * R * BOOK_BINS; g += NPAD) m.bbc()[g] = 0u;
     }
 
     if (lvl >= 0) {
@@ -1147,6 +1315,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
         }
     }
     if (tid < B && (boundary || first)) m.shrow()[5 * R + tid] = m.hdr()->rates[tid];
+    if (SM::L::bucketed) coin_bucket_fill<NPAD>(m, tid, act);  // the coin is final: file it for the block-wide sort
     __syncthreads();  // #5 state final
     if (tid == 0) {
         m.hdr()->t = t + 1;
@@ -1174,6 +1343,7 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
         if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
         if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
         if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
+        if (SM::L::bucketed) coin_bucket_fill<NPAD>(m, tid, tid < c.N);
         __syncthreads();
         mode = 1;
     } else {
@@ -1212,8 +1382,12 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
                      "l"(blob), "r"(c.blob_bytes), "r"(bar)
                      : "memory");
     }
-    if (c.K == 0)
+    if (c.K == 0) {
         for (int l = tid; l < c.n_levels; l += NPAD) m.ahead()[l] = NIL;
+    } else {
+        for (int l = tid; l < c.n_levels * LEVEL_BINS; l += NPAD) m.lbh()[l] = NIL;
+        for (int l = tid; l < 2 * c.R * BOOK_BINS; l += NPAD) m.bbh()[l] = NIL;
+    }
     if (!io.actions)
         for (int i = tid; i < c.A; i += NPAD) m.cdf()[i] = io.cdf[i];
     build_coltab<NS>(c, m, tid, NPAD);
@@ -1250,12 +1424,14 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     const Sm<NS> m{c};
     const uint4* blob = (const uint4*)(state + (size_t)e * c.blob_bytes);
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
+    if (Lay<NS>::bucketed && tid < 36) m.bk_cnt()[tid] = 0u;
     __syncthreads();
     const int t = m.hdr()->t;
     build_coltab<NS>(c, m, tid, NPAD);
     if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
     if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
     if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
+    if (Lay<NS>::bucketed) coin_bucket_fill<NPAD>(m, tid, tid < c.N);
     __syncthreads();
     outputs<NPAD, NS, 0, 0, 0, 0, 0>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");

@@ -87,7 +87,7 @@ def test_per_resource_craft_mode():
     run_episode("config3_resources", 3, 120, craft_mode=inputs.CRAFT_PER_RESOURCE, state_every=10)
 
 
-@pytest.mark.parametrize("N", [1, 2, 5, 31, 32, 33, 63, 97, 129, 250])
+@pytest.mark.parametrize("N", [1, 2, 5, 31, 32, 33, 63, 97, 129, 250, 300, 417, 512, 600, 1024])
 def test_ragged_population_sizes(N):
     cfg = dict(inputs.configs()["config2_paper"], N=N)
     params = dict(cfg["params"], tax_period=20, episode_length=80)
