@@ -154,9 +154,12 @@ void build_layout(DevCfg& c) {
         c.o_ma = o + R * NP * 4;
         take(c.N * c.D_pop * 4);
     } else {
-        c.o_mb = take(R * NP * 4);
-        c.o_ma = take(R * NP * 4);
-        c.o_coltab = take(3 * c.D_pop * 4);  // column table of the unstaged observation loop
+        // matched-order lists, and over the same bytes the per-warp row buffers of the unstaged observation path (the
+        // lists are consumed when the trades settle, the rows are written after the state is final)
+        const int rowbuf = c.n_warps * 8 * c.D_pop * 4;
+        c.o_mb = take(lists > rowbuf ? lists : rowbuf);
+        c.o_ma = c.o_mb + R * NP * 4;
+        c.o_rowbuf = c.o_mb;
         c.o_stage = o;
     }
     c.smem_bytes = o;

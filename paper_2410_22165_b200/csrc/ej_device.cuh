@@ -73,7 +73,7 @@ struct DevCfg {
     // scratch section offsets (bytes from the shared-memory base; all after the blob)
     int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma;
     int o_bbh, o_bbc, o_lbh, o_lmask;  // book-cap path (K > 0): arrival bins per book and per level
-    int o_resq, o_shrow, o_govrow, o_misc, o_cdf, o_coltab, o_stage;
+    int o_resq, o_shrow, o_govrow, o_misc, o_cdf, o_rowbuf, o_stage;
     int smem_bytes;
     unsigned long long gov_obs_offset, obs_floats;
 };
@@ -117,11 +117,14 @@ struct Lay {
     static constexpr int misc = govrow + govrow_cap * 4;       // u64 [2]: tax pool
     // block-wide coin sort (CTAs of 8 warps and more): one bucket of coin keys per warp
     static constexpr bool bucketed = NP >= 416;                 // NP is the array stride (13/16 of the CTA size or the CTA size): CTAs of 512 and 1024 threads
-    static constexpr int bk_cap = 128;                          // keys per bucket (4 per lane at most)
+    static constexpr int bk_warps = NP >= 832 ? 32 : 16;        // warps of such a CTA = buckets
+    // the bucket keys live in key | cslot | anext (3 NP words): those are dead between the settlement of a step's
+    // trades and the next step's arrivals, which is when the buckets are filled and sorted
+    static constexpr int bk_keys = key;
+    static constexpr int bk_cap = (3 * NP / bk_warps) < 128 ? (3 * NP / bk_warps) : 128;  // keys per bucket (sorted 4 per lane at most)
     static constexpr int bk_cnt = misc + 16;                    // u32 [32] bucket sizes, [32] = overflow flag, [33..34] medians
     static constexpr int bk_part = bk_cnt + (bucketed ? 36 * 4 : 0);  // f64 [32][3]: gini, sum, sum of squares per bucket
-    static constexpr int bk_keys = bk_part + (bucketed ? 32 * 3 * 8 : 0);
-    static constexpr int blob = bk_keys + (bucketed ? 32 * bk_cap * 4 : 0);
+    static constexpr int blob = bk_part + (bucketed ? 32 * 3 * 8 : 0);
     // blob sections (byte offsets relative to the blob)
     static constexpr int coin = (int)sizeof(EnvHdr);
     static constexpr int labor = coin + NP * 4;
@@ -205,7 +208,7 @@ struct Sm {
     __device__ __forceinline__ uint32_t* lmask() const { return at<uint32_t>(c.o_lmask); }  // [levels] occupied level bins
     __device__ __forceinline__ uint32_t* cdf() const { return at<uint32_t>(ST ? S::cdf : c.o_cdf); }
     __device__ __forceinline__ float* stage() const { return at<float>(ST ? S::stage : c.o_stage); }
-    __device__ __forceinline__ uint32_t* coltab() const { return at<uint32_t>(c.o_coltab); }
+    __device__ __forceinline__ float* rowbuf() const { return at<float>(c.o_rowbuf); }  // [warps][8][D_pop]: unstaged observation rows
 };
 
 // f3, skill growth ("the respective skill is increased by 0.5%.  This 0.5% bonus shrinks as the agent
@@ -804,27 +807,40 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
         }
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
     }
-    // ---- population rows when they cannot go out as one bulk store: coalesced loop ----
+    // ---- population rows when the env's tile does not fit in shared memory: every warp sends its 32 rows in chunks
+    // of 8 through a private row-major buffer (odd row length: the 8 writers hit distinct banks), then copies the
+    // chunk out with 128-bit coalesced stores.  The env-wide tail of the 8 buffer rows is written once per step.
     if (!FX && obs && !staged) {
-        // element (i, k) = scale_k * value of column k's source array at agent i: the column table
-        // (build_coltab) replaces a chain of ten compares per element
-        extern __shared__ __align__(16) uint8_t ej_smem[];
-        const int D = D_pop, total = N * D;
-        const uint2* tab = reinterpret_cast<const uint2*>(m.coltab());
-        float* dst = obs + (size_t)e * total;
-        // idx = i D + k advances by the CTA size: (i, k) follow without a division per element
-        const int dq = NPAD / D, dr = NPAD - dq * D;
-        int i = tid / D, k = tid - i * D;
-        for (int idx = tid; idx < total; idx += NPAD) {
-            const uint2 col = tab[k];  // source offset | per-agent stride (bit 30) | integer source (bit 31), scale
-            const uint32_t w = *reinterpret_cast<const uint32_t*>(ej_smem + (col.x & 0xFFFFFu) + ((col.x >> 30) & 1u) * (uint32_t)(i * 4));
-            const float f = (col.x >> 31) ? (float)(int)w : __uint_as_float(w);
-            dst[idx] = __fmul_rn(f, __uint_as_float(col.y));  // scale 1 for the unscaled columns: exact
-            i += dq;
-            k += dr;
-            if (k >= D) { k -= D; ++i; }
+        const int D = D_pop, npriv = 3 * R + 4;
+        float* buf = m.rowbuf() + warp * (8 * D);
+        float* dst = obs + (size_t)e * (size_t)(N * D);
+        for (int r = 0; r < 8; ++r)
+            for (int k = lane; k < D - npriv; k += 32) buf[r * D + npriv + k] = m.shrow()[k];
+        const bool vec = (((size_t)N * (size_t)D) & 3u) == 0 && ((8 * D) & 3) == 0;  // 16-byte aligned chunks
+#pragma unroll 1
+        for (int ch = 0; ch < 4; ++ch) {
+            const int row0 = warp * 32 + ch * 8;
+            if (row0 >= N) break;
+            if ((lane >> 3) == ch && act) {
+                float* o = buf + (lane & 7) * D;
+                o[0] = __fmul_rn(m.coin()[tid], c.s_coin);
+                for (int r = 0; r < R; ++r) o[1 + r] = __fmul_rn((float)m.inv()[r * N4 + tid], c.s_count);
+                o[R + 1] = __fmul_rn((float)m.esc_coin()[tid], c.s_coin);
+                for (int r = 0; r < R; ++r) o[R + 2 + r] = __fmul_rn((float)m.esc_res()[r * N4 + tid], c.s_count);
+                for (int r = 0; r < R; ++r) o[2 * R + 2 + r] = m.SG()[r * N4 + tid];
+                o[3 * R + 2] = m.SC()[tid];
+                o[3 * R + 3] = __fmul_rn(m.labor()[tid], c.s_labor);
+            }
+            __syncwarp();
+            const int rows = N - row0 < 8 ? N - row0 : 8, n = rows * D;
+            float* out = dst + row0 * D;
+            if (vec && rows == 8) {
+                for (int j = lane; j < n / 4; j += 32) reinterpret_cast<float4*>(out)[j] = reinterpret_cast<const float4*>(buf)[j];
+            } else {
+                for (int j = lane; j < n; j += 32) out[j] = buf[j];
+            }
+            __syncwarp();
         }
-        __syncthreads();  // the loop reads other agents' state: the next step must not start updating it
     }
 }
 
@@ -877,31 +893,6 @@ __device__ __noinline__ int masked_draw(const DevCfg& c, const SM& m, int tid, u
         target = ((unsigned long long)x0 * S) >> 32;  // S <= 2^32: no overflow
     }
     return pick >= 0 ? pick : first_ok;
-}
-
-// Column table of the population observation row (G25) for shapes whose tile does not fit
-// the staging buffer: per column k one 64-bit entry = byte offset of its source array in shared memory | bit 30:
-// one value per agent (else the env-wide tail) | bit 31: integer source, and the scale.
-template <int NS, class SM>
-__device__ __forceinline__ void build_coltab(const DevCfg& c, const SM& m, int tid, int nthreads) {
-    extern __shared__ __align__(16) uint8_t ej_smem[];
-    if (c.stage_obs) return;
-    const int R = c.R, D = c.D_pop, priv = 3 * R + 4;
-    auto off = [&](const void* p) { return (uint32_t)((const uint8_t*)p - ej_smem); };
-    for (int k = tid; k < D; k += nthreads) {
-        uint32_t base, st = 1u << 30;  // bit 30: one value per agent; bit 31: integer source
-        float sc = 1.0f;
-        if (k >= priv) { base = off(m.shrow() + (k - priv)); st = 0u; }
-        else if (k == 0) { base = off(m.coin()); sc = c.s_coin; }
-        else if (k <= R) { base = off(m.inv() + (k - 1) * NS); st |= 0x80000000u; sc = c.s_count; }
-        else if (k == R + 1) { base = off(m.esc_coin()); st |= 0x80000000u; sc = c.s_coin; }
-        else if (k <= 2 * R + 1) { base = off(m.esc_res() + (k - R - 2) * NS); st |= 0x80000000u; sc = c.s_count; }
-        else if (k <= 3 * R + 1) base = off(m.SG() + (k - 2 * R - 2) * NS);
-        else if (k == 3 * R + 2) base = off(m.SC());
-        else { base = off(m.labor()); sc = c.s_labor; }
-        m.coltab()[2 * k] = base | st;
-        m.coltab()[2 * k + 1] = __float_as_uint(sc);
-    }
 }
 
 // Inputs and outputs of step `s` of a launch (ring slot `slot`), resolved where they are used:
@@ -1390,7 +1381,6 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
     }
     if (!io.actions)
         for (int i = tid; i < c.A; i += NPAD) m.cdf()[i] = io.cdf[i];
-    build_coltab<NS>(c, m, tid, NPAD);
     __syncthreads();  // the tables above, and the mbarrier's initialisation, for every thread
     asm volatile(
         "{\n\t.reg .pred p;\n\tEJ_BLOB_WAIT_%=:\n\t"
@@ -1427,7 +1417,6 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     if (Lay<NS>::bucketed && tid < 36) m.bk_cnt()[tid] = 0u;
     __syncthreads();
     const int t = m.hdr()->t;
-    build_coltab<NS>(c, m, tid, NPAD);
     if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
     if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
     if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
