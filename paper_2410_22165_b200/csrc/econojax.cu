@@ -144,10 +144,18 @@ void build_layout(DevCfg& c) {
     // staging tile of the population observation rows (not zeroed); the matched-order lists
     // mb | ma alias its head (written after the previous step's bulk store has been read,
     // consumed before the rows are staged)
+    // bucket keys of labor and income (block-wide sort of CTAs of 512 / 1024 threads): live between the end of the
+    // state update and the statistics of the same step
+    const int bk2 = for_variant(c.Npad, NP, [&](auto, auto ns) {
+        using L = Lay<decltype(ns)::value>;
+        return L::bucketed ? 2 * L::bk_warps * L::bk_cap * 4 : 0;
+    });
     c.o_stage = o;
     c.stage_obs = 0;
     const int lists = 2 * R * NP * 4;
     if ((c.N * c.D_pop) % 4 == 0 && c.N * c.D_pop * 4 >= lists && o + c.N * c.D_pop * 4 <= 100 * 1024) {
+        c.o_bk2 = bk2 ? take(bk2) : c.o_ahead;  // the staging tile is being written while these keys are live
+        c.o_stage = o;
         c.stage_obs = 1;
         c.stage_alias_bytes = lists;
         c.o_mb = o;
@@ -157,7 +165,10 @@ void build_layout(DevCfg& c) {
         // matched-order lists, and over the same bytes the per-warp row buffers of the unstaged observation path (the
         // lists are consumed when the trades settle, the rows are written after the state is final)
         const int rowbuf = c.n_warps * 8 * c.D_pop * 4;
-        c.o_mb = take(lists > rowbuf ? lists : rowbuf);
+        int region = lists > rowbuf ? lists : rowbuf;
+        if (bk2 > region) region = bk2;  // the same bytes hold the bucket keys of labor and income in between
+        c.o_mb = take(region);
+        c.o_bk2 = c.o_mb;
         c.o_ma = c.o_mb + R * NP * 4;
         c.o_rowbuf = c.o_mb;
         c.o_stage = o;

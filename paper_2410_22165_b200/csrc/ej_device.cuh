@@ -24,10 +24,30 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+#ifdef EJ_PHASE_CLOCK
+#include <stdio.h>
+#endif
 
 #include "../../include/econojax.h"
 
 namespace {
+
+// Debug builds (-DEJ_PHASE_CLOCK): block 0 accumulates the cycles between the barriers of a step and prints them at
+// the end of the launch.  Not compiled into the product library.
+#ifdef EJ_PHASE_CLOCK
+__device__ unsigned long long ej_phase_cycles[16];
+__device__ unsigned long long ej_phase_last;
+#define EJ_MARK(k)                                                                     \
+    do {                                                                               \
+        if (blockIdx.x == 0 && threadIdx.x == 0) {                                     \
+            const unsigned long long now_ = clock64();                                 \
+            ej_phase_cycles[k] += now_ - ej_phase_last;                                \
+            ej_phase_last = now_;                                                      \
+        }                                                                              \
+    } while (0)
+#else
+#define EJ_MARK(k) do { } while (0)
+#endif
 
 constexpr uint32_t NIL = 0xFFFFu;      // null slot of the order pool
 // Book-cap path: a step's candidates are binned by the top bits of their arrival key (a uniform Philox word, G11):
@@ -44,8 +64,10 @@ struct EnvHdr {
     int32_t pad1;
     float rates[EJ_MAX_BRACKETS];
     int32_t last_price[EJ_MAX_RESOURCES];
-    uint32_t coin_spl[32];  // last step's coin order statistics of rank (b+1) N / NW (float bits): bucket bounds of the
-                            // block-wide coin sort of large populations; hints like med_prev, not state
+    // block-wide sort of large populations: bucket bounds of coin, labor, income = last step's order statistics of
+    // rank (b+1) N / NW (float bits), double-buffered (spl_cur names the buffer in force); hints like med_prev, not state
+    uint32_t spl[3][2][32];
+    uint32_t spl_cur, spl_pad[3];
 };
 static_assert(sizeof(EnvHdr) % 16 == 0, "EnvHdr must keep 16-byte alignment");
 
@@ -73,6 +95,7 @@ struct DevCfg {
     // scratch section offsets (bytes from the shared-memory base; all after the blob)
     int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma;
     int o_bbh, o_bbc, o_lbh, o_lmask;  // book-cap path (K > 0): arrival bins per book and per level
+    int o_bk2;                         // bucket keys of labor and income (CTAs of 512 / 1024 threads)
     int o_resq, o_shrow, o_govrow, o_misc, o_cdf, o_rowbuf, o_stage;
     int smem_bytes;
     unsigned long long gov_obs_offset, obs_floats;
@@ -122,9 +145,9 @@ struct Lay {
     // trades and the next step's arrivals, which is when the buckets are filled and sorted
     static constexpr int bk_keys = key;
     static constexpr int bk_cap = (3 * NP / bk_warps) < 128 ? (3 * NP / bk_warps) : 128;  // keys per bucket (sorted 4 per lane at most)
-    static constexpr int bk_cnt = misc + 16;                    // u32 [32] bucket sizes, [32] = overflow flag, [33..34] medians
-    static constexpr int bk_part = bk_cnt + (bucketed ? 36 * 4 : 0);  // f64 [32][3]: gini, sum, sum of squares per bucket
-    static constexpr int blob = bk_part + (bucketed ? 32 * 3 * 8 : 0);
+    static constexpr int bk_cnt = misc + 16;                    // u32 [3][72]: per metric [0..31] bucket sizes, [32..63] values equal to a bound, [64] overflow flag, [65..66] medians
+    static constexpr int bk_part = bk_cnt + (bucketed ? 3 * 72 * 4 : 0);  // f64 [3][32][3]: gini, sum, sum of squares per bucket
+    static constexpr int blob = bk_part + (bucketed ? 3 * 32 * 3 * 8 : 0);
     // blob sections (byte offsets relative to the blob)
     static constexpr int coin = (int)sizeof(EnvHdr);
     static constexpr int labor = coin + NP * 4;
@@ -195,9 +218,12 @@ struct Sm {
     __device__ __forceinline__ float* shrow() const { return at<float>(L::shrow); }
     __device__ __forceinline__ float* govrow() const { return at<float>(L::govrow); }
     __device__ __forceinline__ unsigned long long* misc() const { return at<unsigned long long>(L::misc); }  // [0] tax pool in 2^-20 coin
-    __device__ __forceinline__ uint32_t* bk_cnt() const { return at<uint32_t>(L::bk_cnt); }
-    __device__ __forceinline__ double* bk_part() const { return at<double>(L::bk_part); }
-    __device__ __forceinline__ uint32_t* bk_keys() const { return at<uint32_t>(L::bk_keys); }
+    __device__ __forceinline__ uint32_t* bk_cnt(int k) const { return at<uint32_t>(L::bk_cnt) + k * 72; }
+    __device__ __forceinline__ double* bk_part(int k) const { return at<double>(L::bk_part) + k * 96; }
+    // bucket keys: coin in key | cslot | anext, labor and income in a region of their own (or over the matched lists)
+    __device__ __forceinline__ uint32_t* bk_keys(int k) const {
+        return k == 0 ? at<uint32_t>(L::bk_keys) : at<uint32_t>(c.o_bk2) + (k - 1) * (L::bk_warps * L::bk_cap);
+    }
     __device__ __forceinline__ uint32_t* ahead() const { return at<uint32_t>(ST ? S::ahead : c.o_ahead); }
     __device__ __forceinline__ uint32_t* mb() const { return at<uint32_t>(ST ? S::mb : c.o_mb); }
     __device__ __forceinline__ uint32_t* ma() const { return at<uint32_t>(ST ? S::ma : c.o_ma); }
@@ -477,7 +503,7 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const SM& m, int k
     float lo, hi;
     const int r0 = N >= 2 ? (N >> 1) - 1 : 0, r1 = N >> 1;
     bool found = false;
-    if (k != 0) {  // labor, income: med_prev holds last step's lower median
+    if (k != 0 && !SM::L::bucketed) {  // labor, income: med_prev holds last step's lower median
         uint32_t key[EPL], klo, khi;
 #pragma unroll
         for (int q = 0; q < EPL; ++q) key[q] = __float_as_uint(x[q]);
@@ -490,11 +516,12 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const SM& m, int k
         lo = warp_pick<EPL>(x, r0);
         hi = warp_pick<EPL>(x, r1);
         if (k != 0 && lane == 0) m.hdr()->med_prev[k - 1] = __float_as_uint(lo);
-        if (k == 0 && SM::L::bucketed) {  // EPL = warps of the CTA: renew the bucket bounds of the block-wide sort
+        if (SM::L::bucketed) {  // EPL = warps of the CTA: renew this metric's bucket bounds of the block-wide sort
+            const uint32_t nxt = (m.hdr()->spl_cur & 1u) ^ 1u;
 #pragma unroll 1
             for (int b = 0; b + 1 < EPL; ++b) {
                 const float v = warp_pick<EPL>(x, ((b + 1) * N) / EPL);
-                if (lane == 0) m.hdr()->coin_spl[b] = __float_as_uint(v);
+                if (lane == 0) m.hdr()->spl[k][nxt][b] = __float_as_uint(v);
             }
         }
         if (k == 0 && mode != 2) {
@@ -569,42 +596,59 @@ __device__ __forceinline__ void int_metric_stats(const DevCfg& c, const SM& m, i
     if (lane == 0) gov_triple<NS, NT>(c, m, 3 + r, mean, var, (float)(int)klo, (float)(int)khi, c.s_count);
 }
 
-// ---- block-wide coin statistics of large populations (CTAs of 512 / 1024 threads) ----
-// The coin metric needs the sorted order (median, and gini in its sorted-rank form, G23).  One warp sorting 1024
-// values in registers was the longest branch of the N = 1000 step (profiles/r2a: 26 % of the stall samples on the
-// barrier that waits for it).  Here every warp sorts one BUCKET of coin values: bucket b holds the values in
-// [spl[b-1], spl[b]), the bounds being last step's order statistics of rank (b+1) N / NW (coins drift slowly, so the
-// buckets stay near N / NW values); the rank of a value = sizes of the lower buckets + its place in its bucket.
-// Exact for any bounds; if a bucket overflows (start of an episode, a tax redistribution, many equal coins) the
-// step falls back to the single-warp sort, which also renews the bounds.
+// ---- block-wide statistics of the float metrics of large populations (CTAs of 512 / 1024 threads) ----
+// Coin, labor and income need order statistics (the median; coin also gini in its sorted-rank form, G23).  One warp
+// holding all N values of a metric in registers was the longest branch of the N = 1000 step: 20,000 of its 56,000
+// cycles went by waiting for those three warps (profiles/r2c).  Here every warp sorts one BUCKET per metric: bucket b
+// holds the values strictly between the bounds spl[b-1] and spl[b], the bounds being last step's order statistics
+// of rank (b+1) N / NW (the metrics drift slowly, so a bucket stays near N / NW values).  Values EQUAL to a bound are
+// only counted (they need no sorting), which keeps large groups of equal values -- every income 0 after a tax
+// collection, many agents on the same coin -- out of the buckets.  Rank of a value = sizes of the lower buckets and
+// bound groups + its place in its bucket.  Exact for any bounds; if a bucket overflows (start of an episode, a
+// redistribution) that metric falls back to the single-warp sort, which also renews its bounds.
 
-// Thread `tid` files its agent's final coin of this step; called before the barrier that ends the state update.
+// Thread `tid` files the final value x of metric k of its agent; called before the barrier that ends the state update.
 template <int NPAD, class SM>
-__device__ __forceinline__ void coin_bucket_fill(const SM& m, int tid, bool act) {
+__device__ __forceinline__ void bucket_fill(const SM& m, int k, float x) {
     constexpr int NW = NPAD / 32, CAP = SM::L::bk_cap;
-    if (!act) return;
-    const uint32_t key = __float_as_uint(m.coin()[tid]);
+    const uint32_t key = __float_as_uint(x);
+    const uint32_t* spl = m.hdr()->spl[k][m.hdr()->spl_cur & 1u];
     int lo = 0, hi = NW - 1;  // bucket = number of bounds <= key
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;
-        if (key < m.hdr()->coin_spl[mid]) hi = mid;
+        if (key < spl[mid]) hi = mid;
         else lo = mid + 1;
     }
-    const uint32_t pos = atomicAdd(&m.bk_cnt()[lo], 1u);
-    if (pos < (uint32_t)CAP && !(key >> 31)) m.bk_keys()[lo * CAP + (int)pos] = key;
-    else m.bk_cnt()[32] = 1u;  // overflow (or a negative value): fall back
+    uint32_t* cnt = m.bk_cnt(k);
+    if (lo > 0 && spl[lo - 1] == key) {
+        atomicAdd(&cnt[32 + lo - 1], 1u);  // equal to bound lo-1 (the last of equal bounds): counted, not stored
+    } else {
+        const uint32_t pos = atomicAdd(&cnt[lo], 1u);
+        if (pos < (uint32_t)CAP && !(key >> 31)) m.bk_keys(k)[lo * CAP + (int)pos] = key;
+        else cnt[64] = 1u;  // overflow (or a negative value): fall back
+    }
+}
+template <int NPAD, class SM>
+__device__ __forceinline__ void bucket_fill_all(const SM& m, int tid, bool act) {
+    if (!act) return;
+    bucket_fill<NPAD>(m, 0, m.coin()[tid]);
+    bucket_fill<NPAD>(m, 1, m.labor()[tid]);
+    bucket_fill<NPAD>(m, 2, m.income()[tid]);
 }
 
-// Warp `warp` sorts its bucket (n <= 32 EPL values, blocked layout) and leaves its share of gini, sum and sum of
-// squares; the warp that holds a wanted rank writes that order statistic (medians, next step's bounds).
+// Warp `warp` sorts its bucket of metric k (n <= 32 EPL values, blocked layout), followed in rank order by the ne
+// values equal to its upper bound v; leaves its share of (gini,) sum and sum of squares; the warp that holds a wanted
+// rank writes that order statistic (the two medians, next step's bounds).
 template <int EPL, int NPAD, class SM>
-__device__ __forceinline__ void coin_bucket_sort(const SM& m, int warp, int lane, int n, int off, int N) {
+__device__ __forceinline__ void bucket_sort(const SM& m, int k, int warp, int lane, int n, int ne, int off, int N) {
     constexpr int NW = NPAD / 32, CAP = SM::L::bk_cap;
+    const uint32_t cur = m.hdr()->spl_cur & 1u;
+    const float v_eq = __uint_as_float(m.hdr()->spl[k][cur][warp < NW - 1 ? warp : 0]);  // ne = 0 for the last warp
     float x[EPL];
 #pragma unroll
     for (int q = 0; q < EPL; ++q) {
         const int idx = lane * EPL + q;
-        x[q] = idx < n ? __uint_as_float(m.bk_keys()[warp * CAP + idx]) : INFINITY;
+        x[q] = idx < n ? __uint_as_float(m.bk_keys(k)[warp * CAP + idx]) : INFINITY;
     }
     warp_sort<EPL>(x, lane);
     double g = 0.0, s1 = 0.0, s2 = 0.0;
@@ -612,48 +656,58 @@ __device__ __forceinline__ void coin_bucket_sort(const SM& m, int warp, int lane
     for (int q = 0; q < EPL; ++q) {
         const int idx = lane * EPL + q;
         const double v = idx < n ? (double)x[q] : 0.0;
-        g += (double)(2 * (off + idx) - N + 1) * v;  // sum_k (2k - N + 1) c_(k)  (G23)
+        if (k == 0) g += (double)(2 * (off + idx) - N + 1) * v;  // sum_j (2j - N + 1) c_(j)  (G23)
         s1 += v;
         s2 += v * v;
     }
-    g = warp_sum(g); s1 = warp_sum(s1); s2 = warp_sum(s2);
-    if (lane == 0) { m.bk_part()[warp * 3 + 0] = g; m.bk_part()[warp * 3 + 1] = s1; m.bk_part()[warp * 3 + 2] = s2; }
-    // order statistics held by this bucket: lane b < NW - 1 looks for the bound of rank (b+1) N / NW, lanes 30 / 31
-    // ... the two median ranks are handled below (warp-uniform picks)
+    if (k == 0) g = warp_sum(g);
+    s1 = warp_sum(s1);
+    s2 = warp_sum(s2);
+    if (lane == 0) {
+        if (ne > 0) {  // ranks off+n .. off+n+ne-1 all hold v_eq
+            const double v = (double)v_eq, o = (double)(off + n), c = (double)ne;
+            g += v * (c * (2.0 * o - (double)N + 1.0) + c * (c - 1.0));
+            s1 += c * v;
+            s2 += c * v * v;
+        }
+        double* part = m.bk_part(k) + warp * 3;
+        part[0] = g; part[1] = s1; part[2] = s2;
+    }
+    // order statistics held by this warp: lane b < NW - 1 looks for next step's bound of rank (b+1) N / NW
     {
         const int want = lane < NW - 1 ? ((lane + 1) * N) / NW - off : -1;
-        const bool mine = want >= 0 && want < n;
-        const int src = mine ? want : 0;
+        const bool mine = want >= 0 && want < n + ne;
+        const int src = (mine && want < n) ? want : 0;
         float v = __shfl_sync(FULL, x[0], src / EPL);
 #pragma unroll
         for (int q = 1; q < EPL; ++q) {
             const float y = __shfl_sync(FULL, x[q], src / EPL);
             v = (src % EPL) == q ? y : v;
         }
-        if (mine) m.hdr()->coin_spl[lane] = __float_as_uint(v);
+        if (mine) m.hdr()->spl[k][cur ^ 1u][lane] = __float_as_uint(want < n ? v : v_eq);
     }
     const int r0 = (N >= 2 ? (N >> 1) - 1 : 0) - off, r1 = (N >> 1) - off;
-    if (r0 >= 0 && r0 < n) { const float v = warp_pick<EPL>(x, r0); if (lane == 0) m.bk_cnt()[33] = __float_as_uint(v); }
-    if (r1 >= 0 && r1 < n) { const float v = warp_pick<EPL>(x, r1); if (lane == 0) m.bk_cnt()[34] = __float_as_uint(v); }
+    if (r0 >= 0 && r0 < n + ne) { const float v = r0 < n ? warp_pick<EPL>(x, r0) : v_eq; if (lane == 0) m.bk_cnt(k)[65] = __float_as_uint(v); }
+    if (r1 >= 0 && r1 < n + ne) { const float v = r1 < n ? warp_pick<EPL>(x, r1) : v_eq; if (lane == 0) m.bk_cnt(k)[66] = __float_as_uint(v); }
 }
 
-// All warps: sort the own bucket.  Returns false (for every thread) if the buckets overflowed.
+// All warps: sort the own bucket of metric k.  Nothing to do if the buckets overflowed (the caller falls back).
 template <int NPAD, class SM>
-__device__ __forceinline__ bool coin_bucket_stats(const SM& m, int warp, int lane, int N) {
+__device__ __forceinline__ void bucket_stats(const SM& m, int k, int warp, int lane, int N) {
     constexpr int NW = NPAD / 32;
-    if (m.bk_cnt()[32]) return false;
-    const int mine = lane < NW ? (int)m.bk_cnt()[lane] : 0;
-    int incl = mine;
+    const uint32_t* cnt = m.bk_cnt(k);
+    if (cnt[64]) return;
+    const int nb = lane < NW ? (int)cnt[lane] : 0, neq = lane < NW - 1 ? (int)cnt[32 + lane] : 0;
+    int incl = nb + neq;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
         const int y = __shfl_up_sync(FULL, incl, o);
         if (lane >= o) incl += y;
     }
-    const int n = __shfl_sync(FULL, mine, warp), off = __shfl_sync(FULL, incl - mine, warp);
-    if (n <= 32) coin_bucket_sort<1, NPAD>(m, warp, lane, n, off, N);
-    else if (n <= 64) coin_bucket_sort<2, NPAD>(m, warp, lane, n, off, N);
-    else coin_bucket_sort<4, NPAD>(m, warp, lane, n, off, N);
-    return true;
+    const int n = __shfl_sync(FULL, nb, warp), ne = __shfl_sync(FULL, neq, warp), off = __shfl_sync(FULL, incl - nb - neq, warp);
+    if (n <= 32) bucket_sort<1, NPAD>(m, k, warp, lane, n, ne, off, N);
+    else if (n <= 64) bucket_sort<2, NPAD>(m, k, warp, lane, n, ne, off, N);
+    else bucket_sort<4, NPAD>(m, k, warp, lane, n, ne, off, N);
 }
 
 // Shared tail of the population rows: market statistics of the post-step books.
@@ -744,48 +798,63 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
 
     // ---- government statistics: metric k is owned by one warp (floats from warp 0 up, integer
     // metrics from the last warp down) ----
-    constexpr bool BKT = SM::L::bucketed;  // coin: every warp sorts one bucket (filled before the caller's barrier)
-    bool bk_ok = false;
-    if (BKT) bk_ok = coin_bucket_stats<NPAD>(m, warp, lane, N);
+    constexpr bool BKT = SM::L::bucketed;  // coin, labor, income: every warp sorts one bucket per metric (filled before the caller's barrier)
+    bool fell_back = false;  // some metric's buckets overflowed (the same answer in every thread)
+    if (BKT) {
 #pragma unroll 1
-    for (int k = warp; k < 3; k += NW)
-        if (!(BKT && k == 0)) metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
+        for (int k = 0; k < 3; ++k) {
+            fell_back = fell_back || m.bk_cnt(k)[64] != 0u;
+            bucket_stats<NPAD>(m, k, warp, lane, N);
+        }
+    } else {
+#pragma unroll 1
+        for (int k = warp; k < 3; k += NW) metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
+    }
 #pragma unroll 1
     for (int r = NW - 1 - warp; r < R; r += NW) int_metric_stats<EPL, NS, NT>(c, m, r, lane);
     if (tid < B + 2) m.govrow()[3 * n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
 
     if (any_obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    EJ_MARK(6);
     __syncthreads();
+    EJ_MARK(7);
 
-    if (BKT && warp == 0) {  // coin triple and welfare from the buckets' shares (or the single-warp sort)
-        if (bk_ok) {
-            double g = 0.0, s1 = 0.0, s2 = 0.0;
-            if (lane < NW) { g = m.bk_part()[lane * 3 + 0]; s1 = m.bk_part()[lane * 3 + 1]; s2 = m.bk_part()[lane * 3 + 2]; }
-            g = warp_sum(g); s1 = warp_sum(s1); s2 = warp_sum(s2);
-            if (lane == 0) {
-                const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
-                const double mean = s1 * inv_n;
-                double var = (s2 - s1 * mean) * inv_n;  // population variance from sum and sum of squares (binary64)
-                if (var < 0.0) var = 0.0;
-                gov_triple<NS, NT>(c, m, 0, mean, var, __uint_as_float(m.bk_cnt()[33]), __uint_as_float(m.bk_cnt()[34]), c.s_coin);
-                if (mode != 2) {
-                    const double ug = s1 - (double)c.omega * (g * inv_n);  // Eq.3-5 as in metric_stats
-                    if (mode == 0) {
-                        if (rew) rew[(uint32_t)(e * (N + 1) + N)] = (float)(ug - m.hdr()->u_g_prev);
-                        m.hdr()->u_g_prev = ug;
-                    } else if (rew) {
-                        rew[(uint32_t)(e * (N + 1) + N)] = 0.0f;
+    if (BKT && warp == 0) {  // the three triples and the welfare from the buckets' shares (or the single-warp sort)
+#pragma unroll 1
+        for (int k = 0; k < 3; ++k) {
+            uint32_t* cnt = m.bk_cnt(k);
+            if (!cnt[64]) {
+                double g = 0.0, s1 = 0.0, s2 = 0.0;
+                if (lane < NW) { const double* part = m.bk_part(k) + lane * 3; g = part[0]; s1 = part[1]; s2 = part[2]; }
+                g = warp_sum(g); s1 = warp_sum(s1); s2 = warp_sum(s2);
+                if (lane == 0) {
+                    const double inv_n = NT > 0 ? 1.0 / (double)(NT > 0 ? NT : 1) : c.inv_n;
+                    const double mean = s1 * inv_n;
+                    double var = (s2 - s1 * mean) * inv_n;  // population variance from sum and sum of squares (binary64)
+                    if (var < 0.0) var = 0.0;
+                    gov_triple<NS, NT>(c, m, k, mean, var, __uint_as_float(cnt[65]), __uint_as_float(cnt[66]), k == 1 ? c.s_labor : c.s_coin);
+                    if (k == 0 && mode != 2) {
+                        const double ug = s1 - (double)c.omega * (g * inv_n);  // Eq.3-5 as in metric_stats
+                        if (mode == 0) {
+                            if (rew) rew[(uint32_t)(e * (N + 1) + N)] = (float)(ug - m.hdr()->u_g_prev);
+                            m.hdr()->u_g_prev = ug;
+                        } else if (rew) {
+                            rew[(uint32_t)(e * (N + 1) + N)] = 0.0f;
+                        }
                     }
                 }
+            } else {
+                metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
             }
-        } else {
-            metric_stats<EPL, NS, NT>(c, m, 0, lane, mode, e, rew);
+            __syncwarp();
+            for (int i = lane; i < 72; i += 32) cnt[i] = 0u;  // empty buckets for the next step
         }
-        for (int i = lane; i < 36; i += 32) m.bk_cnt()[i] = 0u;  // empty buckets for the next step
+        if (lane == 0) m.hdr()->spl_cur ^= 1u;  // the bounds written during this step are in force from now on
         __syncwarp();
         if (any_obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
     }
+    if (BKT && fell_back) __syncthreads();  // the single-warp sort read the agents' state: nobody may start the next step before it is done
 
     if (any_obs && tid == 0) {  // bulk stores: the env's contiguous tile, (f2) its env-wide tail, its government row
         if (staged) {
@@ -1054,6 +1123,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
         if (invalid) atomicAdd(&m.hdr()->n_invalid, 1);
     }
     __syncthreads();  // #1 arrivals registered
+    EJ_MARK(1);
 
     // Arrival order of this step's candidates: (key, agent) (G11).  Each candidate finds its rank
     // among the step's arrivals on its level and its successor; with a book cap also its rank on
@@ -1168,6 +1238,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
         }
     }
     __syncthreads();  // #2 books hold this step's arrivals
+    EJ_MARK(2);
 
     // ---------------- P2 match + P3 expire (G14) ----------------
     // One thread per level.  Trades of a resource: q = max_p min(#bids >= p, #asks <= p); the
@@ -1227,6 +1298,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
         if (side == 0 && pidx == 0) m.resq()[r] = q;
     }
     __syncthreads();  // #3 matched lists complete
+    EJ_MARK(3);
 
     // settle trade i of resource r: bid rank i with ask rank i, at the price of the later arrival
     {
@@ -1261,6 +1333,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
         if (tid == 0) m.hdr()->n_trades += total;
     }
     __syncthreads();  // #4 credits complete
+    EJ_MARK(4);
 
     // income from sales (G16), coin credit once per agent
     if (act) {
@@ -1306,8 +1379,9 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
         }
     }
     if (tid < B && (boundary || first)) m.shrow()[5 * R + tid] = m.hdr()->rates[tid];
-    if (SM::L::bucketed) coin_bucket_fill<NPAD>(m, tid, act);  // the coin is final: file it for the block-wide sort
+    if (SM::L::bucketed) bucket_fill_all<NPAD>(m, tid, act);  // coin, labor, income are final: file them for the block-wide sort
     __syncthreads();  // #5 state final
+    EJ_MARK(5);
     if (tid == 0) {
         m.hdr()->t = t + 1;
         m.hdr()->t_in_period = period_end ? 0 : tp + 1;
@@ -1334,7 +1408,7 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
         if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
         if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
         if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
-        if (SM::L::bucketed) coin_bucket_fill<NPAD>(m, tid, tid < c.N);
+        if (SM::L::bucketed) bucket_fill_all<NPAD>(m, tid, tid < c.N);
         __syncthreads();
         mode = 1;
     } else {
@@ -1343,6 +1417,7 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
     // ---------------- P5 rewards, P6 observations ----------------
     outputs<NPAD, NS, RT, NT, BT, PF, FX>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs(), io.rew(), FX ? io.priv() : nullptr,
                                           FX ? io.shared() : nullptr, FX ? io.govp() : nullptr);
+    EJ_MARK(8);
     if (mode == 1) {
         if (tid == 0 && io.io.done) io.done()[e] = 1;
         __syncthreads();  // shrow is rewritten at the very start of the next finished step
@@ -1388,12 +1463,22 @@ __global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_
         "@p bra EJ_BLOB_DONE_%=;\n\tbra EJ_BLOB_WAIT_%=;\n\tEJ_BLOB_DONE_%=:\n\t}" ::"r"(bar)
         : "memory");
     StepPtrs p{io, c, 0, 0};
+#ifdef EJ_PHASE_CLOCK
+    if (blockIdx.x == 0 && tid == 0) { for (int k = 0; k < 16; ++k) ej_phase_cycles[k] = 0; ej_phase_last = clock64(); }
+#endif
 #pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
         p.s = s;
         env_step<NPAD, NS, RT, PT, NT, BT, PF, FX>(c, m, tid, e, p, s == 0);
         p.slot = (p.slot + 1 == io.ring_depth) ? 0 : p.slot + 1;
     }
+#ifdef EJ_PHASE_CLOCK
+    if (blockIdx.x == 0 && tid == 0 && io.n_steps > 1) {
+        printf("phase cycles per step over %d steps (thread 0 of block 0):", io.n_steps);
+        for (int k = 1; k <= 8; ++k) printf(" [%d] %.0f", k, (double)ej_phase_cycles[k] / io.n_steps);
+        printf("\n");
+    }
+#endif
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");  // this thread's state writes, for the bulk store below
     __syncthreads();
     if (tid == 0) {
@@ -1414,13 +1499,13 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     const Sm<NS> m{c};
     const uint4* blob = (const uint4*)(state + (size_t)e * c.blob_bytes);
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
-    if (Lay<NS>::bucketed && tid < 36) m.bk_cnt()[tid] = 0u;
+    if (Lay<NS>::bucketed && tid < 3 * 72) m.bk_cnt(0)[tid] = 0u;
     __syncthreads();
     const int t = m.hdr()->t;
     if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
     if (tid < c.B) m.shrow()[5 * c.R + tid] = m.hdr()->rates[tid];
     if (tid == NPAD - 1) write_timers(c, m, t, m.hdr()->t_in_period);
-    if (Lay<NS>::bucketed) coin_bucket_fill<NPAD>(m, tid, tid < c.N);
+    if (Lay<NS>::bucketed) bucket_fill_all<NPAD>(m, tid, tid < c.N);
     __syncthreads();
     outputs<NPAD, NS, 0, 0, 0, 0, 0>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
