@@ -290,20 +290,23 @@ float w2f(int32_t w) { float f; memcpy(&f, &w, 4); return f; }
 // ---- a12: policy networks ----
 int align128(int x) { return (x + 127) & ~127; }
 
-// Dynamic shared memory of ej_policy_kernel: weights once, then per group an A tile and the fp32 staging tile.
-int policy_group_bytes(const PolicyNet& n, int row_stride) {
+// Dynamic shared memory of ej_policy_kernel: weights once, then two slots per group.  A slot's buffer holds the
+// layer-1 operand (128 x K1p bf16) with the fp32 observation rows beside it, later the hidden activations (128 x 128 bf16).
+int policy_stage_off(const PolicyNet& n) { return align128(PTILE * n.K1p * 2); }
+int policy_slot_bytes(const PolicyNet& n, int row_stride) {
     const int a_cols = n.K1p > PH ? n.K1p : PH;
-    return align128(PTILE * a_cols * 2 + align16(PTILE * row_stride * 4));
+    const int hidden = PTILE * a_cols * 2, first = policy_stage_off(n) + align16(PTILE * row_stride * 4);
+    return align128(hidden > first ? hidden : first);
 }
 int policy_tmem_cols(const PolicyNet& n) { return n.Op > 128 ? 256 : 128; }
 int policy_groups(const PolicyNet& n, int row_stride) {
-    int g = P_TMEM_ALLOC / policy_tmem_cols(n);
-    const int fit = (227 * 1024 - align128(n.blob_bytes)) / policy_group_bytes(n, row_stride);
+    int g = P_TMEM_ALLOC / (2 * policy_tmem_cols(n));
+    const int fit = (227 * 1024 - align128(n.blob_bytes)) / (2 * policy_slot_bytes(n, row_stride));
     if (g > fit) g = fit;
     return g > PGROUPS ? PGROUPS : g;
 }
 int policy_smem_bytes(const PolicyNet& n, int row_stride) {
-    return align128(n.blob_bytes) + policy_groups(n, row_stride) * policy_group_bytes(n, row_stride);
+    return align128(n.blob_bytes) + policy_groups(n, row_stride) * 2 * policy_slot_bytes(n, row_stride);
 }
 
 // Repack a row-major [rows][cols] bf16 matrix into the canonical K-major no-swizzle UMMA layout
@@ -365,14 +368,13 @@ void fill_job(ej_env* h, PolicyArgs& a, const PolicyNet& net, const float* obs, 
     a.state = h->d_state; a.blob_stride = c.blob_bytes;
     a.env_id_base = c.env_id_base; a.seed_lo = c.seed_lo; a.seed_hi = c.seed_hi; a.stream_base = stream_base;
     a.actions = actions; a.logits = logits;
-    const int a_cols = net.K1p > PH ? net.K1p : PH;
     a.smem_W1 = 0;
     a.smem_W2 = a.smem_W1 + net.w1_bytes;
     a.smem_W3 = a.smem_W2 + net.w2_bytes;
     a.smem_bias = a.smem_W3 + net.w3_bytes;
     a.smem_group = align128(net.blob_bytes);
-    a.group_bytes = policy_group_bytes(net, row_stride);
-    a.stage_off = PTILE * a_cols * 2;
+    a.slot_bytes = policy_slot_bytes(net, row_stride);
+    a.stage_off = policy_stage_off(net);
     a.groups = policy_groups(net, row_stride);
     a.tmem_cols = policy_tmem_cols(net);
 }
@@ -402,12 +404,15 @@ int launch_policy(ej_env* h, const float* obs, int32_t* actions, int32_t* gov_ac
     int smem = policy_smem_bytes(h->pop_net, c.D_pop), gov_ctas = 0;
     if (gov_actions) {
         fill_job(h, pl.job[1], h->gov_net, obs + c.gov_obs_offset, c.D_gov_pad, c.E, 1, c.N, 1u, gov_actions, gov_logits);
-        gov_ctas = ctas_for(pl.job[1], h->n_sms / 8 > 0 ? h->n_sms / 8 : 1);
+        // a government tile costs several population tiles (one categorical per bracket): two tiles per CTA, both in
+        // flight at once, end well before the population CTAs do and take fewer SMs away from them than one tile each
+        const int gov_tiles = (c.E + PTILE - 1) / PTILE;
+        gov_ctas = ctas_for(pl.job[1], (gov_tiles + 1) / 2);
         const int sg = policy_smem_bytes(h->gov_net, c.D_gov_pad);
         if (sg > smem) smem = sg;
     }
     pl.split = ctas_for(pl.job[0], h->n_sms - gov_ctas);
-    ej_policy_kernel<<<pl.split + gov_ctas, PGROUPS * PTILE, smem, h->stream>>>(pl);
+    ej_policy_kernel<<<pl.split + gov_ctas, P_THREADS, smem, h->stream>>>(pl);
     h->launches++;
     EJ_CUDA(h, cudaGetLastError(), "ej_policy_kernel launch");
     return EJ_OK;

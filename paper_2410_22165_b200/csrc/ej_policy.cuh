@@ -3,16 +3,13 @@
 // Table 2) on the 5th-generation tensor cores, followed by categorical sampling with
 // the counter-based Philox of G30 (G33).
 //
-// One CTA of 128 threads works on tiles of 128 observation rows (thread i = row i = TMEM lane
-// i).  The three weight matrices stay resident in shared memory in the canonical K-major
-// no-swizzle UMMA layout (8-row x 16-byte core matrices); the activation tile is rebuilt in the
-// same layout between layers.  Each layer is a chain of tcgen05.mma (M=128, N=128|Op, K=16)
-// issued by one thread, accumulating in TMEM; completion comes back through tcgen05.commit on
-// an mbarrier; the epilogue reads its row with tcgen05.ld, adds the bias, applies tanh, rounds
-// to bf16 and writes the next layer's A operand.  One CTA per SM holds the weights once and runs
-// TWO such 128-thread groups on alternating tiles (own A tile, own half of TMEM, own named
-// barrier), so one group's epilogue overlaps the other's MMAs; the fp32 observation tile of the
-// group's next tile is prefetched by a 1-D TMA bulk copy (cp.async.bulk) while it computes.
+// Groups of 128 threads work on tiles of 128 observation rows (thread i = row i = TMEM lane i).  The three weight
+// matrices stay resident in shared memory in the canonical K-major no-swizzle UMMA layout (8-row x 16-byte core
+// matrices); the activation tile is rebuilt in the same layout between layers.  Each layer is a chain of
+// tcgen05.mma (M=128, N=128|Op, K=16) issued by one thread, accumulating in TMEM; completion comes back through
+// tcgen05.commit on an mbarrier; the epilogue reads its row with tcgen05.ld, adds the bias, applies tanh, rounds
+// to bf16 and writes the next layer's A operand.  One CTA per SM holds the weights once and runs two such groups;
+// every group keeps two tiles in flight so that one tile's epilogue overlaps the other's MMAs (see ej_policy_kernel).
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -23,7 +20,8 @@ namespace {
 constexpr int PH = 128;        // hidden width (B:configs[4]: 128 -> 128)
 constexpr int PTILE = 128;     // rows per tile = UMMA M
 constexpr int P_TMEM_ALLOC = 512;  // whole TMEM of the SM (one CTA per SM); group g uses columns [g * tmem_cols, ...)
-constexpr int PGROUPS = 3;         // 128-thread groups per CTA (a job may use fewer)
+constexpr int P_THREADS = 2 * 128 + 2 * 32;  // two row groups + one MMA-issuer warp per group
+constexpr int PGROUPS = 2;         // 128-thread groups per CTA (a job may use fewer); every group keeps two tiles in flight
 
 struct PolicyNet {
     const uint8_t* blob;   // device: W1 | W2 | W3 (canonical bf16) | b1 | b2 | b3 (f32)
@@ -59,8 +57,8 @@ struct PolicyArgs {
     int32_t* actions;        // [rows][n_heads]
     float* logits;           // [rows][n_out] or null
     int smem_W1, smem_W2, smem_W3, smem_bias;  // byte offsets in dynamic shared memory (shared by both groups)
-    int smem_group, group_bytes, stage_off;     // group g: A tile at smem_group + g * group_bytes, fp32 staging at + stage_off
-    int groups, tmem_cols;   // active groups of this job (<= PGROUPS) and TMEM columns per group (128 or 256)
+    int smem_group, slot_bytes, stage_off;      // slot s of group g: operand buffer at smem_group + (2 g + s) * slot_bytes, fp32 rows at + stage_off
+    int groups, tmem_cols;   // active groups of this job (<= PGROUPS) and TMEM columns per slot (128 or 256)
 };
 
 // One launch runs up to two jobs side by side: CTAs [0, split) work on job 0 (population),
@@ -140,15 +138,19 @@ __device__ __forceinline__ uint32_t op_off(int row, int k, int kp) {
     return (uint32_t)((row & 7) * 16 + (row >> 3) * (kp * 16) + (k >> 3) * 128 + (k & 7) * 2);
 }
 
-// Issue one layer: D[128 x n] (+)= A[128 x kp] * W[n x kp]^T, then commit to the mbarrier.
+// Issue one layer: D[128 x n] (+)= A[128 x kp] * W[n x kp]^T, then commit to the mbarrier.  The descriptors of
+// successive K steps differ in the start-address field only (+256 B = +16 in units of 16 B): one add per step.
 __device__ __forceinline__ void issue_layer(uint32_t a_addr, uint32_t w_addr, int kp, int n, uint32_t tmem_d, uint32_t bar) {
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
     const uint32_t idesc = umma_idesc(n);
     const uint32_t sbo = (uint32_t)kp * 16u;  // (kp / 8) core matrices of 128 B per 8-row group
-    for (int k = 0; k < kp / 16; ++k) {
-        const uint64_t da = umma_desc(a_addr + k * 256, 128, sbo);
-        const uint64_t db = umma_desc(w_addr + k * 256, 128, sbo);
-        umma_bf16(tmem_d, da, db, idesc, k > 0 ? 1u : 0u);
+    uint64_t da = umma_desc(a_addr, 128, sbo), db = umma_desc(w_addr, 128, sbo);
+    umma_bf16(tmem_d, da, db, idesc, 0u);
+#pragma unroll 1
+    for (int k = 1; k < kp / 16; ++k) {
+        da += 16u;
+        db += 16u;
+        umma_bf16(tmem_d, da, db, idesc, 1u);
     }
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" ::"r"(bar) : "memory");
 }
@@ -166,28 +168,60 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
     asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
 }
 
+__device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];\n"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+          "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
+          "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
+          "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+}
+
 // Hidden-layer epilogue: this thread's accumulator row -> +bias -> tanh -> bf16 -> A operand (kp = 128).
-__device__ __forceinline__ void hidden_epilogue(uint32_t taddr_row, const float* bias, uint8_t* A, int row) {
-    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-#pragma unroll 1
-    for (int c = 0; c < PH; c += 32) {
-        uint32_t r[32];
-        tmem_ld32(taddr_row + c, r);
+// The special-function unit (16 tanh per clock and SM) bounds this phase and only two or three warps share a
+// scheduler, so a warp must keep the unit fed by itself: the row is handled 32 columns at a time in STAGES -- all
+// bias adds, then 32 tanh back to back, then the packing -- and the accumulators of the next two chunks are already
+// on their way from TMEM (tcgen05.wait::ld waits for every load in flight, hence chunks travel in pairs).  Out of
+// line: compiled on its own, ptxas keeps this order; inlined into the kernel it paired every tanh with its pack.
+__device__ __forceinline__ void epilogue_chunk(const uint32_t (&r)[32], const float* bias, uint8_t* A, int row, int c) {
+    float v[32];
 #pragma unroll
-        for (int g = 0; g < 4; ++g) {
-            uint32_t w[4];
-            const float4 bl = *reinterpret_cast<const float4*>(bias + c + g * 8), bh = *reinterpret_cast<const float4*>(bias + c + g * 8 + 4);
-            const float bb[8] = {bl.x, bl.y, bl.z, bl.w, bh.x, bh.y, bh.z, bh.w};
-#pragma unroll
-            for (int j = 0; j < 4; ++j) {
-                const int k = g * 8 + 2 * j;
-                const float a0 = tanh_fast(__uint_as_float(r[k]) + bb[2 * j]), a1 = tanh_fast(__uint_as_float(r[k + 1]) + bb[2 * j + 1]);
-                const __nv_bfloat162 h = __floats2bfloat162_rn(a0, a1);
-                w[j] = *reinterpret_cast<const uint32_t*>(&h);
-            }
-            *reinterpret_cast<uint4*>(A + op_off(row, c + g * 8, PH)) = make_uint4(w[0], w[1], w[2], w[3]);
-        }
+    for (int g = 0; g < 8; ++g) {
+        const float4 b4 = *reinterpret_cast<const float4*>(bias + c + g * 4);
+        v[4 * g] = __uint_as_float(r[4 * g]) + b4.x;
+        v[4 * g + 1] = __uint_as_float(r[4 * g + 1]) + b4.y;
+        v[4 * g + 2] = __uint_as_float(r[4 * g + 2]) + b4.z;
+        v[4 * g + 3] = __uint_as_float(r[4 * g + 3]) + b4.w;
     }
+#pragma unroll
+    for (int k = 0; k < 32; ++k) v[k] = tanh_fast(v[k]);
+#pragma unroll
+    for (int g = 0; g < 4; ++g) {
+        uint32_t w[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const __nv_bfloat162 h = __floats2bfloat162_rn(v[g * 8 + 2 * j], v[g * 8 + 2 * j + 1]);
+            w[j] = *reinterpret_cast<const uint32_t*>(&h);
+        }
+        *reinterpret_cast<uint4*>(A + op_off(row, c + g * 8, PH)) = make_uint4(w[0], w[1], w[2], w[3]);
+    }
+}
+__device__ __noinline__ void hidden_epilogue(uint32_t taddr_row, const float* bias, uint8_t* A, int row) {
+    asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    uint32_t r0[32], r1[32], r2[32], r3[32];
+    tmem_ld32_nowait(taddr_row, r0);
+    tmem_ld32_nowait(taddr_row + 32, r1);
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+    tmem_ld32_nowait(taddr_row + 64, r2);
+    tmem_ld32_nowait(taddr_row + 96, r3);
+    epilogue_chunk(r0, bias, A, row, 0);
+    epilogue_chunk(r1, bias, A, row, 32);
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+    epilogue_chunk(r2, bias, A, row, 64);
+    epilogue_chunk(r3, bias, A, row, 96);
 }
 
 template <int OFF, int LEN>
@@ -265,6 +299,92 @@ __device__ __forceinline__ int sample_head(uint32_t taddr_row, const float* b3, 
     pick = pick < 0 ? 0 : pick;
     return pick > last ? last : pick;
 }
+
+__device__ __forceinline__ float ex2_fast(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// The population head when its width NL is a compile-time constant (one head, columns 0 .. NL-1): the row of
+// logits is read once, and every later pass (bias, maximum, exponentials, sum, cumulative count) touches exactly
+// the NL live columns -- about 8 instructions per logit where the general window sampler spends 17.
+template <int NL>
+__device__ __forceinline__ int sample_single_head(uint32_t taddr_row, const float* b3, float u, float* logits_row) {
+    constexpr int NCH = (NL + 15) / 16;
+    float l[NCH * 16];
+    load_window<0, NCH>(taddr_row, 0, NCH * 16, l);
+    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+    float m4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};  // four running maxima: short dependence chains
+#pragma unroll
+    for (int q = 0; q < (NL + 3) / 4; ++q) {
+        const float4 b = *reinterpret_cast<const float4*>(b3 + 4 * q);  // b3 is padded to a multiple of 16 floats
+        const float bb[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            if (4 * q + j < NL) {
+                l[4 * q + j] += bb[j];
+                m4[j] = fmaxf(m4[j], l[4 * q + j]);
+            }
+        }
+    }
+    const float mx = fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
+    if (logits_row) {
+#pragma unroll
+        for (int k = 0; k < NL; ++k) logits_row[k] = l[k];
+    }
+    const float mneg = -mx * 1.4426950408889634f;
+#pragma unroll
+    for (int k = 0; k < NL; ++k) l[k] = ex2_fast(__fmaf_rn(l[k], 1.4426950408889634f, mneg));  // exp(l - max)
+    // running sums in the order of the definition (left to right, never reassociated); the total is the last one,
+    // and the sampled index = number of running sums <= u * total: 65 independent compares, no second chain
+#pragma unroll
+    for (int k = 1; k < NL; ++k) l[k] += l[k - 1];
+    const float target = u * l[NL - 1];
+    int below = 0;
+#pragma unroll
+    for (int k = 0; k < NL; ++k) below += (l[k] <= target) ? 1 : 0;
+    return below > NL - 1 ? NL - 1 : below;
+}
+
+// Several equal heads whose count and width are compile-time constants (the government's B = 7 brackets of L = 21
+// rate levels): head H covers the columns [H * HEAD, (H + 1) * HEAD); its 16-column chunks and every register
+// index are known at compile time, so each head costs what sample_single_head costs per logit.  The general window
+// sampler (runtime bounds, masked padding columns, exp2f) made a government tile several times as expensive as a
+// population tile, and the few government CTAs the tail of the whole launch.
+template <int H, int NH, int HEAD>
+struct HeadSampler {
+    template <class PH_>
+    __device__ __forceinline__ static void run(uint32_t taddr_row, const float* b3, float* logits_row, int32_t* out, bool live, PH_&& next_u) {
+        constexpr int LO = H * HEAD, HI = LO + HEAD, C0 = LO & ~15, NCH = (HI - C0 + 15) / 16;
+        float l[NCH * 16];
+        load_window<0, NCH>(taddr_row, C0, C0 + NCH * 16, l);
+        const float u = next_u(H);
+        asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+        float m4[4] = {-INFINITY, -INFINITY, -INFINITY, -INFINITY};
+#pragma unroll
+        for (int k = LO - C0; k < HI - C0; ++k) {
+            l[k] += b3[C0 + k];
+            m4[k & 3] = fmaxf(m4[k & 3], l[k]);
+        }
+        const float mx = fmaxf(fmaxf(m4[0], m4[1]), fmaxf(m4[2], m4[3]));
+        if (logits_row) {
+#pragma unroll
+            for (int k = LO - C0; k < HI - C0; ++k) logits_row[C0 + k] = l[k];
+        }
+        const float mneg = -mx * 1.4426950408889634f;
+#pragma unroll
+        for (int k = LO - C0; k < HI - C0; ++k) l[k] = ex2_fast(__fmaf_rn(l[k], 1.4426950408889634f, mneg));
+#pragma unroll
+        for (int k = LO - C0 + 1; k < HI - C0; ++k) l[k] += l[k - 1];  // running sums, left to right
+        const float target = u * l[HI - C0 - 1];
+        int below = 0;
+#pragma unroll
+        for (int k = LO - C0; k < HI - C0; ++k) below += (l[k] <= target) ? 1 : 0;
+        if (live) out[H] = below > HEAD - 1 ? HEAD - 1 : below;
+        if constexpr (H + 1 < NH) HeadSampler<H + 1, NH, HEAD>::run(taddr_row, b3, logits_row, out, live, next_u);
+    }
+};
 
 // Fallback for heads wider than 80 logits: three sweeps over the TMEM row (maximum; sum of
 // exp(l - max); first index whose cumulative weight exceeds u * sum).
@@ -405,49 +525,52 @@ __device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint3
                  : "memory");
 }
 
-__global__ void __launch_bounds__(PGROUPS* PTILE, 1) ej_policy_kernel(const __grid_constant__ PolicyLaunch pl) {
+// The kernel.  A CTA holds the three weight matrices once and runs PGROUPS groups of 128 threads (thread = row =
+// TMEM lane).  Every group keeps TWO tiles in flight (slots 0 and 1: own operand buffer, own TMEM accumulator
+// columns, own mbarriers) and works through them phase by phase -- operand build, tanh epilogue 1, tanh epilogue 2,
+// sampling -- first for slot 0, then for slot 1: while the threads run one slot's epilogue on the special-function
+// unit, the tensor cores run the other slot's MMAs, so a group never sits on an MMA wait (the first version ran one
+// tile per group and three groups in step: 45 % of a tile's time was operand builds and MMA waits with the
+// special-function unit idle, profiles/r2d).  A slot's buffer holds, in turn, the fp32 observation rows (1-D TMA bulk
+// copy, issued as soon as the slot's last MMA is done, so it lands under the sampling), the layer-1 operand built
+// from them (beside the rows), then the hidden activations (over both).
+__global__ void __launch_bounds__(P_THREADS, 1) ej_policy_kernel(const __grid_constant__ PolicyLaunch pl) {
     const bool second = (int)blockIdx.x >= pl.split;
     const PolicyArgs& a = second ? pl.job[1] : pl.job[0];
     const int bid = second ? (int)blockIdx.x - pl.split : (int)blockIdx.x, nblk = second ? (int)gridDim.x - pl.split : pl.split;
     extern __shared__ __align__(128) uint8_t psm[];
-    __shared__ __align__(8) unsigned long long mbar_mma[PGROUPS], mbar_tma[PGROUPS];
+    __shared__ __align__(8) unsigned long long mbar_mma[PGROUPS][2], mbar_tma[PGROUPS][2], mbar_rdy[PGROUPS][2], mbar_w;
     __shared__ uint32_t tmem_slot;
-    const int tid = threadIdx.x, warp = tid >> 5, grp = tid >> 7, gtid = tid & (PTILE - 1);
+    const int tid = threadIdx.x, warp = tid >> 5, gtid = tid & (PTILE - 1);
+    const bool issuer = tid >= PGROUPS * PTILE;                       // warps 8, 9: MMA issuers of groups 0, 1
+    const int grp = issuer ? (tid - PGROUPS * PTILE) >> 5 : tid >> 7;
     const PolicyNet& n = a.net;
-    uint8_t* A = psm + a.smem_group + grp * a.group_bytes;
-    const float* stage = reinterpret_cast<const float*>(A + a.stage_off);
     const float* b1 = reinterpret_cast<const float*>(psm + a.smem_bias);
     const float* b2 = b1 + PH;
     const float* b3 = b2 + PH;
 
-    // ---- one-time setup: weights to shared memory (once per SM), mbarriers, TMEM ----
-    {
-        const uint4* src = reinterpret_cast<const uint4*>(n.blob);
-        uint4* dst = reinterpret_cast<uint4*>(psm + a.smem_W1);  // W1 | W2 | W3 | biases are contiguous in both
-        for (int i = tid; i < n.blob_bytes / 16; i += PGROUPS * PTILE) dst[i] = src[i];
-    }
+    // ---- one-time setup: weights to shared memory (once per SM, one TMA bulk copy), mbarriers, TMEM ----
     if (tid == 0) {
-        for (int g = 0; g < PGROUPS; ++g) {
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(&mbar_mma[g])) : "memory");
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(&mbar_tma[g])) : "memory");
-        }
+        for (int g = 0; g < PGROUPS; ++g)
+            for (int sl = 0; sl < 2; ++sl) {
+                asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(&mbar_mma[g][sl])) : "memory");
+                asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(&mbar_tma[g][sl])) : "memory");
+                asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;\n" ::"r"(smem_u32(&mbar_rdy[g][sl])), "r"(PTILE) : "memory");
+            }
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;\n" ::"r"(smem_u32(&mbar_w)) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;\n" ::: "memory");
+        tma_load_1d(smem_u32(psm + a.smem_W1), n.blob, (uint32_t)n.blob_bytes, smem_u32(&mbar_w));  // W1 | W2 | W3 | biases, contiguous in both
     }
     if (warp == 0) {
         asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(&tmem_slot)), "r"(P_TMEM_ALLOC) : "memory");
         asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
     }
-    asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");  // weights were written by the generic proxy
     asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
     __syncthreads();
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+    mbar_wait(smem_u32(&mbar_w), 0);  // the weights have landed (async proxy: visible to the MMAs and, after this wait, to every thread)
     const uint32_t tmem_base = tmem_slot;
-    const uint32_t tmem = tmem_base + (uint32_t)(grp * a.tmem_cols);           // this group's columns
-    const uint32_t taddr_row = tmem + ((uint32_t)((warp & 3) * 32) << 16);     // this warp's 32 lanes
-    const uint32_t bar = smem_u32(&mbar_mma[grp]), tbar = smem_u32(&mbar_tma[grp]);
-    const uint32_t a_addr = smem_u32(A), stage_addr = smem_u32(stage), w1_addr = smem_u32(psm + a.smem_W1),
-                   w2_addr = smem_u32(psm + a.smem_W2), w3_addr = smem_u32(psm + a.smem_W3);
-    uint32_t phase = 0, tphase = 0;
+    const uint32_t w1_addr = smem_u32(psm + a.smem_W1), w2_addr = smem_u32(psm + a.smem_W2), w3_addr = smem_u32(psm + a.smem_W3);
 
     const int n_tiles = (a.rows + PTILE - 1) / PTILE;
     const int tile_step = nblk * a.groups;
@@ -456,94 +579,169 @@ __global__ void __launch_bounds__(PGROUPS* PTILE, 1) ej_policy_kernel(const __gr
     auto tile_bytes = [&](int tile) { return (uint32_t)(tile_rows(tile) * a.row_stride * 4); };
     auto tile_src = [&](int tile) { return a.obs + (size_t)tile * PTILE * a.row_stride; };
     auto tma_ok = [&](int tile) { return ((reinterpret_cast<uintptr_t>(tile_src(tile)) | tile_bytes(tile)) & 15u) == 0; };
-    int tile = grp < a.groups ? bid * a.groups + grp : n_tiles;  // surplus groups idle
-    if (tile < n_tiles && gtid == 0 && tma_ok(tile)) tma_load_1d(stage_addr, tile_src(tile), tile_bytes(tile), tbar);
 
-    for (; tile < n_tiles; tile += tile_step) {
-        const int row0 = tile * PTILE, nrows = tile_rows(tile);
-        // ---- observation tile (fp32, staged) -> bf16 A operand (K1p columns, zero padded) ----
-        if (tma_ok(tile)) {
-            mbar_wait(tbar, tphase);
-            tphase ^= 1;
-        } else {  // unaligned tile: plain coalesced copy by the group
-            float* st = const_cast<float*>(stage);
-            const float* src = tile_src(tile);
-            for (int i = gtid; i < nrows * a.row_stride; i += PTILE) st[i] = src[i];
-            group_sync(grp);
-        }
-        {
-            const float* my = stage + gtid * a.row_stride;
-            for (int kc = 0; kc < n.K1p / 8; ++kc) {
-                uint32_t w[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int k = kc * 8 + 2 * j;
-                    const float v0 = (gtid < nrows && k < n.D_in) ? my[k] : 0.0f;
-                    const float v1 = (gtid < nrows && k + 1 < n.D_in) ? my[k + 1] : 0.0f;
-                    const __nv_bfloat162 h = __floats2bfloat162_rn(v0, v1);
-                    w[j] = *reinterpret_cast<const uint32_t*>(&h);
+    // per-slot state of this group
+    uint8_t* const gbase = psm + a.smem_group + grp * (2 * a.slot_bytes);
+    int tile[2];
+    int t_env[2] = {0, 0};  // clock of the row's env (Philox counter), fetched while the slot's operand is built
+    uint32_t ph_mma[2] = {0u, 0u}, ph_tma[2] = {0u, 0u};
+    auto slotA = [&](int sl) { return gbase + sl * a.slot_bytes; };
+    auto slotStage = [&](int sl) { return reinterpret_cast<float*>(gbase + sl * a.slot_bytes + a.stage_off); };
+    auto slotTmem = [&](int sl) { return tmem_base + (uint32_t)((grp * 2 + sl) * a.tmem_cols); };
+    auto rowTmem = [&](int sl) { return slotTmem(sl) + ((uint32_t)((warp & 3) * 32) << 16); };  // this warp's 32 lanes
+    auto barM = [&](int sl) { return smem_u32(&mbar_mma[grp][sl]); };
+    auto barT = [&](int sl) { return smem_u32(&mbar_tma[grp][sl]); };
+    const int first = grp < a.groups ? bid * a.groups + grp : n_tiles;  // surplus groups idle
+    tile[0] = first;
+    tile[1] = first < n_tiles ? first + tile_step : n_tiles;
+    auto barR = [&](int sl) { return smem_u32(&mbar_rdy[grp][sl]); };
+    if (issuer) {
+        // MMA-issuer warp of group `grp`: one lane waits for "operand ready" (all 128 rows of the group have written and
+        // fenced their part) and issues the layer's MMAs, in the order in which the group produces operands.  The row
+        // threads never wait for the tensor pipe to accept an instruction; they only wait for results.
+        if ((tid & 31) == 0) {
+            uint32_t ph_rdy[2] = {0u, 0u};
+            while (tile[0] < n_tiles) {
+#pragma unroll 1
+                for (int stage_i = 0; stage_i < 3; ++stage_i) {
+#pragma unroll 1
+                    for (int sl = 0; sl < 2; ++sl) {
+                        if (tile[sl] >= n_tiles) break;
+                        mbar_wait(barR(sl), ph_rdy[sl]);
+                        ph_rdy[sl] ^= 1u;
+                        const uint32_t a_addr = smem_u32(slotA(sl));
+                        if (stage_i == 0) issue_layer(a_addr, w1_addr, n.K1p, PH, slotTmem(sl), barM(sl));
+                        else if (stage_i == 1) issue_layer(a_addr, w2_addr, PH, PH, slotTmem(sl), barM(sl));
+                        else issue_layer(a_addr, w3_addr, PH, n.Op, slotTmem(sl), barM(sl));
+                    }
                 }
-                *reinterpret_cast<uint4*>(A + op_off(gtid, kc * 8, n.K1p)) = make_uint4(w[0], w[1], w[2], w[3]);
+                tile[0] += 2 * tile_step;
+                tile[1] += 2 * tile_step;
             }
         }
-        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        group_sync(grp);
-        if (gtid == 0) {
-            issue_layer(a_addr, w1_addr, n.K1p, PH, tmem, bar);
-            const int next = tile + tile_step;  // the staging buffer is free: prefetch the group's next tile
-            if (next < n_tiles && tma_ok(next)) tma_load_1d(stage_addr, tile_src(next), tile_bytes(next), tbar);
-        }
-        mbar_wait(bar, phase);
-        phase ^= 1;
-        hidden_epilogue(taddr_row, b1, A, gtid);
-        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        group_sync(grp);
-        if (gtid == 0) issue_layer(a_addr, w2_addr, PH, PH, tmem, bar);
-        mbar_wait(bar, phase);
-        phase ^= 1;
-        hidden_epilogue(taddr_row, b2, A, gtid);
-        asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
-        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        group_sync(grp);
-        if (gtid == 0) issue_layer(a_addr, w3_addr, PH, n.Op, tmem, bar);
-        mbar_wait(bar, phase);
-        phase ^= 1;
-        asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+        tile[0] = tile[1] = n_tiles;  // skip the row-group code below
+    }
+#pragma unroll
+    for (int sl = 0; sl < 2; ++sl)
+        if (tile[sl] < n_tiles && gtid == 0 && tma_ok(tile[sl])) tma_load_1d(smem_u32(slotStage(sl)), tile_src(tile[sl]), tile_bytes(tile[sl]), barT(sl));
 
-        // ---- logits -> softmax -> inverse-CDF sample per head (G33) ----
-        const int row = row0 + gtid;
-        const bool live = gtid < nrows;
-        const int env = live ? row / a.rows_per_env : 0;
-        const int agent = a.fixed_agent >= 0 ? a.fixed_agent : row - env * a.rows_per_env;
-        const int t = live ? *reinterpret_cast<const int*>(a.state + (size_t)env * a.blob_stride) : 0;
-        uint32_t x[4] = {0, 0, 0, 0};
-        for (int h = 0; h < n.n_heads; ++h) {
-            if ((h & 3) == 0)
-                philox4x32_10(a.env_id_base + (uint32_t)env, (uint32_t)agent, (uint32_t)t, a.stream_base + (uint32_t)(h >> 2), a.seed_lo,
-                              a.seed_hi, x[0], x[1], x[2], x[3]);
-            const uint32_t xw = (h & 3) == 0 ? x[0] : (h & 3) == 1 ? x[1] : (h & 3) == 2 ? x[2] : x[3];
-            const float u = u01(xw);
-            const int lo = h * n.head, hi = lo + n.head;
-            float* lrow = (a.logits && live) ? a.logits + (size_t)row * n.n_out : nullptr;
-            int pick;
-            if (a.mask.on) {  // f1: single-head population job (uniform over the CTA)
-                pick = sample_head_masked(taddr_row, b3, n.n_out, u, lrow, a.mask, a.state + (size_t)env * a.blob_stride, agent);
-            } else
-            switch (n.nch) {
-                case 1: pick = sample_head<1>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
-                case 2: pick = sample_head<2>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
-                case 3: pick = sample_head<3>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
-                case 4: pick = sample_head<4>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
-                case 5: pick = sample_head<5>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
-                default: pick = sample_head_sweeps(taddr_row, b3, lo, hi, u, lrow); break;
+    while (tile[0] < n_tiles) {
+        // ---- observation rows (fp32, staged) -> bf16 layer-1 operand (K1p columns, zero padded); layer-1 MMAs ----
+#pragma unroll 1
+        for (int sl = 0; sl < 2; ++sl) {
+            if (tile[sl] >= n_tiles) break;
+            const int nrows = tile_rows(tile[sl]);
+            uint8_t* A = slotA(sl);
+            float* stage = slotStage(sl);
+            if (tma_ok(tile[sl])) {
+                mbar_wait(barT(sl), ph_tma[sl]);
+                ph_tma[sl] ^= 1u;
+            } else {  // unaligned tile: plain coalesced copy by the group
+                const float* src = tile_src(tile[sl]);
+                for (int i = gtid; i < nrows * a.row_stride; i += PTILE) stage[i] = src[i];
+                group_sync(grp);
             }
-            if (live) a.actions[(size_t)row * n.n_heads + h] = pick;
+            {   // the sampler's Philox counter needs the env's clock: a global load, issued a whole tile ahead of its use
+                const int row = tile[sl] * PTILE + gtid;
+                t_env[sl] = gtid < nrows ? *reinterpret_cast<const int*>(a.state + (size_t)(row / a.rows_per_env) * a.blob_stride) : 0;
+            }
+            const float* my = stage + gtid * a.row_stride;
+            const bool in_tile = gtid < nrows;
+            for (int k0 = 0; k0 < n.K1p; k0 += 48) {  // 48 columns at a time: all loads in flight before the first conversion
+                float v[48];
+#pragma unroll
+                for (int j = 0; j < 48; ++j) v[j] = (in_tile && k0 + j < n.D_in) ? my[k0 + j] : 0.0f;  // zero padding, rows beyond the tile
+#pragma unroll
+                for (int c8 = 0; c8 < 6; ++c8) {
+                    if (k0 + c8 * 8 < n.K1p) {
+                        uint32_t w[4];
+#pragma unroll
+                        for (int j = 0; j < 4; ++j) {
+                            const __nv_bfloat162 h = __floats2bfloat162_rn(v[c8 * 8 + 2 * j], v[c8 * 8 + 2 * j + 1]);
+                            w[j] = *reinterpret_cast<const uint32_t*>(&h);
+                        }
+                        *reinterpret_cast<uint4*>(A + op_off(gtid, k0 + c8 * 8, n.K1p)) = make_uint4(w[0], w[1], w[2], w[3]);
+                    }
+                }
+            }
+            asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+            asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+            // operand written and fenced; this thread has also finished sampling the slot's previous tile (TMEM columns reused)
+            asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(barR(sl)) : "memory");
         }
-        // the next tile's MMAs overwrite these TMEM columns and the A tile
-        asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
-        group_sync(grp);
+        // ---- hidden layers: tanh epilogue of one slot under the MMAs of the other ----
+#pragma unroll 1
+        for (int layer = 0; layer < 2; ++layer) {
+#pragma unroll 1
+            for (int sl = 0; sl < 2; ++sl) {
+                if (tile[sl] >= n_tiles) break;
+                uint8_t* A = slotA(sl);
+                mbar_wait(barM(sl), ph_mma[sl]);
+                ph_mma[sl] ^= 1u;
+                hidden_epilogue(rowTmem(sl), layer == 0 ? b1 : b2, A, gtid);
+                asm volatile("fence.proxy.async.shared::cta;\n" ::: "memory");
+                asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+                asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(barR(sl)) : "memory");
+            }
+        }
+        // ---- logits -> softmax -> inverse-CDF sample per head (G33) ----
+#pragma unroll 1
+        for (int sl = 0; sl < 2; ++sl) {
+            if (tile[sl] >= n_tiles) break;
+            const int cur = tile[sl], nrows = tile_rows(cur);
+            const uint32_t taddr_row = rowTmem(sl);
+            mbar_wait(barM(sl), ph_mma[sl]);
+            ph_mma[sl] ^= 1u;
+            asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
+            // the slot's operand buffer is free: fetch the observation rows of its next tile under the sampling
+            tile[sl] = cur + 2 * tile_step;
+            if (tile[sl] < n_tiles && gtid == 0 && tma_ok(tile[sl]))
+                tma_load_1d(smem_u32(slotStage(sl)), tile_src(tile[sl]), tile_bytes(tile[sl]), barT(sl));
+            const int row = cur * PTILE + gtid;
+            const bool live = gtid < nrows;
+            const int env = live ? row / a.rows_per_env : 0;
+            const int agent = a.fixed_agent >= 0 ? a.fixed_agent : row - env * a.rows_per_env;
+            const int t = t_env[sl];
+            uint32_t x[4] = {0, 0, 0, 0};
+            if (!a.mask.on && n.n_heads == 7 && n.head == 21) {  // the government's 7 brackets x 21 levels
+                float* lrow = (a.logits && live) ? a.logits + (size_t)row * n.n_out : nullptr;
+                auto next_u = [&](int h) {
+                    if ((h & 3) == 0)
+                        philox4x32_10(a.env_id_base + (uint32_t)env, (uint32_t)agent, (uint32_t)t, a.stream_base + (uint32_t)(h >> 2), a.seed_lo,
+                                      a.seed_hi, x[0], x[1], x[2], x[3]);
+                    return u01((h & 3) == 0 ? x[0] : (h & 3) == 1 ? x[1] : (h & 3) == 2 ? x[2] : x[3]);
+                };
+                HeadSampler<0, 7, 21>::run(taddr_row, b3, lrow, a.actions + (size_t)row * 7, live, next_u);
+            } else
+            for (int h = 0; h < n.n_heads; ++h) {
+                if ((h & 3) == 0)
+                    philox4x32_10(a.env_id_base + (uint32_t)env, (uint32_t)agent, (uint32_t)t, a.stream_base + (uint32_t)(h >> 2), a.seed_lo,
+                                  a.seed_hi, x[0], x[1], x[2], x[3]);
+                const uint32_t xw = (h & 3) == 0 ? x[0] : (h & 3) == 1 ? x[1] : (h & 3) == 2 ? x[2] : x[3];
+                const float u = u01(xw);
+                const int lo = h * n.head, hi = lo + n.head;
+                float* lrow = (a.logits && live) ? a.logits + (size_t)row * n.n_out : nullptr;
+                int pick;
+                if (a.mask.on) {  // f1: single-head population job (uniform over the CTA)
+                    pick = sample_head_masked(taddr_row, b3, n.n_out, u, lrow, a.mask, a.state + (size_t)env * a.blob_stride, agent);
+                } else if (n.n_heads == 1 && n.head == 65) {  // R = 3 (BASELINE.json configs[4]): 3 + 1 + 60 + 1 actions
+                    pick = sample_single_head<65>(taddr_row, b3, u, lrow);
+                } else if (n.n_heads == 1 && n.head == 44) {  // R = 2
+                    pick = sample_single_head<44>(taddr_row, b3, u, lrow);
+                } else
+                switch (n.nch) {
+                    case 1: pick = sample_head<1>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                    case 2: pick = sample_head<2>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                    case 3: pick = sample_head<3>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                    case 4: pick = sample_head<4>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                    case 5: pick = sample_head<5>(taddr_row, b3, lo, hi, n.Op, u, lrow); break;
+                    default: pick = sample_head_sweeps(taddr_row, b3, lo, hi, u, lrow); break;
+                }
+                if (live) a.actions[(size_t)row * n.n_heads + h] = pick;
+            }
+            // the slot's next layer-1 MMAs overwrite these TMEM columns: ordered by the fence + group barrier of the next build
+            asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
+        }
     }
 
     asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory");
