@@ -82,9 +82,11 @@ def lib():
     """Load libeconojax.so (building it in-tree if the source is newer).  Raises if unavailable."""
     global _lib
     if _lib is None:
-        path = _build.LIB
-        if not os.path.exists(path) or os.path.getmtime(path) < os.path.getmtime(_build.SRC):
-            path = _build.build_lib()
+        path = os.environ.get("EJ_LIB")  # a prebuilt library (development builds); default: the in-tree build
+        if not path:
+            path = _build.LIB
+            if not os.path.exists(path) or os.path.getmtime(path) < os.path.getmtime(_build.SRC):
+                path = _build.build_lib()
         L = C.CDLL(path)
         vp = C.c_void_p
         L.ej_create.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(EjParams), C.POINTER(vp)]

@@ -56,7 +56,7 @@ struct ej_env {
     // the step kernel variant of this handle's shape (CTA size, array stride, specialised R / P)
     void (*step_fn)(const DevCfg, uint8_t*, const StepIO) = nullptr;
     void (*step_fn_fx)(const DevCfg, uint8_t*, const StepIO) = nullptr;  // f2: factored observations
-    int step_RT = 0, step_PT = 0;
+    int step_RT = 0, step_PT = 0, step_pf = 0;
 };
 
 namespace {
@@ -105,9 +105,19 @@ int for_variant(int Npad, int ns, F&& f) {
     }
 }
 
+// Shapes with a fully specialised step kernel (R, P, N, B and the paper's mechanics as compile-time constants, 16-bit
+// order-pool words): BASELINE.json's N = 100 shapes and the paper's section-5 shape r = 4.  select_step_kernel
+// instantiates exactly these.
+bool is_paper_shape(const DevCfg& c) {
+    const bool paper = c.M == 15 && c.Mp_log2 == 4 && c.K == 0 && c.craft_mode == EJ_CRAFT_SINGLE && c.craft_units == 2 &&
+                       c.craft_distinct == 2 && c.allow_noop == 1 && c.expiry <= 31;
+    if (!paper || c.N != 100 || c.Npad != 128 || c.N4 != tight_stride(128)) return false;
+    return (c.P == 10 && c.B == 7 && (c.R == 2 || c.R == 3 || c.R == 6)) || (c.P == 3 && c.B == 3 && c.R == 4);
+}
+
 // Shared-memory layout: the NP-only sections come from Lay<NP> (compile-time constants shared
 // with the kernels); the R-, P-, M-dependent sections are placed here.
-void build_layout(DevCfg& c) {
+void build_layout(DevCfg& c, bool allow_pool16 = true) {
     const int NP = c.N4, R = c.R, nl = c.n_levels;  // NP: stride of the per-agent arrays
     for_variant(c.Npad, NP, [&](auto, auto ns) {
         using L = Lay<decltype(ns)::value>;
@@ -126,7 +136,10 @@ void build_layout(DevCfg& c) {
     c.o_head = take(nl * 2);
     c.o_tail = take(nl * 2);
     c.o_cnt = take(2 * nl * 4);
-    c.o_pool = take((c.N << c.Mp_log2) * 4);
+    c.pool16 = (allow_pool16 && is_paper_shape(c)) ? 1 : 0;
+    c.o_pool = take((c.N << c.Mp_log2) * (c.pool16 ? 2 : 4));
+    c.o_spl = o;  // bucket bounds of the block-wide sort (hints), sized by the kernel variant
+    o += for_variant(c.Npad, NP, [&](auto, auto ns) { return Lay<decltype(ns)::value>::spl_bytes; });
     c.blob_bytes = o;
     // runtime scratch (absolute offsets; zeroed at kernel start up to the staging tile)
     o = c.o_blob + c.blob_bytes;
@@ -148,7 +161,7 @@ void build_layout(DevCfg& c) {
     // state update and the statistics of the same step
     const int bk2 = for_variant(c.Npad, NP, [&](auto, auto ns) {
         using L = Lay<decltype(ns)::value>;
-        return L::bucketed ? 2 * L::bk_warps * L::bk_cap * 4 : 0;
+        return L::bk_metrics > 1 ? (L::bk_metrics - 1) * L::bk_warps * L::bk_cap * 4 : 0;
     });
     c.o_stage = o;
     c.stage_obs = 0;
@@ -186,22 +199,24 @@ void select_step_kernel(ej_env* h) {
     h->step_fn_fx = nullptr;  // f2 variants exist for CTAs of up to 256 threads (build time)
     if constexpr (MT <= 256) h->step_fn_fx = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0, 1>;
     h->step_RT = h->step_PT = 0;
+    h->step_pf = 0;
     // pf = 1 also fixes the paper's mechanics (Table 2; PF in ej_device.cuh)
     auto pick = [&](auto rt, auto pt, auto nt, auto bt, auto pf) {
         constexpr int RT = decltype(rt)::value, PT = decltype(pt)::value, NT = decltype(nt)::value, BT = decltype(bt)::value;
         constexpr int PF = decltype(pf)::value;
-        const bool paper = c.M == 15 && c.Mp_log2 == 4 && c.K == 0 && c.craft_mode == EJ_CRAFT_SINGLE && c.craft_units == 2 &&
-                           c.craft_distinct == 2 && c.allow_noop == 1 && c.stage_obs == 1;
+        const bool paper = c.pool16 == 1 && c.stage_obs == 1;
         bool lay_ok = true;
         if constexpr (PF == 1) {  // the kernel's compile-time layout must be the one build_layout() made
             using S = StaticLay<NS, RT, PT, NT>;
             lay_ok = c.o_esc_res == S::esc_res && c.o_SG == S::SG && c.o_head == S::head && c.o_tail == S::tail && c.o_cnt == S::cnt &&
-                     c.o_pool == S::pool && c.blob_bytes == S::blob_bytes && c.o_ahead == S::ahead && c.o_cdf == S::cdf &&
+                     c.o_pool == S::pool && c.o_spl == S::spl && c.blob_bytes == S::blob_bytes && c.o_ahead == S::ahead && c.o_cdf == S::cdf &&
                      c.o_stage == S::stage && c.o_mb == S::mb && c.o_ma == S::ma;
         }
         if (c.R == RT && c.P == PT && (NT == 0 || (c.N == NT && c.B == BT)) && (PF == 0 || (paper && lay_ok))) {
             h->step_fn = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF>;
-            if constexpr (PF == 1 && RT == 2) h->step_fn_fx = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF, 1>;  // headline shape
+            h->step_pf = PF;
+            // f2: the factored variant must read the same (16-bit) order pool as the dense one
+            if constexpr (PF == 1) h->step_fn_fx = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF, 1>;
             h->step_RT = RT; h->step_PT = PT;
         }
     };
@@ -554,6 +569,10 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
         return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "N/R/max_active_orders (state exceeds 227 KB of shared memory)");
     }
     int rc = set_smem_attr(h);
+    if (rc == EJ_OK && c.pool16 && !h->step_pf) {  // no kernel for the 16-bit pool words of this layout: plain layout, generic kernel
+        build_layout(c, false);
+        rc = set_smem_attr(h);
+    }
     if (rc != EJ_OK) { memcpy(g_create_err, h->err, 256); delete h; return rc; }
     cudaError_t ce = cudaMalloc(&h->d_state, (size_t)E * c.blob_bytes);
     if (ce == cudaSuccess) ce = cudaMemset(h->d_state, 0, (size_t)E * c.blob_bytes);
@@ -837,7 +856,8 @@ int ej_get_state(ej_env* h, int32_t env_begin, int32_t env_count, int32_t* words
         const float* SG = (const float*)(s + c.o_SG); const int* inv = (const int*)(s + c.o_inv);
         const int* esc_res = (const int*)(s + c.o_esc_res);
         const uint16_t* head = (const uint16_t*)(s + c.o_head); const int* cnt = (const int*)(s + c.o_cnt) + (((const EnvHdr*)s)->t & 1) * c.n_levels;
-        const uint32_t* pool = (const uint32_t*)(s + c.o_pool);
+        const uint32_t* pool32 = (const uint32_t*)(s + c.o_pool);
+        const uint16_t* pool16 = (const uint16_t*)(s + c.o_pool);
         int32_t* w = words + (size_t)k * W;
         memset(w, 0, W * 4);
         size_t q = 0;
@@ -867,15 +887,24 @@ int ej_get_state(ej_env* h, int32_t env_begin, int32_t env_count, int32_t* words
                 uint32_t hh = head[b * P + p];
                 int guard = 0;
                 while (hh != NIL && guard++ < cap + 1) {
-                    const uint32_t pe = pool[hh];
-                    const int age = (int)(((uint32_t)hd->t - (pe >> 16)) & 0xFFFFu);
+                    int age;
+                    uint32_t nxt;
+                    if (c.pool16) {  // next (11 bits, 0x7FF = none) | placed_at mod 32
+                        const uint32_t pe = pool16[hh];
+                        age = (int)(((uint32_t)hd->t - (pe >> 11)) & 31u);
+                        nxt = (pe & 0x7FFu) == 0x7FFu ? NIL : (pe & 0x7FFu);
+                    } else {         // next (16 bits) | placed_at (16 bits)
+                        const uint32_t pe = pool32[hh];
+                        age = (int)(((uint32_t)hd->t - (pe >> 16)) & 0xFFFFu);
+                        nxt = pe & 0xFFFFu;
+                    }
                     if (out < cap) {
                         w[q0 + 3 * out] = c.prices[p];
                         w[q0 + 3 * out + 1] = (int32_t)(hh >> c.Mp_log2);
                         w[q0 + 3 * out + 2] = hd->t - age;
                     }
                     ++out;
-                    hh = pe & 0xFFFFu;
+                    hh = nxt;
                 }
             }
             q = q0 + 3 * (size_t)cap;
@@ -904,7 +933,7 @@ int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t*
         double* cf = (double*)(s + c.o_cf);
         float* SG = (float*)(s + c.o_SG); int* inv = (int*)(s + c.o_inv); int* esc_res = (int*)(s + c.o_esc_res);
         uint16_t* head = (uint16_t*)(s + c.o_head); uint16_t* tail = (uint16_t*)(s + c.o_tail);
-        int* cnt = (int*)(s + c.o_cnt); uint32_t* pool = (uint32_t*)(s + c.o_pool);
+        int* cnt = (int*)(s + c.o_cnt); uint32_t* pool32 = (uint32_t*)(s + c.o_pool); uint16_t* pool16 = (uint16_t*)(s + c.o_pool);
         const int32_t* w = words + (size_t)k * W;
         size_t q = 0;
         hd->t = w[q++];
@@ -942,10 +971,16 @@ int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t*
                 while (!((free_bits >> bit) & 1u)) ++bit;
                 mask[owner] |= 1u << bit;
                 const uint32_t slot = ((uint32_t)owner << c.Mp_log2) + (uint32_t)bit;
-                pool[slot] = NIL | (((uint32_t)placed & 0xFFFFu) << 16);
                 const int l = b * P + p;
-                if (tail[l] != NIL) pool[tail[l]] = (pool[tail[l]] & 0xFFFF0000u) | slot;
-                else head[l] = (uint16_t)slot;
+                if (c.pool16) {
+                    if (hd->t - placed > 31) return fail(h, EJ_ERR_PARAM, "bad field: %s", "words (order older than the expiry)");
+                    pool16[slot] = (uint16_t)(0x7FFu | (((uint32_t)placed & 31u) << 11));
+                    if (tail[l] != NIL) pool16[tail[l]] = (uint16_t)((pool16[tail[l]] & 0xF800u) | slot);
+                } else {
+                    pool32[slot] = NIL | (((uint32_t)placed & 0xFFFFu) << 16);
+                    if (tail[l] != NIL) pool32[tail[l]] = (pool32[tail[l]] & 0xFFFF0000u) | slot;
+                }
+                if (tail[l] == NIL) head[l] = (uint16_t)slot;
                 tail[l] = (uint16_t)slot;
                 cnt[l]++;
                 // a resting book is uncrossed (G13): the kernels size their matched-order lists by that

@@ -30,6 +30,10 @@
 
 #include "../../include/econojax.h"
 
+#ifndef EJ_CTAS_128
+#define EJ_CTAS_128 9  // resident 128-thread CTAs per SM the step kernel is compiled for (registers)
+#endif
+
 namespace {
 
 // Debug builds (-DEJ_PHASE_CLOCK): block 0 accumulates the cycles between the barriers of a step and prints them at
@@ -50,6 +54,28 @@ __device__ unsigned long long ej_phase_last;
 #endif
 
 constexpr uint32_t NIL = 0xFFFFu;      // null slot of the order pool
+// Order-pool word of a slot: next slot of its price level's FIFO | step at which the order was placed.  Two formats:
+//   W = 0  32 bits: next (16) | placed_at (16): any shape;
+//   W = 1  16 bits: next (11, 0x7FF = none) | placed_at mod 32 (5): the paper's mechanics at N <= 127 (16 slots per agent:
+//          N * 16 <= 2032 slots) with order_expiry <= 31 (30) -- an order's age t - placed_at never exceeds the
+//          expiry, so five bits of the clock identify it.  Halves the pool (3.2 KB per economy at N = 100), which
+//          is what lets one more CTA stay resident per SM.
+template <int W> struct PoolW;
+template <> struct PoolW<0> {
+    using T = uint32_t;
+    __device__ __forceinline__ static T make(uint32_t nxt, int t) { return nxt | (((uint32_t)t & 0xFFFFu) << 16); }
+    __device__ __forceinline__ static uint32_t next(T w) { return w & 0xFFFFu; }
+    __device__ __forceinline__ static uint32_t age(T w, int t) { return ((uint32_t)t - (w >> 16)) & 0xFFFFu; }
+    __device__ __forceinline__ static T with_next(T w, uint32_t nxt) { return (w & 0xFFFF0000u) | nxt; }
+};
+template <> struct PoolW<1> {
+    using T = uint16_t;
+    __device__ __forceinline__ static T make(uint32_t nxt, int t) { return (T)((nxt & 0x7FFu) | (((uint32_t)t & 31u) << 11)); }  // NIL & 0x7FF = 0x7FF
+    __device__ __forceinline__ static uint32_t next(T w) { const uint32_t n = w & 0x7FFu; return n == 0x7FFu ? NIL : n; }
+    __device__ __forceinline__ static uint32_t age(T w, int t) { return ((uint32_t)t - ((uint32_t)w >> 11)) & 31u; }
+    __device__ __forceinline__ static T with_next(T w, uint32_t nxt) { return (T)((w & 0xF800u) | (nxt & 0x7FFu)); }
+};
+
 // Book-cap path: a step's candidates are binned by the top bits of their arrival key (a uniform Philox word, G11):
 // 256 bins per book give the rank of a candidate on its book, 32 bins per level its neighbours on its level.
 constexpr int BOOK_BINS = 256, BOOK_BIN_SHIFT = 24, LEVEL_BINS = 32, LEVEL_BIN_SHIFT = 27;
@@ -64,10 +90,6 @@ struct EnvHdr {
     int32_t pad1;
     float rates[EJ_MAX_BRACKETS];
     int32_t last_price[EJ_MAX_RESOURCES];
-    // block-wide sort of large populations: bucket bounds of coin, labor, income = last step's order statistics of
-    // rank (b+1) N / NW (float bits), double-buffered (spl_cur names the buffer in force); hints like med_prev, not state
-    uint32_t spl[3][2][32];
-    uint32_t spl_cur, spl_pad[3];
 };
 static_assert(sizeof(EnvHdr) % 16 == 0, "EnvHdr must keep 16-byte alignment");
 
@@ -77,6 +99,7 @@ struct DevCfg {
     int recipP;  // ceil(2^16 / P): k / P == (k * recipP) >> 16 for k < 2RP <= 512
     int A, base_craft, base_buy, base_sell, n_levels, n_groups, D_pop, D_gov, D_gov_pad;
     int N4, Npad, n_metrics, n_warps, shrow_len, stage_obs;
+    int pool16;             // order-pool words are 16 bits (PoolW<1>): the shape-specialised paper-mechanics kernels
     int stage_alias_bytes;  // head of the staging tile that the matched-order lists overwrite every step
     int prices[EJ_MAX_PRICES];
     float thresholds[EJ_MAX_BRACKETS];
@@ -90,7 +113,7 @@ struct DevCfg {
     uint32_t env_id_base, seed_lo, seed_hi;
     // blob section offsets (bytes from the blob base)
     int o_coin, o_labor, o_income, o_SC, o_esc_coin, o_mask, o_cf, o_SG, o_inv, o_esc_res;
-    int o_head, o_tail, o_cnt, o_pool, blob_bytes;
+    int o_head, o_tail, o_cnt, o_pool, o_spl, blob_bytes;
     int o_blob, o_scratch1;  // absolute: blob start (= Lay<Npad>::blob), first byte after the blob
     // scratch section offsets (bytes from the shared-memory base; all after the blob)
     int o_key, o_cinfo, o_cslot, o_anext, o_ahead, o_credit, o_sale, o_mb, o_ma;
@@ -138,16 +161,23 @@ struct Lay {
     static constexpr int govrow = shrow + shrow_cap * 4;
     static constexpr int govrow_cap = 80;  // >= ceil4(3 (3 + 16) + 16 + 2)
     static constexpr int misc = govrow + govrow_cap * 4;       // u64 [2]: tax pool
-    // block-wide coin sort (CTAs of 8 warps and more): one bucket of coin keys per warp
-    static constexpr bool bucketed = NP >= 416;                 // NP is the array stride (13/16 of the CTA size or the CTA size): CTAs of 512 and 1024 threads
-    static constexpr int bk_warps = NP >= 832 ? 32 : 16;        // warps of such a CTA = buckets
-    // the bucket keys live in key | cslot | anext (3 NP words): those are dead between the settlement of a step's
-    // trades and the next step's arrivals, which is when the buckets are filled and sorted
+    // block-wide sort of the float metrics (bucket_fill / bucket_sort below): one bucket per warp and metric.  NP is the
+    // array stride (13/16 of the CTA size, or the CTA size): CTAs of 512 / 1024 threads sort coin, labor and income this way.
+    static constexpr int bk_warps = NP >= 832 ? 32 : NP >= 416 ? 16 : NP >= 208 ? 8 : 4;
+    // (measured at N = 100: bucketing the coin across the four warps of a 128-thread CTA cost 9 us per batched step,
+    // 32.4 -> 42 us; the register network on one warp is cheaper there, so small CTAs do not bucket)
+    static constexpr int bk_metrics = NP >= 416 ? 3 : 0;
+    static constexpr bool bucketed = bk_metrics > 0;
+    // the coin's bucket keys live in key | cslot | anext (3 NP words): those are dead between the settlement of a
+    // step's trades and the next step's arrivals, which is when the buckets are filled and sorted
     static constexpr int bk_keys = key;
     static constexpr int bk_cap = (3 * NP / bk_warps) < 128 ? (3 * NP / bk_warps) : 128;  // keys per bucket (sorted 4 per lane at most)
-    static constexpr int bk_cnt = misc + 16;                    // u32 [3][72]: per metric [0..31] bucket sizes, [32..63] values equal to a bound, [64] overflow flag, [65..66] medians
-    static constexpr int bk_part = bk_cnt + (bucketed ? 3 * 72 * 4 : 0);  // f64 [3][32][3]: gini, sum, sum of squares per bucket
-    static constexpr int blob = bk_part + (bucketed ? 3 * 32 * 3 * 8 : 0);
+    static constexpr int bk_cnt_words = 2 * bk_warps + 4;       // per metric: bucket sizes | values equal to a bound | overflow flag, two medians
+    static constexpr int bk_cnt = misc + 16;
+    static constexpr int bk_part = bk_cnt + ((bk_metrics * bk_cnt_words * 4 + 15) & ~15);  // f64 [metrics][warps][3]: gini, sum, sum of squares per bucket
+    static constexpr int blob = bk_part + ((bk_metrics * bk_warps * 3 * 8 + 15) & ~15);
+    // bucket bounds (hints, kept in the blob): u32 [metrics][2][warps] double-buffered, then the index of the buffer in force
+    static constexpr int spl_bytes = bucketed ? ((bk_metrics * 2 * bk_warps * 4 + 4 + 15) & ~15) : 0;
     // blob sections (byte offsets relative to the blob)
     static constexpr int coin = (int)sizeof(EnvHdr);
     static constexpr int labor = coin + NP * 4;
@@ -174,7 +204,8 @@ struct StaticLay {
     static constexpr int tail = lay_align16(head + nl * 2);
     static constexpr int cnt = lay_align16(tail + nl * 2);
     static constexpr int pool = lay_align16(cnt + 2 * nl * 4);
-    static constexpr int blob_bytes = lay_align16(pool + (N << 4) * 4);
+    static constexpr int spl = lay_align16(pool + (N << 4) * 2);  // 16-bit pool words (PoolW<1>)
+    static constexpr int blob_bytes = spl + Lay<NP>::spl_bytes;
     static constexpr int ahead = Lay<NP>::blob + blob_bytes;  // absolute from here on
     static constexpr int cdf = lay_align16(ahead + nl * 4);
     static constexpr int stage = lay_align16(cdf + A * 4);
@@ -207,7 +238,8 @@ struct Sm {
     __device__ __forceinline__ uint16_t* head() const { return at<uint16_t>(L::blob + (ST ? S::head : c.o_head)); }
     __device__ __forceinline__ uint16_t* tail() const { return at<uint16_t>(L::blob + (ST ? S::tail : c.o_tail)); }
     __device__ __forceinline__ int* cnt() const { return at<int>(L::blob + (ST ? S::cnt : c.o_cnt)); }  // [2][n_levels]: buffer (t & 1) is current
-    __device__ __forceinline__ uint32_t* pool() const { return at<uint32_t>(L::blob + (ST ? S::pool : c.o_pool)); }
+    template <int W>
+    __device__ __forceinline__ typename PoolW<W>::T* pool() const { return at<typename PoolW<W>::T>(L::blob + (ST ? S::pool : c.o_pool)); }
     __device__ __forceinline__ uint32_t* key() const { return at<uint32_t>(L::key); }
     __device__ __forceinline__ uint32_t* cslot() const { return at<uint32_t>(L::cslot); }
     __device__ __forceinline__ uint32_t* anext() const { return at<uint32_t>(L::anext); }
@@ -218,8 +250,10 @@ struct Sm {
     __device__ __forceinline__ float* shrow() const { return at<float>(L::shrow); }
     __device__ __forceinline__ float* govrow() const { return at<float>(L::govrow); }
     __device__ __forceinline__ unsigned long long* misc() const { return at<unsigned long long>(L::misc); }  // [0] tax pool in 2^-20 coin
-    __device__ __forceinline__ uint32_t* bk_cnt(int k) const { return at<uint32_t>(L::bk_cnt) + k * 72; }
-    __device__ __forceinline__ double* bk_part(int k) const { return at<double>(L::bk_part) + k * 96; }
+    __device__ __forceinline__ uint32_t* bk_cnt(int k) const { return at<uint32_t>(L::bk_cnt) + k * L::bk_cnt_words; }
+    __device__ __forceinline__ double* bk_part(int k) const { return at<double>(L::bk_part) + k * (L::bk_warps * 3); }
+    __device__ __forceinline__ uint32_t* spl(int k, uint32_t buf) const { return at<uint32_t>(L::blob + (ST ? S::spl : c.o_spl)) + (k * 2 + (int)buf) * L::bk_warps; }
+    __device__ __forceinline__ uint32_t* spl_cur() const { return at<uint32_t>(L::blob + (ST ? S::spl : c.o_spl)) + L::bk_metrics * 2 * L::bk_warps; }
     // bucket keys: coin in key | cslot | anext, labor and income in a region of their own (or over the matched lists)
     __device__ __forceinline__ uint32_t* bk_keys(int k) const {
         return k == 0 ? at<uint32_t>(L::bk_keys) : at<uint32_t>(c.o_bk2) + (k - 1) * (L::bk_warps * L::bk_cap);
@@ -503,7 +537,7 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const SM& m, int k
     float lo, hi;
     const int r0 = N >= 2 ? (N >> 1) - 1 : 0, r1 = N >> 1;
     bool found = false;
-    if (k != 0 && !SM::L::bucketed) {  // labor, income: med_prev holds last step's lower median
+    if (k != 0 && k >= SM::L::bk_metrics) {  // labor, income (when not bucketed): med_prev holds last step's lower median
         uint32_t key[EPL], klo, khi;
 #pragma unroll
         for (int q = 0; q < EPL; ++q) key[q] = __float_as_uint(x[q]);
@@ -516,12 +550,12 @@ __device__ __forceinline__ void metric_stats(const DevCfg& c, const SM& m, int k
         lo = warp_pick<EPL>(x, r0);
         hi = warp_pick<EPL>(x, r1);
         if (k != 0 && lane == 0) m.hdr()->med_prev[k - 1] = __float_as_uint(lo);
-        if (SM::L::bucketed) {  // EPL = warps of the CTA: renew this metric's bucket bounds of the block-wide sort
-            const uint32_t nxt = (m.hdr()->spl_cur & 1u) ^ 1u;
+        if (k < SM::L::bk_metrics) {  // EPL = warps of the CTA: renew this metric's bucket bounds of the block-wide sort
+            const uint32_t nxt = (*m.spl_cur() & 1u) ^ 1u;
 #pragma unroll 1
             for (int b = 0; b + 1 < EPL; ++b) {
                 const float v = warp_pick<EPL>(x, ((b + 1) * N) / EPL);
-                if (lane == 0) m.hdr()->spl[k][nxt][b] = __float_as_uint(v);
+                if (lane == 0) m.spl(k, nxt)[b] = __float_as_uint(v);
             }
         }
         if (k == 0 && mode != 2) {
@@ -612,7 +646,7 @@ template <int NPAD, class SM>
 __device__ __forceinline__ void bucket_fill(const SM& m, int k, float x) {
     constexpr int NW = NPAD / 32, CAP = SM::L::bk_cap;
     const uint32_t key = __float_as_uint(x);
-    const uint32_t* spl = m.hdr()->spl[k][m.hdr()->spl_cur & 1u];
+    const uint32_t* spl = m.spl(k, *m.spl_cur() & 1u);
     int lo = 0, hi = NW - 1;  // bucket = number of bounds <= key
     while (lo < hi) {
         const int mid = (lo + hi) >> 1;
@@ -621,19 +655,21 @@ __device__ __forceinline__ void bucket_fill(const SM& m, int k, float x) {
     }
     uint32_t* cnt = m.bk_cnt(k);
     if (lo > 0 && spl[lo - 1] == key) {
-        atomicAdd(&cnt[32 + lo - 1], 1u);  // equal to bound lo-1 (the last of equal bounds): counted, not stored
+        atomicAdd(&cnt[NW + lo - 1], 1u);  // equal to bound lo-1 (the last of equal bounds): counted, not stored
     } else {
         const uint32_t pos = atomicAdd(&cnt[lo], 1u);
         if (pos < (uint32_t)CAP && !(key >> 31)) m.bk_keys(k)[lo * CAP + (int)pos] = key;
-        else cnt[64] = 1u;  // overflow (or a negative value): fall back
+        else cnt[2 * NW] = 1u;  // overflow (or a negative value): fall back
     }
 }
 template <int NPAD, class SM>
 __device__ __forceinline__ void bucket_fill_all(const SM& m, int tid, bool act) {
     if (!act) return;
     bucket_fill<NPAD>(m, 0, m.coin()[tid]);
-    bucket_fill<NPAD>(m, 1, m.labor()[tid]);
-    bucket_fill<NPAD>(m, 2, m.income()[tid]);
+    if (SM::L::bk_metrics > 1) {
+        bucket_fill<NPAD>(m, 1, m.labor()[tid]);
+        bucket_fill<NPAD>(m, 2, m.income()[tid]);
+    }
 }
 
 // Warp `warp` sorts its bucket of metric k (n <= 32 EPL values, blocked layout), followed in rank order by the ne
@@ -642,8 +678,8 @@ __device__ __forceinline__ void bucket_fill_all(const SM& m, int tid, bool act) 
 template <int EPL, int NPAD, class SM>
 __device__ __forceinline__ void bucket_sort(const SM& m, int k, int warp, int lane, int n, int ne, int off, int N) {
     constexpr int NW = NPAD / 32, CAP = SM::L::bk_cap;
-    const uint32_t cur = m.hdr()->spl_cur & 1u;
-    const float v_eq = __uint_as_float(m.hdr()->spl[k][cur][warp < NW - 1 ? warp : 0]);  // ne = 0 for the last warp
+    const uint32_t cur = *m.spl_cur() & 1u;
+    const float v_eq = __uint_as_float(m.spl(k, cur)[warp < NW - 1 ? warp : 0]);  // ne = 0 for the last warp
     float x[EPL];
 #pragma unroll
     for (int q = 0; q < EPL; ++q) {
@@ -684,11 +720,11 @@ __device__ __forceinline__ void bucket_sort(const SM& m, int k, int warp, int la
             const float y = __shfl_sync(FULL, x[q], src / EPL);
             v = (src % EPL) == q ? y : v;
         }
-        if (mine) m.hdr()->spl[k][cur ^ 1u][lane] = __float_as_uint(want < n ? v : v_eq);
+        if (mine) m.spl(k, cur ^ 1u)[lane] = __float_as_uint(want < n ? v : v_eq);
     }
     const int r0 = (N >= 2 ? (N >> 1) - 1 : 0) - off, r1 = (N >> 1) - off;
-    if (r0 >= 0 && r0 < n + ne) { const float v = r0 < n ? warp_pick<EPL>(x, r0) : v_eq; if (lane == 0) m.bk_cnt(k)[65] = __float_as_uint(v); }
-    if (r1 >= 0 && r1 < n + ne) { const float v = r1 < n ? warp_pick<EPL>(x, r1) : v_eq; if (lane == 0) m.bk_cnt(k)[66] = __float_as_uint(v); }
+    if (r0 >= 0 && r0 < n + ne) { const float v = r0 < n ? warp_pick<EPL>(x, r0) : v_eq; if (lane == 0) m.bk_cnt(k)[2 * NW + 1] = __float_as_uint(v); }
+    if (r1 >= 0 && r1 < n + ne) { const float v = r1 < n ? warp_pick<EPL>(x, r1) : v_eq; if (lane == 0) m.bk_cnt(k)[2 * NW + 2] = __float_as_uint(v); }
 }
 
 // All warps: sort the own bucket of metric k.  Nothing to do if the buckets overflowed (the caller falls back).
@@ -696,8 +732,8 @@ template <int NPAD, class SM>
 __device__ __forceinline__ void bucket_stats(const SM& m, int k, int warp, int lane, int N) {
     constexpr int NW = NPAD / 32;
     const uint32_t* cnt = m.bk_cnt(k);
-    if (cnt[64]) return;
-    const int nb = lane < NW ? (int)cnt[lane] : 0, neq = lane < NW - 1 ? (int)cnt[32 + lane] : 0;
+    if (cnt[2 * NW]) return;
+    const int nb = lane < NW ? (int)cnt[lane] : 0, neq = lane < NW - 1 ? (int)cnt[NW + lane] : 0;
     int incl = nb + neq;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -798,18 +834,18 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
 
     // ---- government statistics: metric k is owned by one warp (floats from warp 0 up, integer
     // metrics from the last warp down) ----
-    constexpr bool BKT = SM::L::bucketed;  // coin, labor, income: every warp sorts one bucket per metric (filled before the caller's barrier)
+    constexpr bool BKT = SM::L::bucketed;  // coin (large CTAs: labor and income too): every warp sorts one bucket per metric, filled before the caller's barrier
+    constexpr int BKM = SM::L::bk_metrics, BKF = 2 * SM::L::bk_warps;  // bucketed metrics; index of a metric's overflow flag
     bool fell_back = false;  // some metric's buckets overflowed (the same answer in every thread)
     if (BKT) {
 #pragma unroll 1
-        for (int k = 0; k < 3; ++k) {
-            fell_back = fell_back || m.bk_cnt(k)[64] != 0u;
+        for (int k = 0; k < BKM; ++k) {
+            fell_back = fell_back || m.bk_cnt(k)[BKF] != 0u;
             bucket_stats<NPAD>(m, k, warp, lane, N);
         }
-    } else {
-#pragma unroll 1
-        for (int k = warp; k < 3; k += NW) metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
     }
+#pragma unroll 1
+    for (int k = BKM + warp; k < 3; k += NW) metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
 #pragma unroll 1
     for (int r = NW - 1 - warp; r < R; r += NW) int_metric_stats<EPL, NS, NT>(c, m, r, lane);
     if (tid < B + 2) m.govrow()[3 * n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
@@ -821,9 +857,9 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
 
     if (BKT && warp == 0) {  // the three triples and the welfare from the buckets' shares (or the single-warp sort)
 #pragma unroll 1
-        for (int k = 0; k < 3; ++k) {
+        for (int k = 0; k < BKM; ++k) {
             uint32_t* cnt = m.bk_cnt(k);
-            if (!cnt[64]) {
+            if (!cnt[BKF]) {
                 double g = 0.0, s1 = 0.0, s2 = 0.0;
                 if (lane < NW) { const double* part = m.bk_part(k) + lane * 3; g = part[0]; s1 = part[1]; s2 = part[2]; }
                 g = warp_sum(g); s1 = warp_sum(s1); s2 = warp_sum(s2);
@@ -832,7 +868,7 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
                     const double mean = s1 * inv_n;
                     double var = (s2 - s1 * mean) * inv_n;  // population variance from sum and sum of squares (binary64)
                     if (var < 0.0) var = 0.0;
-                    gov_triple<NS, NT>(c, m, k, mean, var, __uint_as_float(cnt[65]), __uint_as_float(cnt[66]), k == 1 ? c.s_labor : c.s_coin);
+                    gov_triple<NS, NT>(c, m, k, mean, var, __uint_as_float(cnt[BKF + 1]), __uint_as_float(cnt[BKF + 2]), k == 1 ? c.s_labor : c.s_coin);
                     if (k == 0 && mode != 2) {
                         const double ug = s1 - (double)c.omega * (g * inv_n);  // Eq.3-5 as in metric_stats
                         if (mode == 0) {
@@ -847,9 +883,9 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
                 metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
             }
             __syncwarp();
-            for (int i = lane; i < 72; i += 32) cnt[i] = 0u;  // empty buckets for the next step
+            for (int i = lane; i < SM::L::bk_cnt_words; i += 32) cnt[i] = 0u;  // empty buckets for the next step
         }
-        if (lane == 0) m.hdr()->spl_cur ^= 1u;  // the bounds written during this step are in force from now on
+        if (lane == 0) *m.spl_cur() ^= 1u;  // the bounds written during this step are in force from now on
         __syncwarp();
         if (any_obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
         __syncwarp();
@@ -1216,9 +1252,9 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
 
     if (lvl >= 0) {
         if (accepted) {
-            m.pool()[slot] = nxt | (((uint32_t)t & 0xFFFFu) << 16);
+            m.template pool<PF>()[slot] = PoolW<PF>::make(nxt, t);
             if (lrank == 0) {
-                if (old_tail != NIL) m.pool()[old_tail] = (m.pool()[old_tail] & 0xFFFF0000u) | slot;
+                if (old_tail != NIL) m.template pool<PF>()[old_tail] = PoolW<PF>::with_next(m.template pool<PF>()[old_tail], slot);
                 else m.head()[lvl] = (uint16_t)slot;
             }
             if (nxt == NIL) m.tail()[lvl] = (uint16_t)slot;
@@ -1266,14 +1302,14 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
             uint32_t* dst = (side ? m.ma() : m.mb()) + r * N4 + better;
             for (int k = 0; k < tk; ++k) {
                 dst[k] = h | ((uint32_t)pidx << 16);
-                h = m.pool()[h] & 0xFFFFu;
+                h = PoolW<PF>::next(m.template pool<PF>()[h]);
             }
             n -= tk;
         }
         int nexp = 0;
         while (h != NIL) {
-            const uint32_t pe = m.pool()[h];
-            const uint32_t age = ((uint32_t)t - (pe >> 16)) & 0xFFFFu;
+            const typename PoolW<PF>::T pe = m.template pool<PF>()[h];
+            const uint32_t age = PoolW<PF>::age(pe, t);
             if ((int)age < c.expiry) break;
             const int owner = (int)(h >> MPL);
             if (side == 0) {
@@ -1286,7 +1322,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
             atomicAnd(&m.mask()[owner], ~(1u << (h & ((1u << MPL) - 1u))));
             ++nexp;
             --n;
-            h = pe & 0xFFFFu;
+            h = PoolW<PF>::next(pe);
         }
         if (tk > 0 || nexp > 0) {
             m.head()[l] = (uint16_t)h;
@@ -1311,8 +1347,8 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
                 const uint32_t sb = eb & 0xFFFFu, sa = ea & 0xFFFFu;
                 const int pb = c.prices[eb >> 16], pa = c.prices[ea >> 16];
                 const int ob = (int)(sb >> MPL), oa = (int)(sa >> MPL);
-                const uint32_t age_b = ((uint32_t)t - (m.pool()[sb] >> 16)) & 0xFFFFu;
-                const uint32_t age_a = ((uint32_t)t - (m.pool()[sa] >> 16)) & 0xFFFFu;
+                const uint32_t age_b = PoolW<PF>::age(m.template pool<PF>()[sb], t);
+                const uint32_t age_a = PoolW<PF>::age(m.template pool<PF>()[sa], t);
                 bool bid_later;
                 if (age_b != age_a) bid_later = age_b < age_a;
                 else if (m.key()[ob] != m.key()[oa]) bid_later = m.key()[ob] > m.key()[oa];
@@ -1425,7 +1461,7 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
 }
 
 template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX = 0>
-__global__ void __launch_bounds__(NPAD, (1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
+__global__ void __launch_bounds__(NPAD, (NPAD == 128 ? EJ_CTAS_128 : 1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const __grid_constant__ StepIO io) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
     uint8_t* const sblob = ej_smem + Lay<NS>::blob;
@@ -1499,7 +1535,7 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     const Sm<NS> m{c};
     const uint4* blob = (const uint4*)(state + (size_t)e * c.blob_bytes);
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) ((uint4*)sblob)[i] = blob[i];
-    if (Lay<NS>::bucketed && tid < 3 * 72) m.bk_cnt(0)[tid] = 0u;
+    if (Lay<NS>::bucketed && tid < Lay<NS>::bk_metrics * Lay<NS>::bk_cnt_words) m.bk_cnt(0)[tid] = 0u;
     __syncthreads();
     const int t = m.hdr()->t;
     if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt() + (t & 1) * c.n_levels);
