@@ -95,6 +95,8 @@ def lib():
             L.orc_obs_dim_pop.argtypes = [C.c_void_p]; L.orc_obs_dim_pop.restype = C.c_int32
             L.orc_obs_dim_gov.argtypes = [C.c_void_p]; L.orc_obs_dim_gov.restype = C.c_int32
             L.orc_reset.argtypes = [C.c_void_p, C.c_uint64]
+            L.orc_begin_episode.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_int32]
+            L.orc_step_auto.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.c_void_p] * 6
             L.orc_observe.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p]
             L.orc_step.argtypes = [C.c_void_p, C.c_int32, C.c_int32] + [C.c_void_p] * 6
             L.orc_draw_actions.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -170,7 +172,12 @@ class OracleEnv:
         self.L.orc_observe(self.h, env_begin, n, _ptr(obs_pop), _ptr(obs_gov))
         return obs_pop, obs_gov
 
-    def step(self, actions, gov_actions, env_begin=0, want_obs=True):
+    def begin_episode(self, episode: int, env_begin=0, env_count=None):
+        """f4: start episode `episode` in the given envs (orc_reset starts episode 0 everywhere)."""
+        n = self.E - env_begin if env_count is None else env_count
+        self.L.orc_begin_episode(self.h, env_begin, n, int(episode))
+
+    def step(self, actions, gov_actions, env_begin=0, want_obs=True, auto_reset=False):
         actions = np.ascontiguousarray(actions, np.int32)
         gov_actions = np.ascontiguousarray(gov_actions, np.int32)
         n = actions.shape[0]
@@ -179,8 +186,8 @@ class OracleEnv:
         obs_gov = np.zeros((n, self.D_gov), np.float32) if want_obs else None
         rew = np.zeros((n, self.N + 1), np.float32)
         done = np.zeros((n,), np.uint8)
-        self.L.orc_step(self.h, env_begin, n, _ptr(actions), _ptr(gov_actions), _ptr(obs_pop), _ptr(obs_gov),
-                        _ptr(rew), _ptr(done))
+        fn = self.L.orc_step_auto if auto_reset else self.L.orc_step
+        fn(self.h, env_begin, n, _ptr(actions), _ptr(gov_actions), _ptr(obs_pop), _ptr(obs_gov), _ptr(rew), _ptr(done))
         return obs_pop, obs_gov, rew, done
 
     def draw_actions(self, cdf, env_begin=0, env_count=None, masked=False):
@@ -249,4 +256,5 @@ def parse_state(words: np.ndarray) -> dict:
         books.append(w[q:q + 3 * n].reshape(n, 3).copy())
         q += 3 * cap
     out["books"] = books  # index 2*r + side, rows (price, owner, placed_at) in priority order
+    out["episode"] = int(w[q]) if q < len(w) else 0  # f4: last word
     return out

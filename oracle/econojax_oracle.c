@@ -226,6 +226,7 @@ typedef struct orc_book {
 
 typedef struct orc_env {
     int32_t t;
+    int32_t episode;   /* f4: index of the episode this env is in (0 after orc_reset); part of every Philox counter (G44) */
     float* coin;       /* [N] inventory coin C_i */
     float* labor;      /* [N] cumulative labor L_i */
     float* income;     /* [N] earnings since the last collection (G16) */
@@ -309,22 +310,24 @@ void orc_destroy(orc_sim* s) {
 int32_t orc_obs_dim_pop(const orc_sim* s) { return 6 + 8 * s->R + s->p.num_brackets; }
 int32_t orc_obs_dim_gov(const orc_sim* s) { return 3 * (3 + s->R) + s->p.num_brackets + 2; }
 
-static void draw(const orc_sim* s, uint32_t env_gid, uint32_t agent, uint32_t t, uint32_t stream, uint32_t x[4]) {
-    uint32_t ctr[4] = { env_gid, agent, t, stream };
+/* Counter = (global env id, agent, t, stream | episode << 8) (G30; G44: the episode index rides in the upper bits of
+ * the stream word, so episode 0 draws exactly what the counters of G30 draw). */
+static void draw(const orc_sim* s, uint32_t episode, uint32_t env_gid, uint32_t agent, uint32_t t, uint32_t stream, uint32_t x[4]) {
+    uint32_t ctr[4] = { env_gid, agent, t, stream | (episode << 8) };
     uint32_t key[2] = { (uint32_t)(s->seed & 0xFFFFFFFFu), (uint32_t)(s->seed >> 32) };
     orc_philox4x32_10(ctr, key, x);
 }
 
 /* Skill draw number d of an agent: Philox stream 16, "t" field = d/4, word d%4 (G30).
  * NORMAL_CLIP (f3, G42): stream 17, "t" fields 3d, 3d+1, 3d+2 give the twelve words of draw d. */
-static float skill_draw(const orc_sim* s, uint32_t env_gid, uint32_t agent, int32_t d) {
+static float skill_draw(const orc_sim* s, uint32_t episode, uint32_t env_gid, uint32_t agent, int32_t d) {
     uint32_t x[4];
     if (s->p.skill_init == ORC_SKILL_NORMAL_CLIP) {
         uint32_t w[12];
-        for (int32_t j = 0; j < 3; ++j) draw(s, env_gid, agent, (uint32_t)(3 * d + j), 17u, &w[4 * j]);
+        for (int32_t j = 0; j < 3; ++j) draw(s, episode, env_gid, agent, (uint32_t)(3 * d + j), 17u, &w[4 * j]);
         return orc_normal_skill(w, s->p.skill_mean, s->p.skill_std, s->p.skill_clip_lo, s->p.skill_clip_hi);
     }
-    draw(s, env_gid, agent, (uint32_t)(d / 4), 16u, x);
+    draw(s, episode, env_gid, agent, (uint32_t)(d / 4), 16u, x);
     float u = orc_u01(x[d % 4]);
     if (s->p.skill_init == ORC_SKILL_UNIFORM01) return u;
     /* Pareto(alpha=4, x_m=1) by inversion with correctly rounded ops only (G29, 8(c) "Skill init"). */
@@ -343,33 +346,43 @@ static double env_welfare(const orc_sim* s, const orc_env* v) {
     return ug;
 }
 
-/* every agent holds starting_coin, nothing else; books empty; rates zero; t = 0. */
+/* every agent holds starting_coin, nothing else; books empty; rates zero; t = 0.  Skills are drawn anew
+ * from the counters of the given episode (f4, G44); the counters (trades, invalid actions, ...) keep running over
+ * episodes. */
+static void init_env(const orc_sim* s, orc_env* v, uint32_t gid, int32_t episode, int32_t clear_counters) {
+    const int32_t N = s->N, R = s->R;
+    v->t = 0;
+    v->episode = episode;
+    for (int32_t i = 0; i < N; ++i) {
+        v->coin[i] = s->p.starting_coin;
+        v->labor[i] = 0.0f;
+        v->income[i] = 0.0f;
+        v->esc_coin[i] = 0;
+        v->n_live[i] = 0;
+        for (int32_t r = 0; r < R; ++r) {
+            v->inv[i * R + r] = 0;
+            v->esc_res[i * R + r] = 0;
+            v->SG[i * R + r] = skill_draw(s, (uint32_t)episode, gid, (uint32_t)i, r);
+        }
+        v->SC[i] = skill_draw(s, (uint32_t)episode, gid, (uint32_t)i, R);
+    }
+    for (int32_t b = 0; b < 2 * R; ++b) v->book[b].n = 0;
+    for (int32_t r = 0; r < R; ++r) v->last_price[r] = 0;
+    for (int32_t b = 0; b < ORC_MAX_BRACKETS; ++b) v->rates[b] = 0.0f;
+    if (clear_counters) v->n_trades = v->n_placed = v->n_invalid = v->n_expired = v->n_bad_gov = 0;
+    v->u_g_prev = env_welfare(s, v);
+}
+
 void orc_reset(orc_sim* s, uint64_t seed) {
     s->seed = seed;
-    const int32_t N = s->N, R = s->R;
-    for (int32_t e = 0; e < s->E; ++e) {
-        orc_env* v = &s->env[e];
-        uint32_t gid = s->p.env_id_base + (uint32_t)e;
-        v->t = 0;
-        for (int32_t i = 0; i < N; ++i) {
-            v->coin[i] = s->p.starting_coin;
-            v->labor[i] = 0.0f;
-            v->income[i] = 0.0f;
-            v->esc_coin[i] = 0;
-            v->n_live[i] = 0;
-            for (int32_t r = 0; r < R; ++r) {
-                v->inv[i * R + r] = 0;
-                v->esc_res[i * R + r] = 0;
-                v->SG[i * R + r] = skill_draw(s, gid, (uint32_t)i, r);
-            }
-            v->SC[i] = skill_draw(s, gid, (uint32_t)i, R);
-        }
-        for (int32_t b = 0; b < 2 * R; ++b) v->book[b].n = 0;
-        for (int32_t r = 0; r < R; ++r) v->last_price[r] = 0;
-        for (int32_t b = 0; b < ORC_MAX_BRACKETS; ++b) v->rates[b] = 0.0f;
-        v->n_trades = v->n_placed = v->n_invalid = v->n_expired = v->n_bad_gov = 0;
-        v->u_g_prev = env_welfare(s, v);
-    }
+    for (int32_t e = 0; e < s->E; ++e) init_env(s, &s->env[e], s->p.env_id_base + (uint32_t)e, 0, 1);
+}
+
+/* f4 (G44): start episode `episode` in envs [env_begin, +env_count): the state of a reset, with every random draw of
+ * the episode keyed by its index.  orc_reset = episode 0 everywhere. */
+void orc_begin_episode(orc_sim* s, int32_t env_begin, int32_t env_count, int32_t episode) {
+    for (int32_t k = 0; k < env_count; ++k)
+        init_env(s, &s->env[env_begin + k], s->p.env_id_base + (uint32_t)(env_begin + k), episode, 0);
 }
 
 /* Observation layouts: SURVEY 8(c) "Population observation layout" / "Government observation
@@ -481,7 +494,7 @@ static void step_env(const orc_sim* s, orc_env* v, uint32_t gid, const int32_t* 
     int32_t n_cand = 0;
     for (int32_t i = 0; i < N; ++i) {
         uint32_t x[4];
-        draw(s, gid, (uint32_t)i, (uint32_t)t, 0u, x);
+        draw(s, (uint32_t)v->episode, gid, (uint32_t)i, (uint32_t)t, 0u, x);
         const int32_t a = act[i];
         if (a < 0 || a >= A) { v->n_invalid++; continue; } /* G2 */
         if (a < R) { /* gather r */
@@ -655,6 +668,30 @@ void orc_step(orc_sim* s, int32_t env_begin, int32_t env_count, const int32_t* a
     }
 }
 
+/* f4 (G44), the step of an auto-resetting rollout: the plain step; an env whose episode ends with it (done = 1)
+ * then starts its next episode at once, and the observation returned for that step is the one of the fresh state
+ * (the terminal observation is not returned: the caller's policy acts on what it is given next).  Rewards and done are
+ * those of the step itself. */
+void orc_step_auto(orc_sim* s, int32_t env_begin, int32_t env_count, const int32_t* actions,
+                   const int32_t* gov_actions, float* obs_pop, float* obs_gov, float* rew, uint8_t* done) {
+    const size_t N = (size_t)s->N, B = (size_t)s->p.num_brackets;
+    const size_t Dp = (size_t)orc_obs_dim_pop(s), Dg = (size_t)orc_obs_dim_gov(s);
+    for (int32_t k = 0; k < env_count; ++k) {
+        const int32_t e = env_begin + k;
+        orc_env* v = &s->env[e];
+        uint8_t d = 0;
+        float* op = obs_pop ? obs_pop + (size_t)k * N * Dp : NULL;
+        float* og = obs_gov ? obs_gov + (size_t)k * Dg : NULL;
+        step_env(s, v, s->p.env_id_base + (uint32_t)e, actions + (size_t)k * N, gov_actions + (size_t)k * B, op, og,
+                 rew ? rew + (size_t)k * (N + 1) : NULL, &d);
+        if (done) done[k] = d;
+        if (d) {
+            orc_begin_episode(s, e, 1, v->episode + 1);
+            if (op || og) build_obs(s, v, 0, op, og);
+        }
+    }
+}
+
 /* f3 (G41): one correctly rounded binary32 operation per step of the formula. */
 float orc_progress_skill(float skill, float rate, float max) {
     const float frac = skill / max;
@@ -690,14 +727,14 @@ void orc_draw_actions(const orc_sim* s, int32_t env_begin, int32_t env_count, co
         const uint32_t t = (uint32_t)s->env[e].t;
         for (int32_t i = 0; i < N; ++i) {
             uint32_t x[4];
-            draw(s, gid, (uint32_t)i, t, 0u, x);
+            draw(s, (uint32_t)s->env[e].episode, gid, (uint32_t)i, t, 0u, x);
             int32_t a = 0;
             while (a < A - 1 && !(x[0] < cdf[a])) ++a;
             actions[(size_t)k * N + i] = a;
         }
         for (int32_t b = 0; b < B; ++b) {
             uint32_t x[4];
-            draw(s, gid, (uint32_t)N, t, (uint32_t)(1 + b / 4), x);
+            draw(s, (uint32_t)s->env[e].episode, gid, (uint32_t)N, t, (uint32_t)(1 + b / 4), x);
             gov_actions[(size_t)k * B + b] = (int32_t)(((uint64_t)x[b % 4] * (uint64_t)s->p.num_rate_levels) >> 32);
         }
     }
@@ -708,7 +745,7 @@ static int32_t dump_cap(const orc_sim* s) { return s->N * s->p.max_active_orders
 
 size_t orc_state_words(const orc_sim* s) {
     const size_t N = (size_t)s->N, R = (size_t)s->R, B = (size_t)s->p.num_brackets;
-    return 13 + B + R + N * (6 + 3 * R) + 2 * R * (1 + 3 * (size_t)dump_cap(s));
+    return 13 + B + R + N * (6 + 3 * R) + 2 * R * (1 + 3 * (size_t)dump_cap(s)) + 1;  /* last word: episode (f4) */
 }
 
 static int32_t f2w(float f) { int32_t w; memcpy(&w, &f, 4); return w; }
@@ -754,6 +791,7 @@ void orc_get_state(const orc_sim* s, int32_t env_begin, int32_t env_count, int32
             free(c);
             q = q0 + 3 * (size_t)cap;
         }
+        w[q++] = v->episode;
     }
 }
 
@@ -846,7 +884,7 @@ void orc_draw_actions_masked(const orc_sim* s, int32_t env_begin, int32_t env_co
         orc_action_mask(s, e, 1, mask);
         for (int32_t i = 0; i < N; ++i) {
             uint32_t x[4];
-            draw(s, gid, (uint32_t)i, t, 0u, x);
+            draw(s, (uint32_t)s->env[e].episode, gid, (uint32_t)i, t, 0u, x);
             uint64_t S = 0;
             for (int32_t a = 0; a < A; ++a) {
                 const uint64_t hi = (a == A - 1) ? ((uint64_t)1 << 32) : (uint64_t)cdf[a];

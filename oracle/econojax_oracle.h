@@ -143,6 +143,13 @@ const char* orc_last_error(void);
 int32_t orc_obs_dim_pop(const orc_sim* s); /* 6 + 8R + B */
 int32_t orc_obs_dim_gov(const orc_sim* s); /* 3(3+R) + B + 2 */
 void orc_reset(orc_sim* s, uint64_t seed);
+/* f4 (G44): envs [env_begin, +env_count) start episode `episode`: the state of a reset, every random draw of the
+ * episode keyed by (seed, env, agent, t, stream | episode << 8).  orc_reset starts episode 0 everywhere. */
+void orc_begin_episode(orc_sim* s, int32_t env_begin, int32_t env_count, int32_t episode);
+/* f4: orc_step for an auto-resetting rollout: an env whose episode ends with this step starts its next episode at
+ * once and returns the observation of the fresh state; rewards and done are the step's own. */
+void orc_step_auto(orc_sim* s, int32_t env_begin, int32_t env_count, const int32_t* actions,
+                   const int32_t* gov_actions, float* obs_pop, float* obs_gov, float* rew, uint8_t* done);
 /* Observation of the current state of envs [env_begin, env_begin+env_count) (used after reset). */
 void orc_observe(orc_sim* s, int32_t env_begin, int32_t env_count, float* obs_pop, float* obs_gov);
 /* One step of envs [env_begin, env_begin+env_count).  actions [env_count][N], gov_actions

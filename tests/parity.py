@@ -174,7 +174,7 @@ def check_dump_invariants(w, cfg, steps):
         both = valid[:, 1:] & valid[:, :-1] & (d == 0)
         assert (np.diff(book[:, :, 2], axis=1)[both] >= 0).all()
         best[b] = np.where(n > 0, book[:, 0, 0], -1)
-    assert q == w.shape[1]
+    assert q + 1 == w.shape[1] and (w[:, q] >= 0).all()             # last word: episode index (f4)
     assert (want_coin == esc_coin).all() and (want_res == esc_res).all()            # escrow = sum of live orders
     assert (live == n_live).all() and live.max() <= M
     for r in range(R):                                                               # uncrossed after matching

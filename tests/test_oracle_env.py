@@ -595,3 +595,75 @@ def test_sharded_oracle_helper_equals_one_oracle():
             res = o.step(acts[s][lo:lo + o.E], gov[s][lo:lo + o.E])
             assert np.array_equal(outs[s][4][lo:lo + o.E], res[2])
     assert np.array_equal(sh.state(), np.concatenate([o.get_state() for o in ones]))
+
+
+# ---------------- f4: episodes and auto-reset (G44) ----------------
+def test_episode_keying_and_begin_episode(small_params):
+    """Every random draw of an episode is keyed by (seed, env, agent, t, stream | episode << 8): episode 0 draws what
+    G30's counters draw (all other tests pin that), a later episode is recomputed here from orc_philox4x32_10."""
+    import ctypes as C
+
+    L = oracle.lib()
+
+    def philox(ctr, key):
+        c, k, o = (C.c_uint32 * 4)(*ctr), (C.c_uint32 * 2)(*key), (C.c_uint32 * 4)()
+        L.orc_philox4x32_10(c, k, o)
+        return list(o)
+
+    p = dict(small_params, starting_coin=15.0, env_id_base=9)          # uniform skills: skill = (x >> 8) * 2^-24
+    seed = 0xABCDEF0123
+    key = [seed & 0xFFFFFFFF, seed >> 32]
+    env = make(2, 3, 2, p, seed=seed)
+    first = env.get_state().copy()
+    assert [st(env, e)["episode"] for e in range(2)] == [0, 0]
+    acts, gov = inputs.action_stream(dict(E=2, N=3, R=2, T=50, seed=1, action_mix="uniform", params=p), 5, seed=1, E=2)
+    for t in range(5):
+        env.step(acts[t], gov[t], want_obs=False)
+    env.begin_episode(3, env_begin=1, env_count=1)                      # env 1 only
+    s0, s1 = st(env, 0), st(env, 1)
+    assert s0["t"] == 5 and s0["episode"] == 0 and s1["t"] == 0 and s1["episode"] == 3
+    assert (s1["coin"] == 15.0).all() and not s1["inv"].any() and (s1["labor"] == 0).all() and all(len(b) == 0 for b in s1["books"])
+    assert s1["counters"].sum() >= 0 and (s1["counters"] == oracle.parse_state(env.get_state()[1])["counters"]).all()
+    for i in range(3):
+        x = philox([9 + 1, i, 0, 16 | (3 << 8)], key)                  # skill draws d = 0, 1, 2 are words 0, 1, 2 of block 0
+        want = [np.float32((w >> 8) * 2.0 ** -24) for w in x[:3]]
+        assert s1["SG"][i].tolist() == want[:2] and s1["SC"][i] == want[2]
+    assert (s1["SG"] != oracle.parse_state(first[1])["SG"]).any()        # not the skills of episode 0
+    # the step draws of the new episode: the arrival key of a placed order is word 2 of stream 0 | 3 << 8
+    cdf = inputs.action_cdf(dict(E=2, N=3, R=2, T=50, seed=1, action_mix="uniform", params=p))
+    a1, _ = env.draw_actions(cdf, env_begin=1, env_count=1)
+    x0 = philox([10, 0, 0, 0 | (3 << 8)], key)[0]
+    assert a1[0, 0] == int(np.searchsorted(cdf.astype(np.uint64), x0, side="right"))
+    env.begin_episode(0, env_begin=1, env_count=1)
+    assert (env.get_state()[1][:6] == first[1][:6]).all() and (st(env, 1)["SG"] == oracle.parse_state(first[1])["SG"]).all()
+
+
+def test_auto_reset_equals_reset_T_steps_reset_T_steps():
+    """orc_step_auto over 2 T + 3 steps = episode 0 for T steps, begin_episode(1), T steps, begin_episode(2), 3 steps; the
+    observation of the step that ends an episode is the one of the fresh state; rewards and done are the step's own."""
+    cfg = inputs.configs()["tiny_dense"]
+    T, E = cfg["T"], 3
+    acts, gov = inputs.action_stream(cfg, 2 * T + 3, seed=5, E=E)
+    a = make(E, cfg["N"], cfg["R"], cfg["params"], seed=5)
+    b = make(E, cfg["N"], cfg["R"], cfg["params"], seed=5)
+    n_done = 0
+    for t in range(2 * T + 3):
+        pa, ga, ra, da = a.step(acts[t], gov[t], auto_reset=True)
+        pb, gb, rb, db = b.step(acts[t], gov[t])
+        assert np.array_equal(ra, rb) and np.array_equal(da, db)
+        if (t + 1) % T == 0:
+            assert (da == 1).all()
+            n_done += 1
+            b.begin_episode((t + 1) // T)
+            pb, gb = b.observe()
+            assert pb[0, 0, -1] == 0.0 and pb[0, 0, 0] == np.float32(cfg["params"]["starting_coin"]) * np.float32(0.01)
+        else:
+            assert (da == 0).all()
+        assert np.array_equal(pa, pb) and np.array_equal(ga, gb)
+        assert np.array_equal(a.get_state(), b.get_state())
+    assert n_done == 2 and st(a)["episode"] == 2 and st(a)["t"] == 3
+    # the second episode is not a replay of the first
+    c = make(E, cfg["N"], cfg["R"], cfg["params"], seed=5)
+    for t in range(3):
+        c.step(acts[2 * T + t], gov[2 * T + t], want_obs=False)
+    assert (st(c)["inv"] != st(a)["inv"]).any() or (st(c)["SG"] != st(a)["SG"]).any()
