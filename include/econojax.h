@@ -138,6 +138,16 @@ typedef struct ej_rollout_io {
     float* obs_priv_ring;             /* [ring_depth][E][N][3R + 4] */
     float* obs_shared_ring;           /* [ring_depth][E][ceil4(5R + B + 2)] */
     float* obs_gov_ring;              /* [ring_depth][E][D_gov_pad] government rows (optional) */
+    /* f4 (the rollout a PPO loop runs; G44).  auto_reset != 0: an env whose episode ends at a step
+     * (done = 1 in done_ring) starts its next episode within the same step -- the state of ej_reset, every random draw
+     * of the new episode keyed by (seed, global env, agent, t, stream | episode << 8), event counters kept -- and the
+     * observation written for that step is the one of the fresh state (the one the policy acts on next; the terminal
+     * observation is not written).  Rewards and done are the step's own, so with ring_depth = T the rings rew_ring
+     * [T][E][N+1] and done_ring [T][E] are what a backward GAE scan reads.  An env already finished when the call begins
+     * starts its next episode with the call's first step.  auto_reset == 0 (default): envs stay done (G28).  Not available
+     * together with the factored observation rings (EJ_ERR_PARAM). */
+    int32_t auto_reset;
+    int32_t reserved0;
 } ej_rollout_io;
 
 /* One tanh MLP  in_dim -> 128 -> 128 -> out_dim  (Table 2; BASELINE.json
@@ -217,7 +227,7 @@ int ej_step_host_factored(ej_env* h, const int32_t* actions, const int32_t* gov_
 /* T steps in ONE persistent launch: each env's state stays in shared memory for the whole
  * call.  Actions come from io->actions_in / gov_actions_in or, when NULL, from the Philox/CDF
  * generator (ej_set_action_cdf; uniform over the A actions by default).  io may be NULL
- * (no outputs).  No auto-reset: envs that reach episode_length stay done (G28).
+ * (no outputs).  Envs that reach episode_length stay done (G28) unless io->auto_reset is set (f4).
  * Limits (EJ_ERR_PARAM): ring_depth * obs_floats < 2^32 and, with actions_in, T * E * N < 2^32
  * (the kernels index rings and action streams with 32-bit element offsets). */
 int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* io);

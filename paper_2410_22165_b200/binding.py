@@ -60,6 +60,7 @@ class EjRolloutIO(C.Structure):
         ("actions_ring", C.c_void_p), ("gov_actions_ring", C.c_void_p),
         ("pop_logits_ring", C.c_void_p), ("gov_logits_ring", C.c_void_p),
         ("obs_priv_ring", C.c_void_p), ("obs_shared_ring", C.c_void_p), ("obs_gov_ring", C.c_void_p),
+        ("auto_reset", C.c_int32), ("reserved0", C.c_int32),
     ]
 
 
@@ -384,7 +385,7 @@ class Env:
 
     def rollout(self, T, ring_depth=1, actions_in=None, gov_actions_in=None, obs_ring=None, rew_ring=None,
                 done_ring=None, actions_ring=None, gov_actions_ring=None, pop_logits_ring=None, gov_logits_ring=None,
-                obs_priv_ring=None, obs_shared_ring=None, obs_gov_ring=None):
+                obs_priv_ring=None, obs_shared_ring=None, obs_gov_ring=None, auto_reset=False):
         io = EjRolloutIO()
         io.struct_size = C.sizeof(EjRolloutIO)
         io.ring_depth = ring_depth
@@ -393,6 +394,7 @@ class Env:
         io.actions_ring, io.gov_actions_ring = _dp(actions_ring), _dp(gov_actions_ring)
         io.pop_logits_ring, io.gov_logits_ring = _dp(pop_logits_ring), _dp(gov_logits_ring)
         io.obs_priv_ring, io.obs_shared_ring, io.obs_gov_ring = _dp(obs_priv_ring), _dp(obs_shared_ring), _dp(obs_gov_ring)
+        io.auto_reset = 1 if auto_reset else 0
         ej_rollout(self.h, T, io)
 
     # f2, factored observations: the three rings of one step (widths from ej_layout)

@@ -3,6 +3,7 @@
 // ej_device.cuh.  Everything on the step path runs on the device; this file only marshals.
 #include <cuda_runtime.h>
 #include <math.h>
+#include <stddef.h>
 #include <stdint.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -56,6 +57,7 @@ struct ej_env {
     // the step kernel variant of this handle's shape (CTA size, array stride, specialised R / P)
     void (*step_fn)(const DevCfg, uint8_t*, const StepIO) = nullptr;
     void (*step_fn_fx)(const DevCfg, uint8_t*, const StepIO) = nullptr;  // f2: factored observations
+    void (*step_fn_ar)(const DevCfg, uint8_t*, const StepIO) = nullptr;  // f4: auto-resetting rollouts
     int step_RT = 0, step_PT = 0, step_pf = 0;
 };
 
@@ -196,6 +198,7 @@ template <int MT, int NS>
 void select_step_kernel(ej_env* h) {
     const DevCfg& c = h->c;
     h->step_fn = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0>;
+    h->step_fn_ar = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0, 0, 1>;
     h->step_fn_fx = nullptr;  // f2 variants exist for CTAs of up to 256 threads (build time)
     if constexpr (MT <= 256) h->step_fn_fx = ej_step_kernel<MT, NS, 0, 0, 0, 0, 0, 1>;
     h->step_RT = h->step_PT = 0;
@@ -214,6 +217,7 @@ void select_step_kernel(ej_env* h) {
         }
         if (c.R == RT && c.P == PT && (NT == 0 || (c.N == NT && c.B == BT)) && (PF == 0 || (paper && lay_ok))) {
             h->step_fn = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF>;
+            h->step_fn_ar = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF, 0, 1>;
             h->step_pf = PF;
             // f2: the factored variant must read the same (16-bit) order pool as the dense one
             if constexpr (PF == 1) h->step_fn_fx = ej_step_kernel<MT, NS, RT, PT, NT, BT, PF, 1>;
@@ -259,7 +263,7 @@ int launch_step(ej_env* h, const StepIO& io) {
         return fail(h, EJ_ERR_PARAM, "bad field: %s", "observation pointer (must be 16-byte aligned)");
     if (misaligned4(io.actions) || misaligned4(io.gov_actions) || misaligned4(io.rew) || misaligned4(io.actions_out) || misaligned4(io.gov_out))
         return fail(h, EJ_ERR_PARAM, "bad field: %s", "actions / rewards pointer (must be 4-byte aligned)");
-    (io.obs_priv ? h->step_fn_fx : h->step_fn)<<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, io);
+    (io.obs_priv ? h->step_fn_fx : io.auto_reset ? h->step_fn_ar : h->step_fn)<<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, io);
     h->launches++;
     EJ_CUDA(h, cudaGetLastError(), "ej_step_kernel launch");
     return EJ_OK;
@@ -287,6 +291,7 @@ int set_smem_attr(ej_env* h) {
         constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
         select_step_kernel<MT, NS>(h);
         EJ_CUDA(h, raise_smem_attr((const void*)h->step_fn, c.smem_bytes), "smem attr (step)");
+        EJ_CUDA(h, raise_smem_attr((const void*)h->step_fn_ar, c.smem_bytes), "smem attr (step, auto-reset)");
         if (h->step_fn_fx) EJ_CUDA(h, raise_smem_attr((const void*)h->step_fn_fx, c.smem_bytes), "smem attr (step, factored)");
         EJ_CUDA(h, raise_smem_attr((const void*)ej_observe_kernel<MT, NS>, c.smem_bytes), "smem attr (observe)");
         EJ_CUDA(h, raise_smem_attr((const void*)ej_reset_kernel<MT, NS>, c.smem_bytes), "smem attr (reset)");
@@ -296,7 +301,7 @@ int set_smem_attr(ej_env* h) {
 
 size_t state_words(const DevCfg& c) {
     const size_t N = c.N, R = c.R, B = c.B, cap = (size_t)c.N * c.M;
-    return 13 + B + R + N * (6 + 3 * R) + 2 * R * (1 + 3 * cap);
+    return 13 + B + R + N * (6 + 3 * R) + 2 * R * (1 + 3 * cap) + 1;  // last word: episode index (f4)
 }
 
 int32_t f2w(float f) { int32_t w; memcpy(&w, &f, 4); return w; }
@@ -380,7 +385,7 @@ void fill_job(ej_env* h, PolicyArgs& a, const PolicyNet& net, const float* obs, 
     memset(&a, 0, sizeof(a));
     a.net = net;
     a.obs = obs; a.row_stride = row_stride; a.rows = rows; a.rows_per_env = rows_per_env; a.fixed_agent = fixed_agent;
-    a.state = h->d_state; a.blob_stride = c.blob_bytes;
+    a.state = h->d_state; a.blob_stride = c.blob_bytes; a.o_episode = (int)offsetof(EnvHdr, episode);
     a.env_id_base = c.env_id_base; a.seed_lo = c.seed_lo; a.seed_hi = c.seed_hi; a.stream_base = stream_base;
     a.actions = actions; a.logits = logits;
     a.smem_W1 = 0;
@@ -465,7 +470,7 @@ int rollout_with_policy(ej_env* h, int T, const ej_rollout_io* rio, const StepIO
         if (gov_supplied) gov = const_cast<int32_t*>(base.gov_actions + (size_t)s * EB);
         StepIO io;
         memset(&io, 0, sizeof(io));
-        io.cdf = base.cdf; io.n_steps = 1; io.ring_depth = 1;
+        io.cdf = base.cdf; io.n_steps = 1; io.ring_depth = 1; io.auto_reset = base.auto_reset;
         io.actions = act; io.gov_actions = gov;
         io.obs = base.obs ? base.obs + (size_t)slot * c.obs_floats : h->d_pobs;
         io.rew = base.rew ? base.rew + (size_t)slot * (EN + c.E) : nullptr;
@@ -766,12 +771,14 @@ int ej_rollout(ej_env* h, int32_t T, const ej_rollout_io* rio) {
         io.actions = rio->actions_in; io.gov_actions = rio->gov_actions_in;
         io.obs = rio->obs_ring; io.rew = rio->rew_ring; io.done = rio->done_ring;
         io.actions_out = rio->actions_ring; io.gov_out = rio->gov_actions_ring;
+        io.auto_reset = rio->auto_reset ? 1 : 0;
         if (rio->obs_priv_ring || rio->obs_shared_ring || rio->obs_gov_ring) {  // f2: factored observations
             const DevCfg& c = h->c;
             if (!rio->obs_priv_ring || !rio->obs_shared_ring) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring / io.obs_shared_ring (set both)");
             if (rio->obs_ring) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_ring (must be NULL with factored observations)");
             if (!h->step_fn_fx || !c.stage_obs || (c.N * (3 * c.R + 4)) % 4 != 0) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring (shape cannot stage factored observations)");
             if (h->has_policy && !rio->actions_in) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.obs_priv_ring (not available in policy mode)");
+            if (rio->auto_reset) return fail(h, EJ_ERR_PARAM, "bad field: %s", "io.auto_reset (not available with factored observations)");
             io.obs_priv = rio->obs_priv_ring; io.obs_shared = rio->obs_shared_ring; io.obs_gov = rio->obs_gov_ring;
         }
     }
@@ -909,6 +916,7 @@ int ej_get_state(ej_env* h, int32_t env_begin, int32_t env_count, int32_t* words
             }
             q = q0 + 3 * (size_t)cap;
         }
+        w[q++] = hd->episode;
     }
     return EJ_OK;
 }
@@ -990,6 +998,8 @@ int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t*
             if ((b & 1) == 0 && n == 0) best_bid = 0;
             q += 3 * (size_t)cap;
         }
+        hd->episode = w[q++];
+        if (hd->episode < 0 || hd->episode >= (1 << 24)) return fail(h, EJ_ERR_PARAM, "bad field: %s", "words (episode)");
     }
     EJ_CUDA(h, cudaStreamSynchronize(h->stream), "set_state sync");
     EJ_CUDA(h, cudaMemcpy(h->d_state + (size_t)env_begin * c.blob_bytes, blobs.data(), blobs.size(), cudaMemcpyHostToDevice), "set_state copy");

@@ -31,7 +31,7 @@
 #include "../../include/econojax.h"
 
 #ifndef EJ_CTAS_128
-#define EJ_CTAS_128 9  // resident 128-thread CTAs per SM the step kernel is compiled for (registers)
+#define EJ_CTAS_128 8  // resident 128-thread CTAs per SM the step kernel is compiled for (register budget 64; 9 fit the shared memory at the headline shape but measured no faster)
 #endif
 
 namespace {
@@ -87,7 +87,7 @@ struct EnvHdr {
     uint32_t med_prev[2 + EJ_MAX_RESOURCES];  // previous lower medians of labor, income (float bits) and inv[r]: hints, not state
     double u_g_prev;
     int32_t t_in_period;  // t % tax_period, kept incrementally (no integer division on the step path)
-    int32_t pad1;
+    int32_t episode;      // f4: episode index (0 after ej_reset), part of every Philox counter: stream | episode << 8 (G44)
     float rates[EJ_MAX_BRACKETS];
     int32_t last_price[EJ_MAX_RESOURCES];
 };
@@ -135,6 +135,7 @@ struct StepIO {
     const uint32_t* cdf;         // [A] device
     int n_steps, ring_depth;
     int masked;                  // f1: the generator draws among the available actions only
+    int auto_reset;              // f4: an env whose episode ends starts the next one in the same step (G44)
     float* obs_priv;             // f2 rings (factored observations): [E][N][3R+4], [E][ceil4(5R+B+2)], [E][D_gov_pad]
     float* obs_shared;
     float* obs_gov;
@@ -1035,6 +1036,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
     constexpr int N4 = NS;  // stride of the per-agent arrays
     const bool act = tid < N;
     const uint32_t gid = c.env_id_base + (uint32_t)e;
+    const uint32_t ep_bits = (uint32_t)m.hdr()->episode << 8;  // G44: the episode index in the upper bits of the stream word
     int* cnt_cur = m.cnt() + (t & 1) * nl;
     int* cnt_nxt = m.cnt() + ((t & 1) ^ 1) * nl;
 
@@ -1042,7 +1044,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
     uint32_t x0 = 0, x1 = 0, x2 = 0, x3 = 0;
     int a = -1;
     if (act) {
-        philox4x32_10(gid, (uint32_t)tid, (uint32_t)t, 0u, c.seed_lo, c.seed_hi, x0, x1, x2, x3);
+        philox4x32_10(gid, (uint32_t)tid, (uint32_t)t, ep_bits, c.seed_lo, c.seed_hi, x0, x1, x2, x3);
         if (io.io.actions) {
             a = io.actions()[(uint32_t)(e * N + tid)];
         } else if (io.io.masked) {
@@ -1069,7 +1071,7 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
             gov_lvl = io.gov_actions()[(uint32_t)(e * B + tid)];
         } else {
             uint32_t g0, g1, g2, g3;
-            philox4x32_10(gid, (uint32_t)N, (uint32_t)t, (uint32_t)(1 + tid / 4), c.seed_lo, c.seed_hi, g0, g1, g2, g3);
+            philox4x32_10(gid, (uint32_t)N, (uint32_t)t, (uint32_t)(1 + tid / 4) | ep_bits, c.seed_lo, c.seed_hi, g0, g1, g2, g3);
             const uint32_t gx = (tid & 3) == 0 ? g0 : (tid & 3) == 1 ? g1 : (tid & 3) == 2 ? g2 : g3;
             gov_lvl = (int)(((unsigned long long)gx * (unsigned long long)c.L) >> 32);
         }
@@ -1429,13 +1431,108 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
     rows = (first || c.skill_rate > 0.0f) ? 2 : (boundary ? 1 : 0);
 }
 
+// Initial state of an episode (G29, G30, G44) in the shared-memory blob: every agent holds starting_coin and
+// nothing else, books empty, rates 0, t = 0, skills drawn from the counters of (seed, global env, agent, episode).  The
+// env's event counters are cleared only by ej_reset.  Called by all threads; the caller synchronises afterwards.
+template <int NPAD, int NS, class SM>
+__device__ __noinline__ void init_env_state(const DevCfg& c, const SM& m, int tid, uint32_t gid, int episode, bool clear_counters) {
+    const uint32_t ep = (uint32_t)episode << 8;
+    if (tid < c.N) {
+        m.coin()[tid] = c.starting_coin;
+        m.cf()[tid] = coin_utility(c.starting_coin, c.ua, c.inv_ua);
+        m.labor()[tid] = 0.0f;
+        m.income()[tid] = 0.0f;
+        m.esc_coin()[tid] = 0;
+        m.mask()[tid] = 0u;
+        for (int r = 0; r < c.R; ++r) { m.inv()[r * NS + tid] = 0; m.esc_res()[r * NS + tid] = 0; }
+        uint32_t x[4] = {0, 0, 0, 0};
+        for (int d = 0; d <= c.R; ++d) {  // skill draw d: Philox stream 16, "t" field d/4, word d%4
+            if ((d & 3) == 0) philox4x32_10(gid, (uint32_t)tid, (uint32_t)(d >> 2), 16u | ep, c.seed_lo, c.seed_hi, x[0], x[1], x[2], x[3]);
+            const uint32_t w = (d & 3) == 0 ? x[0] : (d & 3) == 1 ? x[1] : (d & 3) == 2 ? x[2] : x[3];
+            float v = u01(w);
+            if (c.skill_init == EJ_SKILL_NORMAL_CLIP) {
+                // f3 (P:345; G42): z = sum of twelve 24-bit uniforms - 6 (stream 17, "t" fields 3d .. 3d+2); the
+                // sum is an integer, z and std * z are exact in binary64, one rounding to binary32, then the clip
+                long long sum = 0;
+                for (int j = 0; j < 3; ++j) {
+                    uint32_t y0, y1, y2, y3;
+                    philox4x32_10(gid, (uint32_t)tid, (uint32_t)(3 * d + j), 17u | ep, c.seed_lo, c.seed_hi, y0, y1, y2, y3);
+                    sum += (long long)(y0 >> 8) + (long long)(y1 >> 8) + (long long)(y2 >> 8) + (long long)(y3 >> 8);
+                }
+                const double z = __dsub_rn(__dmul_rn((double)sum, 1.0 / 16777216.0), 6.0);
+                v = __double2float_rn(__dadd_rn((double)c.skill_mean, __dmul_rn((double)c.skill_std, z)));
+                if (v < c.clip_lo) v = c.clip_lo;
+                if (v > c.clip_hi) v = c.clip_hi;
+            } else if (c.skill_init == EJ_SKILL_PARETO_CLIP) {  // Pareto(4) by inversion: 1/sqrt(sqrt(1-u))
+                float rr = __fsqrt_rn(__fsub_rn(1.0f, v));
+                rr = __fsqrt_rn(rr);
+                v = __fdiv_rn(1.0f, rr);
+                if (v < c.clip_lo) v = c.clip_lo;
+                if (v > c.clip_hi) v = c.clip_hi;
+            }
+            if (d < c.R) m.SG()[d * NS + tid] = v;
+            else m.SC()[tid] = v;
+        }
+    }
+    for (int l = tid; l < c.n_levels; l += NPAD) {
+        m.head()[l] = (uint16_t)NIL;
+        m.tail()[l] = (uint16_t)NIL;
+        m.cnt()[l] = 0;
+        m.cnt()[c.n_levels + l] = 0;
+    }
+    if (tid < EJ_MAX_BRACKETS) m.hdr()->rates[tid] = 0.0f;
+    if (tid < EJ_MAX_RESOURCES) m.hdr()->last_price[tid] = 0;
+    if (tid == 0) {  // all coins equal: gini = 0, prod = N * coin (exact)
+        EnvHdr* hd = m.hdr();
+        hd->t = 0;
+        hd->t_in_period = 0;
+        hd->episode = episode;
+        if (clear_counters) hd->n_trades = hd->n_placed = hd->n_invalid = hd->n_expired = hd->n_bad_gov = 0;
+        const double prod = (double)c.N * (double)c.starting_coin;
+        const double eq = (double)c.omega * (1.0 - 0.0) + (1.0 - (double)c.omega);
+        hd->u_g_prev = eq * prod;
+    }
+}
+
+// f4 (G44), the cold half of an auto-resetting step: the episode has just ended and its rewards are out; start the next
+// episode and write the fresh state's observation.  Out of line, with its own copy of outputs(): the hot path of a
+// step keeps its single inlined call.
+template <int NPAD, int NS, int RT, int NT, int BT, int PF, int FX, class SM>
+__device__ __noinline__ void renew_episode(const DevCfg& c, const SM& m, int tid, int e, const StepPtrs& io) {
+    const int ep = m.hdr()->episode + 1;
+    __syncthreads();  // the rewards and statistics of the terminal state are done
+    init_env_state<NPAD, NS>(c, m, tid, c.env_id_base + (uint32_t)e, ep, false);
+    __syncthreads();
+    if (tid < c.R) write_market_row<0>(c, m, tid, m.cnt());
+    if (tid < c.B) m.shrow()[5 * c.R + tid] = 0.0f;
+    if (tid == NPAD - 1) write_timers(c, m, 0, 0);
+    if (SM::L::bucketed) bucket_fill_all<NPAD>(m, tid, tid < c.N);
+    __syncthreads();
+    outputs<NPAD, NS, RT, NT, BT, PF, FX>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, io.obs(), nullptr, FX ? io.priv() : nullptr, FX ? io.shared() : nullptr,
+                                          FX ? io.govp() : nullptr);
+}
+
 // One environment step: P1-P4 (or nothing for a finished env, G28), then P5 rewards and P6
-// observations.  outputs() has this single call site (instruction footprint).
-template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX, class SM>
+// observations.  outputs() has this single call site on the hot path (instruction footprint).
+// f4 (G44), auto-reset: a step that ends an episode gives its rewards and done as usual, then the env starts its next
+// episode at once and the step's observation is the one of the fresh state (renew_episode).
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX, int AR, class SM>
 __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const StepPtrs& io, bool first) {
-    const int t = m.hdr()->t;
+    int t = m.hdr()->t;
     // the previous step's bulk stores must have read the staging tile before it is rewritten
     if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    // AR = 1: the kernel variant launched for auto-resetting rollouts.  A template parameter because the renewal code,
+    // compiled into the one kernel, cost the plain rollout 2-8 % while unused (registers: spills at 1024 threads).
+    const bool auto_reset = AR != 0 && io.io.auto_reset != 0;
+    const uint32_t gid = c.env_id_base + (uint32_t)e;
+    if (auto_reset && t >= c.T) {  // finished before this call began: its next episode starts with this step
+        const int ep = m.hdr()->episode + 1;
+        __syncthreads();
+        init_env_state<NPAD, NS>(c, m, tid, gid, ep, false);
+        __syncthreads();
+        t = 0;
+        first = true;
+    }
     float coin_pre = 0.f, labor_pre = 0.f;
     double cf_pre = 0.0;
     int mode = 0, rows = 2;
@@ -1451,8 +1548,11 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
         step_body<NPAD, NS, RT, PT, NT, BT, PF>(c, m, tid, e, io, first, t, coin_pre, labor_pre, cf_pre, rows);
     }
     // ---------------- P5 rewards, P6 observations ----------------
-    outputs<NPAD, NS, RT, NT, BT, PF, FX>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, io.obs(), io.rew(), FX ? io.priv() : nullptr,
-                                          FX ? io.shared() : nullptr, FX ? io.govp() : nullptr);
+    const bool renew = auto_reset && mode == 0 && t + 1 == c.T;  // this step ended the episode: its observation comes from renew_episode
+    outputs<NPAD, NS, RT, NT, BT, PF, FX>(c, m, tid, e, mode, rows, coin_pre, labor_pre, cf_pre, renew ? nullptr : io.obs(), io.rew(),
+                                          (FX && !renew) ? io.priv() : nullptr, (FX && !renew) ? io.shared() : nullptr,
+                                          (FX && !renew) ? io.govp() : nullptr);
+    if (AR != 0 && renew) renew_episode<NPAD, NS, RT, NT, BT, PF, FX>(c, m, tid, e, io);
     EJ_MARK(8);
     if (mode == 1) {
         if (tid == 0 && io.io.done) io.done()[e] = 1;
@@ -1460,7 +1560,7 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
     }
 }
 
-template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX = 0>
+template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX = 0, int AR = 0>
 __global__ void __launch_bounds__(NPAD, (NPAD == 128 ? EJ_CTAS_128 : 1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const __grid_constant__ StepIO io) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
@@ -1505,7 +1605,7 @@ __global__ void __launch_bounds__(NPAD, (NPAD == 128 ? EJ_CTAS_128 : 1024 / NPAD
 #pragma unroll 1
     for (int s = 0; s < io.n_steps; ++s) {
         p.s = s;
-        env_step<NPAD, NS, RT, PT, NT, BT, PF, FX>(c, m, tid, e, p, s == 0);
+        env_step<NPAD, NS, RT, PT, NT, BT, PF, FX, AR>(c, m, tid, e, p, s == 0);
         p.slot = (p.slot + 1 == io.ring_depth) ? 0 : p.slot + 1;
     }
 #ifdef EJ_PHASE_CLOCK
@@ -1547,7 +1647,7 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
-// Reset (G29, G30): one CTA per env builds the blob in shared memory and stores it.
+// Reset (ej_reset): one CTA per env builds the blob of episode 0 in shared memory and stores it.
 template <int NPAD, int NS>
 __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
@@ -1556,45 +1656,7 @@ __global__ void __launch_bounds__(NPAD) ej_reset_kernel(const __grid_constant__ 
     const Sm<NS> m{c};
     for (int i = tid; i < c.blob_bytes / 4; i += NPAD) ((uint32_t*)sblob)[i] = 0u;
     __syncthreads();
-    const uint32_t gid = c.env_id_base + (uint32_t)e;
-    if (tid < c.N) {
-        m.coin()[tid] = c.starting_coin;
-        m.cf()[tid] = coin_utility(c.starting_coin, c.ua, c.inv_ua);
-        uint32_t x[4] = {0, 0, 0, 0};
-        for (int d = 0; d <= c.R; ++d) {  // skill draw d: Philox stream 16, "t" field d/4, word d%4
-            if ((d & 3) == 0) philox4x32_10(gid, (uint32_t)tid, (uint32_t)(d >> 2), 16u, c.seed_lo, c.seed_hi, x[0], x[1], x[2], x[3]);
-            const uint32_t w = (d & 3) == 0 ? x[0] : (d & 3) == 1 ? x[1] : (d & 3) == 2 ? x[2] : x[3];
-            float v = u01(w);
-            if (c.skill_init == EJ_SKILL_NORMAL_CLIP) {
-                // f3 (P:345; G42): z = sum of twelve 24-bit uniforms - 6 (stream 17, "t" fields 3d .. 3d+2); the
-                // sum is an integer, z and std * z are exact in binary64, one rounding to binary32, then the clip
-                long long sum = 0;
-                for (int j = 0; j < 3; ++j) {
-                    uint32_t y0, y1, y2, y3;
-                    philox4x32_10(gid, (uint32_t)tid, (uint32_t)(3 * d + j), 17u, c.seed_lo, c.seed_hi, y0, y1, y2, y3);
-                    sum += (long long)(y0 >> 8) + (long long)(y1 >> 8) + (long long)(y2 >> 8) + (long long)(y3 >> 8);
-                }
-                const double z = __dsub_rn(__dmul_rn((double)sum, 1.0 / 16777216.0), 6.0);
-                v = __double2float_rn(__dadd_rn((double)c.skill_mean, __dmul_rn((double)c.skill_std, z)));
-                if (v < c.clip_lo) v = c.clip_lo;
-                if (v > c.clip_hi) v = c.clip_hi;
-            } else if (c.skill_init == EJ_SKILL_PARETO_CLIP) {  // Pareto(4) by inversion: 1/sqrt(sqrt(1-u))
-                float rr = __fsqrt_rn(__fsub_rn(1.0f, v));
-                rr = __fsqrt_rn(rr);
-                v = __fdiv_rn(1.0f, rr);
-                if (v < c.clip_lo) v = c.clip_lo;
-                if (v > c.clip_hi) v = c.clip_hi;
-            }
-            if (d < c.R) m.SG()[d * NS + tid] = v;
-            else m.SC()[tid] = v;
-        }
-    }
-    for (int l = tid; l < c.n_levels; l += NPAD) { m.head()[l] = (uint16_t)NIL; m.tail()[l] = (uint16_t)NIL; }
-    if (tid == 0) {  // all coins equal: gini = 0, prod = N * coin (exact)
-        const double prod = (double)c.N * (double)c.starting_coin;
-        const double eq = (double)c.omega * (1.0 - 0.0) + (1.0 - (double)c.omega);
-        m.hdr()->u_g_prev = eq * prod;
-    }
+    init_env_state<NPAD, NS>(c, m, tid, c.env_id_base + (uint32_t)e, 0, true);
     __syncthreads();
     uint4* blob = (uint4*)(state + (size_t)e * c.blob_bytes);
     for (int i = tid; i < c.blob_bytes / 16; i += NPAD) blob[i] = ((uint4*)sblob)[i];

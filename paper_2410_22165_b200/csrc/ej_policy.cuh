@@ -52,6 +52,7 @@ struct PolicyArgs {
     int fixed_agent;         // Philox "agent" field when rows_per_env == 1 (government: N), else -1
     const uint8_t* state;    // env state blobs: the clock t is the first int32 of each
     int blob_stride;         // bytes between env blobs
+    int o_episode;           // byte offset of the episode index in a blob (f4: part of the Philox counter)
     uint32_t env_id_base, seed_lo, seed_hi;
     uint32_t stream_base;    // Philox stream of head 0 (population 0, government 1); head h uses word h % 4 of stream + h / 4
     int32_t* actions;        // [rows][n_heads]
@@ -583,7 +584,7 @@ __global__ void __launch_bounds__(P_THREADS, 1) ej_policy_kernel(const __grid_co
     // per-slot state of this group
     uint8_t* const gbase = psm + a.smem_group + grp * (2 * a.slot_bytes);
     int tile[2];
-    int t_env[2] = {0, 0};  // clock of the row's env (Philox counter), fetched while the slot's operand is built
+    int t_env[2] = {0, 0}, ep_env[2] = {0, 0};  // clock and episode of the row's env (Philox counter), fetched while the slot's operand is built
     uint32_t ph_mma[2] = {0u, 0u}, ph_tma[2] = {0u, 0u};
     auto slotA = [&](int sl) { return gbase + sl * a.slot_bytes; };
     auto slotStage = [&](int sl) { return reinterpret_cast<float*>(gbase + sl * a.slot_bytes + a.stage_off); };
@@ -643,7 +644,9 @@ __global__ void __launch_bounds__(P_THREADS, 1) ej_policy_kernel(const __grid_co
             }
             {   // the sampler's Philox counter needs the env's clock: a global load, issued a whole tile ahead of its use
                 const int row = tile[sl] * PTILE + gtid;
-                t_env[sl] = gtid < nrows ? *reinterpret_cast<const int*>(a.state + (size_t)(row / a.rows_per_env) * a.blob_stride) : 0;
+                const uint8_t* blob = a.state + (size_t)(row / a.rows_per_env) * a.blob_stride;
+                t_env[sl] = gtid < nrows ? *reinterpret_cast<const int*>(blob) : 0;
+                ep_env[sl] = gtid < nrows ? *reinterpret_cast<const int*>(blob + a.o_episode) : 0;
             }
             const float* my = stage + gtid * a.row_stride;
             const bool in_tile = gtid < nrows;
@@ -702,12 +705,13 @@ __global__ void __launch_bounds__(P_THREADS, 1) ej_policy_kernel(const __grid_co
             const int env = live ? row / a.rows_per_env : 0;
             const int agent = a.fixed_agent >= 0 ? a.fixed_agent : row - env * a.rows_per_env;
             const int t = t_env[sl];
+            const uint32_t ep_bits = (uint32_t)ep_env[sl] << 8;  // G44
             uint32_t x[4] = {0, 0, 0, 0};
             if (!a.mask.on && n.n_heads == 7 && n.head == 21) {  // the government's 7 brackets x 21 levels
                 float* lrow = (a.logits && live) ? a.logits + (size_t)row * n.n_out : nullptr;
                 auto next_u = [&](int h) {
                     if ((h & 3) == 0)
-                        philox4x32_10(a.env_id_base + (uint32_t)env, (uint32_t)agent, (uint32_t)t, a.stream_base + (uint32_t)(h >> 2), a.seed_lo,
+                        philox4x32_10(a.env_id_base + (uint32_t)env, (uint32_t)agent, (uint32_t)t, (a.stream_base + (uint32_t)(h >> 2)) | ep_bits, a.seed_lo,
                                       a.seed_hi, x[0], x[1], x[2], x[3]);
                     return u01((h & 3) == 0 ? x[0] : (h & 3) == 1 ? x[1] : (h & 3) == 2 ? x[2] : x[3]);
                 };
@@ -715,7 +719,7 @@ __global__ void __launch_bounds__(P_THREADS, 1) ej_policy_kernel(const __grid_co
             } else
             for (int h = 0; h < n.n_heads; ++h) {
                 if ((h & 3) == 0)
-                    philox4x32_10(a.env_id_base + (uint32_t)env, (uint32_t)agent, (uint32_t)t, a.stream_base + (uint32_t)(h >> 2), a.seed_lo,
+                    philox4x32_10(a.env_id_base + (uint32_t)env, (uint32_t)agent, (uint32_t)t, (a.stream_base + (uint32_t)(h >> 2)) | ep_bits, a.seed_lo,
                                   a.seed_hi, x[0], x[1], x[2], x[3]);
                 const uint32_t xw = (h & 3) == 0 ? x[0] : (h & 3) == 1 ? x[1] : (h & 3) == 2 ? x[2] : x[3];
                 const float u = u01(xw);
