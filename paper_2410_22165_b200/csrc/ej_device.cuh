@@ -848,7 +848,9 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
 #pragma unroll 1
     for (int k = BKM + warp; k < 3; k += NW) metric_stats<EPL, NS, NT>(c, m, k, lane, mode, e, rew);
 #pragma unroll 1
-    for (int r = NW - 1 - warp; r < R; r += NW) int_metric_stats<EPL, NS, NT>(c, m, r, lane);
+    // integer metrics: from the last warp down; in bucketed kernels from warp 0 up (their last warp closes the float
+    // metrics after the barrier and has the fewest observation rows to write)
+    for (int r = BKT ? warp : NW - 1 - warp; r < R; r += NW) int_metric_stats<EPL, NS, NT>(c, m, r, lane);
     if (tid < B + 2) m.govrow()[3 * n_metrics + tid] = m.shrow()[5 * R + tid];  // B + 2 <= 18 < NPAD
 
     if (any_obs) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -856,7 +858,8 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
     __syncthreads();
     EJ_MARK(7);
 
-    if (BKT && warp == 0) {  // the three triples and the welfare from the buckets' shares (or the single-warp sort)
+    constexpr int CLOSER = BKT ? NW - 1 : 0;  // warp that closes the statistics and issues the bulk stores
+    if (BKT && warp == CLOSER) {  // the three triples and the welfare from the buckets' shares (or the single-warp sort)
 #pragma unroll 1
         for (int k = 0; k < BKM; ++k) {
             uint32_t* cnt = m.bk_cnt(k);
@@ -893,7 +896,7 @@ __device__ void outputs(const DevCfg& c, const SM& m, int tid, int e, int mode, 
     }
     if (BKT && fell_back) __syncthreads();  // the single-warp sort read the agents' state: nobody may start the next step before it is done
 
-    if (any_obs && tid == 0) {  // bulk stores: the env's contiguous tile, (f2) its env-wide tail, its government row
+    if (any_obs && tid == CLOSER * 32) {  // bulk stores: the env's contiguous tile, (f2) its env-wide tail, its government row
         if (staged) {
             float* dst = FX ? priv + (uint32_t)(e * N * DP) : obs + (uint32_t)(e * N * D_pop);
             const uint32_t src = (uint32_t)__cvta_generic_to_shared(m.stage());
@@ -1520,7 +1523,7 @@ template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX, int 
 __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const StepPtrs& io, bool first) {
     int t = m.hdr()->t;
     // the previous step's bulk stores must have read the staging tile before it is rewritten
-    if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    if (tid == (SM::L::bucketed ? NPAD - 32 : 0)) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");  // the thread that issued them
     // AR = 1: the kernel variant launched for auto-resetting rollouts.  A template parameter because the renewal code,
     // compiled into the one kernel, cost the plain rollout 2-8 % while unused (registers: spills at 1024 threads).
     const bool auto_reset = AR != 0 && io.io.auto_reset != 0;
@@ -1624,6 +1627,8 @@ __global__ void __launch_bounds__(NPAD, (NPAD == 128 ? EJ_CTAS_128 : 1024 / NPAD
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
         asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
     }
+    // bucketed kernels: the observation stores of the last step were issued by the first thread of the last warp
+    if (Lay<NS>::bucketed && tid == NPAD - 32) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
 template <int NPAD, int NS>
@@ -1644,7 +1649,7 @@ __global__ void __launch_bounds__(NPAD) ej_observe_kernel(const __grid_constant_
     if (Lay<NS>::bucketed) bucket_fill_all<NPAD>(m, tid, tid < c.N);
     __syncthreads();
     outputs<NPAD, NS, 0, 0, 0, 0, 0>(c, m, tid, e, 2, 2, 0.f, 0.f, 0.0, obs, nullptr);
-    if (tid == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
+    if (tid == (Lay<NS>::bucketed ? NPAD - 32 : 0)) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");  // the thread that issued the stores
 }
 
 // Reset (ej_reset): one CTA per env builds the blob of episode 0 in shared memory and stores it.
