@@ -275,6 +275,27 @@ int ej_set_policy(ej_env* h, const ej_mlp* pop, const ej_mlp* gov);
 int ej_policy_act(ej_env* h, const float* obs, int32_t* actions_out, int32_t* gov_actions_out, float* pop_logits_out,
                   float* gov_logits_out);
 
+/* A rollout for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): E fresh economies (the state ej_reset(seed) gives) stepped T times with the caller's actions, in ONE call
+ * that needs no handle and calls no cudaMalloc, cudaFree or other allocating routine.  The state blobs the kernels work
+ * on live in a static device array of EJ_NOALLOC_SCRATCH_BYTES (4 MiB: 430 envs at N = 100, R = 2; 267 at R = 6; 34 at N = 1000),
+ * which every GPU that loads the library holds until the process exits; E * device_state_bytes beyond it: EJ_ERR_PARAM
+ * with the limit in ej_last_error(NULL).  Outputs are those of ej_rollout with ring_depth = T on a handle that was
+ * just reset with the same seed:
+ *  actions      device [T][E][N] int32;  gov_actions  device [T][E][B] int32  (both required)
+ *  obs_ring     device [T][obs_floats] float, 16-byte aligned, or NULL
+ *  rew_ring     device [T][E][N+1] float, or NULL;  done_ring  device [T][E] uint8, or NULL
+ *  cuda_stream  cudaStream_t (as void*) the two kernels are enqueued on; the call does not synchronise
+ * Every call shares the one scratch array and leaves its final state in it: calls that overlap on the GPU (different
+ * streams, or graphs replayed concurrently) race; calls on one stream are ordered.  Each call starts by rewriting
+ * every byte of the E blobs it uses, so nothing of an earlier call is read.  The first call on a device looks up
+ * the array's device address (and raises the kernels' shared-memory limit): make it outside a graph capture, e.g.
+ * with T = 0, which only does this set-up.  Errors: EJ_ERR_PARAM (field named), EJ_ERR_CUDA; text in
+ * ej_last_error(NULL). */
+#define EJ_NOALLOC_SCRATCH_BYTES (4u << 20)
+int ej_rollout_noalloc(int32_t E, int32_t N, int32_t R, const ej_params* p, uint64_t seed, int32_t T, const int32_t* actions,
+                       const int32_t* gov_actions, float* obs_ring, float* rew_ring, uint8_t* done_ring, void* cuda_stream);
+
 /* Number of kernels this handle has launched so far (bench.py's gpu_launches). */
 int64_t ej_launch_count(const ej_env* h);
 

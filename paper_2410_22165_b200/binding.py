@@ -74,7 +74,8 @@ class EjMlp(C.Structure):
 
 EXPORTS = ("ej_create", "ej_destroy", "ej_set_stream", "ej_layout", "ej_last_error", "ej_reset", "ej_observe",
            "ej_step", "ej_step_host", "ej_step_host_factored", "ej_rollout", "ej_set_action_cdf", "ej_get_state", "ej_set_state",
-           "ej_launch_count", "ej_set_policy", "ej_policy_act", "ej_action_mask", "ej_set_action_masking")
+           "ej_launch_count", "ej_set_policy", "ej_policy_act", "ej_action_mask", "ej_set_action_masking", "ej_rollout_noalloc")
+NOALLOC_SCRATCH_BYTES = 4 << 20
 
 _lib = None
 
@@ -109,6 +110,7 @@ def lib():
         L.ej_launch_count.argtypes = [vp]; L.ej_launch_count.restype = C.c_int64
         L.ej_set_policy.argtypes = [vp, C.POINTER(EjMlp), C.POINTER(EjMlp)]
         L.ej_policy_act.argtypes = [vp, vp, vp, vp, vp, vp]
+        L.ej_rollout_noalloc.argtypes = [C.c_int32, C.c_int32, C.c_int32, C.POINTER(EjParams), C.c_uint64, C.c_int32, vp, vp, vp, vp, vp, vp]
         for name in EXPORTS:
             if name not in ("ej_last_error", "ej_launch_count"):
                 getattr(L, name).restype = C.c_int
@@ -249,6 +251,12 @@ def make_mlp(net: dict) -> EjMlp:
     m.in_dim, m.hidden, m.out_dim = keep[0].shape[1], keep[0].shape[0], keep[2].shape[0]
     m._keep = keep
     return m
+
+
+def ej_rollout_noalloc(E: int, N: int, R: int, params: EjParams, seed: int, T: int, actions: int | None, gov_actions: int | None,
+                       obs_ring: int | None, rew_ring: int | None, done_ring: int | None, cuda_stream: int | None):
+    _check(None, lib().ej_rollout_noalloc(E, N, R, C.byref(params), C.c_uint64(seed), T, actions, gov_actions, obs_ring, rew_ring,
+                                          done_ring, cuda_stream))
 
 
 def ej_launch_count(h) -> int:

@@ -30,6 +30,12 @@ int align16(int x) { return (x + 15) & ~15; }
 
 }  // namespace
 
+// Scratch of ej_rollout_noalloc: the state blobs the reset and step kernels work on, which every other entry point
+// keeps in memory that ej_create allocates.  File scope, fixed size: every GPU that loads the library holds these
+// EJ_NOALLOC_SCRATCH_BYTES until the process exits.  In HOST code this name is a stand-in, not a device address: the
+// kernels are given the pointer that cudaGetSymbolAddress returns (noalloc_scratch_ptr below).
+static __device__ __align__(256) unsigned char g_noalloc_scratch[EJ_NOALLOC_SCRATCH_BYTES];
+
 struct ej_env {
     DevCfg c;
     ej_params p;
@@ -482,16 +488,10 @@ int rollout_with_policy(ej_env* h, int T, const ej_rollout_io* rio, const StepIO
     return EJ_OK;
 }
 
-}  // namespace
-
-extern "C" {
-
-const char* ej_last_error(const ej_env* h) { return h ? h->err : g_create_err; }
-
-int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out) {
-    g_create_err[0] = 0;
-    if (!out) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "out");
-    *out = nullptr;
+// The two halves of ej_create that need no allocation (shared with ej_rollout_noalloc): validation of the shape and
+// the parameters, and the device configuration of a handle (constants, shared-memory layout, kernel variant).  Errors
+// go to the create-error string (ej_last_error(NULL)).
+int check_shape_and_params(int32_t E, int32_t N, int32_t R, const ej_params* p, int* mp_log2_out) {
     if (!p) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "params");
     if (p->struct_size != sizeof(ej_params)) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "struct_size");
     if (E < 1) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "E");
@@ -521,15 +521,12 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     if (p->skill_growth_rate > 0.0f && !(p->skill_max > 0.0f)) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "skill_max");
     int mp_log2 = 0;
     while ((1 << mp_log2) < p->max_active_orders) ++mp_log2;
+    *mp_log2_out = mp_log2;
     if (((int64_t)N << mp_log2) >= 65535) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "max_active_orders (N * M too large)");
+    return EJ_OK;
+}
 
-    int ndev = 0;
-    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
-        cudaGetLastError();
-        return fail(nullptr, EJ_ERR_CUDA, "%s", "no CUDA device: this library has no CPU fallback");
-    }
-    ej_env* h = new (std::nothrow) ej_env();
-    if (!h) return fail(nullptr, EJ_ERR_NOMEM, "%s", "host allocation failed");
+int configure_handle(ej_env* h, int32_t E, int32_t N, int32_t R, const ej_params* p, int mp_log2) {
     h->p = *p;
     DevCfg& c = h->c;
     memset(&c, 0, sizeof(c));
@@ -570,7 +567,6 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
     c.obs_floats = c.gov_obs_offset + (unsigned long long)E * c.D_gov_pad;
     build_layout(c);
     if (c.smem_bytes > 227 * 1024) {
-        delete h;
         return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "N/R/max_active_orders (state exceeds 227 KB of shared memory)");
     }
     int rc = set_smem_attr(h);
@@ -578,7 +574,38 @@ int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out)
         build_layout(c, false);
         rc = set_smem_attr(h);
     }
-    if (rc != EJ_OK) { memcpy(g_create_err, h->err, 256); delete h; return rc; }
+    if (rc != EJ_OK) { memcpy(g_create_err, h->err, 256); return rc; }
+    return EJ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ej_last_error(const ej_env* h) { return h ? h->err : g_create_err; }
+
+int ej_create(int32_t E, int32_t N, int32_t R, const ej_params* p, ej_env** out) {
+    g_create_err[0] = 0;
+    if (!out) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "out");
+    *out = nullptr;
+    int mp_log2 = 0;
+    {
+        const int vrc = check_shape_and_params(E, N, R, p, &mp_log2);
+        if (vrc != EJ_OK) return vrc;
+    }
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(nullptr, EJ_ERR_CUDA, "%s", "no CUDA device: this library has no CPU fallback");
+    }
+    ej_env* h = new (std::nothrow) ej_env();
+    if (!h) return fail(nullptr, EJ_ERR_NOMEM, "%s", "host allocation failed");
+    {
+        const int crc = configure_handle(h, E, N, R, p, mp_log2);
+        if (crc != EJ_OK) { delete h; return crc; }
+    }
+    DevCfg& c = h->c;
     cudaError_t ce = cudaMalloc(&h->d_state, (size_t)E * c.blob_bytes);
     if (ce == cudaSuccess) ce = cudaMemset(h->d_state, 0, (size_t)E * c.blob_bytes);
     if (ce == cudaSuccess) ce = cudaMalloc(&h->d_cdf, (size_t)c.A * 4);
@@ -1004,6 +1031,79 @@ int ej_set_state(ej_env* h, int32_t env_begin, int32_t env_count, const int32_t*
     EJ_CUDA(h, cudaStreamSynchronize(h->stream), "set_state sync");
     EJ_CUDA(h, cudaMemcpy(h->d_state + (size_t)env_begin * c.blob_bytes, blobs.data(), blobs.size(), cudaMemcpyHostToDevice), "set_state copy");
     return EJ_OK;
+}
+
+// Device address of g_noalloc_scratch on the CURRENT device, looked up once per device (fixed table, no allocation).
+static int noalloc_scratch_ptr(uint8_t** out) {
+    static std::mutex mu;
+    static uint8_t* ptr_of_device[64] = {nullptr};
+    int dev = -1;
+    cudaError_t ce = cudaGetDevice(&dev);
+    if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaGetDevice");
+    if (dev < 0 || dev >= 64) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "current CUDA device (ordinal must be below 64)");
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr_of_device[dev]) {
+        void* ptr = nullptr;
+        ce = cudaGetSymbolAddress(&ptr, g_noalloc_scratch);  // with device `dev` current: the address is per device
+        if (ce != cudaSuccess) return cuda_fail(nullptr, ce, "cudaGetSymbolAddress(g_noalloc_scratch)");
+        if (!ptr) return fail(nullptr, EJ_ERR_CUDA, "%s", "cudaGetSymbolAddress returned a null scratch address");
+        ptr_of_device[dev] = (uint8_t*)ptr;
+    }
+    *out = ptr_of_device[dev];
+    return EJ_OK;
+}
+
+int ej_rollout_noalloc(int32_t E, int32_t N, int32_t R, const ej_params* p, uint64_t seed, int32_t T, const int32_t* actions,
+                       const int32_t* gov_actions, float* obs_ring, float* rew_ring, uint8_t* done_ring, void* cuda_stream) {
+    g_create_err[0] = 0;
+    int mp_log2 = 0;
+    int rc = check_shape_and_params(E, N, R, p, &mp_log2);
+    if (rc != EJ_OK) return rc;
+    if (T < 0) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "T");
+    ej_env h;  // on the stack: no handle, no heap
+    rc = configure_handle(&h, E, N, R, p, mp_log2);
+    if (rc != EJ_OK) return rc;
+    const DevCfg& c = h.c;
+    const unsigned long long need = (unsigned long long)E * (unsigned long long)c.blob_bytes;
+    if (need > (unsigned long long)EJ_NOALLOC_SCRATCH_BYTES) {
+        snprintf(g_create_err, sizeof(g_create_err),
+                 "bad field: E (ej_rollout_noalloc: %d envs x %d state bytes = %llu bytes exceed the static scratch of %llu bytes; at most %llu envs of this shape)",
+                 (int)E, c.blob_bytes, need, (unsigned long long)EJ_NOALLOC_SCRATCH_BYTES,
+                 (unsigned long long)EJ_NOALLOC_SCRATCH_BYTES / (unsigned long long)c.blob_bytes);
+        return EJ_ERR_PARAM;
+    }
+    uint8_t* scratch = nullptr;
+    rc = noalloc_scratch_ptr(&scratch);  // first call on a device: set-up (make it outside a graph capture)
+    if (rc != EJ_OK) return rc;
+    if (T == 0) return EJ_OK;            // set-up only
+    if (!actions) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "actions");
+    if (!gov_actions) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "gov_actions");
+    const unsigned long long lim = 1ull << 32;  // the kernels index rings and action streams with 32-bit element offsets
+    if ((unsigned long long)T * c.obs_floats >= lim) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "T (T * obs_floats must stay below 2^32)");
+    if ((unsigned long long)T * E * N >= lim) return fail(nullptr, EJ_ERR_PARAM, "bad field: %s", "T (T * E * N must stay below 2^32)");
+    h.stream = (cudaStream_t)cuda_stream;
+    h.d_state = scratch;
+    h.c.seed_lo = (uint32_t)(seed & 0xFFFFFFFFull);
+    h.c.seed_hi = (uint32_t)(seed >> 32);
+    // reset: every byte of the E blobs is rewritten (the kernel builds a blob from zero and stores all of it), so
+    // nothing of an earlier call's contents survives into this one
+    rc = for_variant(c.Npad, c.N4, [&](auto mt, auto ns) {
+        constexpr int MT = decltype(mt)::value, NS = decltype(ns)::value;
+        ej_reset_kernel<MT, NS><<<c.E, c.Npad, c.smem_bytes, h.stream>>>(c, h.d_state);
+        EJ_CUDA(&h, cudaGetLastError(), "ej_reset_kernel launch");
+        return EJ_OK;
+    });
+    if (rc == EJ_OK) {
+        StepIO io;
+        memset(&io, 0, sizeof(io));
+        io.n_steps = T; io.ring_depth = T;
+        io.actions = actions; io.gov_actions = gov_actions;
+        io.obs = obs_ring; io.rew = rew_ring; io.done = done_ring;
+        rc = launch_step(&h, io);
+    }
+    if (rc != EJ_OK) memcpy(g_create_err, h.err, 256);
+    h.d_state = nullptr;  // the scratch is not the handle's to free
+    return rc;
 }
 
 }  // extern "C"
