@@ -291,6 +291,35 @@ def main():
         step_ms = e0.elapsed_time(e1) / ks
         run_steps.t += ks + min(3, ks)
 
+    # ---- a12 alone (policy workloads): the tcgen05 policy kernel against the tensor roofline ----
+    policy_kernel = None
+    if use_policy:
+        obs_p = env.observe()
+        a_p = torch.zeros((E, N), dtype=torch.int32, device=dev)
+        g_p = torch.zeros((E, B), dtype=torch.int32, device=dev)
+        for _ in range(5):
+            env.policy_act(obs_p, a_p, g_p)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        reps_p = 50
+        e0.record()
+        for _ in range(reps_p):
+            env.policy_act(obs_p, a_p, g_p)
+        e1.record()
+        torch.cuda.synchronize()
+        p_ms = e0.elapsed_time(e1) / reps_p
+        L = len(cfg["params"]["rate_table"])
+        flop = 2.0 * E * N * (env.D_pop * 128 + 128 * 128 + 128 * env.A) + 2.0 * E * (env.D_gov * 128 + 128 * 128 + 128 * B * L)
+        try:
+            with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+                tpeak, tsrc = float(json.load(f)["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst)"
+        except Exception:
+            tpeak, tsrc = 1590.0, "fallback (B200_PROFILING.md)"
+        policy_kernel = {"kernel": "ej_policy_kernel (ej_policy_act, one launch, same obs every call: inputs L2-resident)", "bound": "tensor",
+                         "us_per_launch": 1e3 * p_ms, "flop_per_launch": flop, "achieved": flop / (p_ms * 1e-3) / 1e12, "peak": tpeak,
+                         "unit": "TFLOP/s", "frac": flop / (p_ms * 1e-3) / 1e12 / tpeak, "peak_source": tsrc}
+        del obs_p, a_p, g_p
+
     # ---- f2: the same rollout with factored observations (private block + env-wide block), reported beside it ----
     fx = None
     if not use_policy and (N * (3 * R + 4)) % 4 == 0 and N * env.D_pop * 4 <= 64 * 1024:
@@ -342,7 +371,7 @@ def main():
 
         # the same through ej_step_host_factored (f2): every observation value once, env-wide columns once per env
         if fx is not None:
-            dpv, dsh = 3 * cfg["R"] + 4, (5 * cfg["R"] + B + 2 + 3) // 4 * 4
+            dpv, dsh = env.D_priv, env.D_shared_pad
             h_priv = torch.zeros((E, N, dpv), dtype=torch.float32).pin_memory()
             h_shared = torch.zeros((E, dsh), dtype=torch.float32).pin_memory()
             h_govr = torch.zeros((E, env.D_gov_pad), dtype=torch.float32).pin_memory()
@@ -395,6 +424,8 @@ def main():
     }
     if fx:
         line["factored_obs"] = fx
+    if policy_kernel:
+        line["policy_kernel"] = policy_kernel
     traffic_path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_path):
         try:
