@@ -241,8 +241,10 @@ def main():
     t_steady = min(2 * int(cfg["params"]["order_expiry"]), max(0, T - 1))
 
     def to_steady_state():
-        if run_steps.t < t_steady or (run_steps.t + K > T and t_steady + K <= T):
-            if run_steps.t > t_steady or run_steps.t + K > T:
+        """Every repetition times the SAME episode window [t_steady, t_steady + K): the cost of a step drifts over an
+        episode (agents get richer, more bids are valid), so windows at different places are not comparable."""
+        if run_steps.t != t_steady:
+            if run_steps.t > t_steady:
                 env.reset(cfg["seed"])
                 run_steps.t = 0
             run_steps(t_steady - run_steps.t)
@@ -406,7 +408,7 @@ def main():
         "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_desc(name, cfg, E), "E_per_gpu": E, "api": "ej_rollout (policy kernels + step kernel per step)" if use_policy else "ej_rollout (persistent kernel)",
                    "episode_steps": windows[mid],
-                   "timing": "median of %d repetitions of K = %d steps, each bracketed by barrier + synchronize, every repetition starting at an episode step >= %d (2 x order expiry: books in steady state)" % (REPS, K, t_steady),
+                   "timing": "median of %d repetitions of K = %d steps, each bracketed by barrier + synchronize, every repetition over the same episode window starting at step %d (2 x order expiry: books in steady state)" % (REPS, K, t_steady),
                    "l2": "outputs go to a ring of %d steps x %.1f MB (> 126 MB L2); action streams %d steps x %.1f MB" % (
                        depth, bytes_env_step * E / 1e6, chunk, 4e-6 * E * (N + B))},
         "env_steps_per_sec": world * E * K / (ms * 1e-3),
