@@ -269,7 +269,14 @@ int launch_step(ej_env* h, const StepIO& io) {
         return fail(h, EJ_ERR_PARAM, "bad field: %s", "observation pointer (must be 16-byte aligned)");
     if (misaligned4(io.actions) || misaligned4(io.gov_actions) || misaligned4(io.rew) || misaligned4(io.actions_out) || misaligned4(io.gov_out))
         return fail(h, EJ_ERR_PARAM, "bad field: %s", "actions / rewards pointer (must be 4-byte aligned)");
-    (io.obs_priv ? h->step_fn_fx : io.auto_reset ? h->step_fn_ar : h->step_fn)<<<c.E, c.Npad, c.smem_bytes, h->stream>>>(c, h->d_state, io);
+    int smem = c.smem_bytes;
+    if (io.obs_priv && h->step_pf) {
+        // f2 on the shape-specialised kernels: the staged tile holds the 3R + 4 private columns only, so the launch asks
+        // for what that tile (or the matched-order lists under it) needs: 10 instead of 9 CTAs fit an SM at the headline shape
+        const int lists = 2 * c.R * c.N4 * 4, tile = align16(c.N * (3 * c.R + 4) * 4);
+        smem = c.o_stage + (lists > tile ? lists : tile);
+    }
+    (io.obs_priv ? h->step_fn_fx : io.auto_reset ? h->step_fn_ar : h->step_fn)<<<c.E, c.Npad, smem, h->stream>>>(c, h->d_state, io);
     h->launches++;
     EJ_CUDA(h, cudaGetLastError(), "ej_step_kernel launch");
     return EJ_OK;

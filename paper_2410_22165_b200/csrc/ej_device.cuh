@@ -30,6 +30,9 @@
 
 #include "../../include/econojax.h"
 
+#ifndef EJ_CTAS_128_FX
+#define EJ_CTAS_128_FX 10  // the shape-specialised factored variants: their small tile lets 10 CTAs fit an SM (47 registers, no spills)
+#endif
 #ifndef EJ_CTAS_128
 #define EJ_CTAS_128 8  // resident 128-thread CTAs per SM the step kernel is compiled for (register budget 64; 9 fit the shared memory at the headline shape but measured no faster)
 #endif
@@ -1564,7 +1567,7 @@ __device__ void env_step(const DevCfg& c, const SM& m, int tid, int e, const Ste
 }
 
 template <int NPAD, int NS, int RT, int PT, int NT, int BT, int PF, int FX = 0, int AR = 0>
-__global__ void __launch_bounds__(NPAD, (NPAD == 128 ? EJ_CTAS_128 : 1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
+__global__ void __launch_bounds__(NPAD, (NPAD == 128 ? ((PF && FX) ? EJ_CTAS_128_FX : EJ_CTAS_128) : 1024 / NPAD < 8 ? 1024 / NPAD : 8)) ej_step_kernel(const __grid_constant__ DevCfg c, uint8_t* __restrict__ state,
                                                        const __grid_constant__ StepIO io) {
     extern __shared__ __align__(16) uint8_t ej_smem[];
     uint8_t* const sblob = ej_smem + Lay<NS>::blob;
