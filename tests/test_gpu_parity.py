@@ -410,7 +410,7 @@ def test_error_paths():
     assert ei.value.code == binding.EJ_ERR_STATE
 
 
-@pytest.mark.parametrize("name", ["config2_paper", "tiny_dense", "config3_resources"])
+@pytest.mark.parametrize("name", ["config2_paper", "tiny_dense", "config3_resources", "config4_population"])
 def test_government_statistics_on_adversarial_states(name):
     """a10 on states the episodes never reach: inventories from 0 to 60,000 (the 64-bit sum path of
     the integer metrics), all-equal and two-valued populations, and jumps between rounds so that the
@@ -448,7 +448,8 @@ def test_government_statistics_on_adversarial_states(name):
         exact(pop.cpu().numpy(), o_pop, "%s round %d (%s) pop obs" % (name, rnd, shape))
         close(gov.cpu().numpy(), o_gov, "%s round %d (%s) gov obs" % (name, rnd, shape))
         acts = np.full((E, N), A - 1, np.int32)  # everyone idles: the step kernel's statistics of the same state
-        pair.step_and_compare(acts, np.zeros((E, pair.g.B), np.int32), "%s round %d (%s) noop step" % (name, rnd, shape))
+        for rep in range(3):                     # (bucketed kernels: fall-back step, then steps on the renewed bounds)
+            pair.step_and_compare(acts, np.zeros((E, pair.g.B), np.int32), "%s round %d (%s) noop step %d" % (name, rnd, shape, rep))
 
 
 # ---------------- properties that hold at any size, checked on EVERY env of the full-size launches ----------------
