@@ -1378,6 +1378,14 @@ __device__ __forceinline__ void step_body(const DevCfg& c, const SM& m, int tid,
     }
     __syncthreads();  // #4 credits complete
     EJ_MARK(4);
+#ifdef EJ_DEBUG_POISON
+    // Debug builds (-DEJ_DEBUG_POISON): everything that is dead from here to the next step's arrivals -- the matched-order
+    // lists (they alias the head of the staging tile), arrival keys, candidate slots, arrival stacks -- is overwritten
+    // with a pattern, so that a stale read of aliased bytes shows up as a parity failure instead of going unnoticed.
+    for (int i = tid; i < 2 * R * N4; i += NPAD) m.mb()[i] = 0xDEADBEEFu;
+    if (tid < N4) { m.key()[tid] = 0xDEADBEEFu; m.cslot()[tid] = 0xDEADBEEFu; m.anext()[tid] = 0xDEADBEEFu; }
+    __syncthreads();
+#endif
 
     // income from sales (G16), coin credit once per agent
     if (act) {
