@@ -182,47 +182,70 @@ __device__ __forceinline__ void tmem_ld32_nowait(uint32_t taddr, uint32_t (&r)[3
 }
 
 // Hidden-layer epilogue: this thread's accumulator row -> +bias -> tanh -> bf16 -> A operand (kp = 128).
-// The special-function unit (16 tanh per clock and SM) bounds this phase and only two or three warps share a
-// scheduler, so a warp must keep the unit fed by itself: the row is handled 32 columns at a time in STAGES -- all
-// bias adds, then 32 tanh back to back, then the packing -- and the accumulators of the next two chunks are already
-// on their way from TMEM (tcgen05.wait::ld waits for every load in flight, hence chunks travel in pairs).  Out of
-// line: compiled on its own, ptxas keeps this order; inlined into the kernel it paired every tanh with its pack.
-__device__ __forceinline__ void epilogue_chunk(const uint32_t (&r)[32], const float* bias, uint8_t* A, int row, int c) {
-    float v[32];
-#pragma unroll
-    for (int g = 0; g < 8; ++g) {
-        const float4 b4 = *reinterpret_cast<const float4*>(bias + c + g * 4);
-        v[4 * g] = __uint_as_float(r[4 * g]) + b4.x;
-        v[4 * g + 1] = __uint_as_float(r[4 * g + 1]) + b4.y;
-        v[4 * g + 2] = __uint_as_float(r[4 * g + 2]) + b4.z;
-        v[4 * g + 3] = __uint_as_float(r[4 * g + 3]) + b4.w;
-    }
-#pragma unroll
-    for (int k = 0; k < 32; ++k) v[k] = tanh_fast(v[k]);
-#pragma unroll
-    for (int g = 0; g < 4; ++g) {
-        uint32_t w[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-            const __nv_bfloat162 h = __floats2bfloat162_rn(v[g * 8 + 2 * j], v[g * 8 + 2 * j + 1]);
-            w[j] = *reinterpret_cast<const uint32_t*>(&h);
-        }
-        *reinterpret_cast<uint4*>(A + op_off(row, c + g * 8, PH)) = make_uint4(w[0], w[1], w[2], w[3]);
-    }
+// Out of line: compiled on its own, ptxas keeps the order written here; inlined into the kernel it paired every
+// tanh with its pack.
+template <int OFF>
+__device__ __forceinline__ void tmem_ld32_into(uint32_t taddr, float (&r)[PH]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];\n"
+        : "=f"(r[OFF + 0]), "=f"(r[OFF + 1]), "=f"(r[OFF + 2]), "=f"(r[OFF + 3]), "=f"(r[OFF + 4]), "=f"(r[OFF + 5]), "=f"(r[OFF + 6]),
+          "=f"(r[OFF + 7]), "=f"(r[OFF + 8]), "=f"(r[OFF + 9]), "=f"(r[OFF + 10]), "=f"(r[OFF + 11]), "=f"(r[OFF + 12]),
+          "=f"(r[OFF + 13]), "=f"(r[OFF + 14]), "=f"(r[OFF + 15]), "=f"(r[OFF + 16]), "=f"(r[OFF + 17]), "=f"(r[OFF + 18]),
+          "=f"(r[OFF + 19]), "=f"(r[OFF + 20]), "=f"(r[OFF + 21]), "=f"(r[OFF + 22]), "=f"(r[OFF + 23]), "=f"(r[OFF + 24]),
+          "=f"(r[OFF + 25]), "=f"(r[OFF + 26]), "=f"(r[OFF + 27]), "=f"(r[OFF + 28]), "=f"(r[OFF + 29]), "=f"(r[OFF + 30]),
+          "=f"(r[OFF + 31])
+        : "r"(taddr)
+        : "memory");
 }
+// volatile forms: the order of these statements in the source is the order ptxas keeps
+__device__ __forceinline__ float tanh_v(float x) { float y; asm volatile("tanh.approx.f32 %0, %1;" : "=f"(y) : "f"(x)); return y; }
+__device__ __forceinline__ float fadd_v(float a, float b) { float y; asm volatile("add.f32 %0, %1, %2;" : "=f"(y) : "f"(a), "f"(b)); return y; }
+__device__ __forceinline__ uint32_t pack_v(float lo, float hi) {  // bf16x2, round to nearest even: lo in bits 0..15
+    uint32_t w;
+    asm volatile("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(w) : "f"(hi), "f"(lo));
+    return w;
+}
+// The row as ONE software pipeline over its 128 columns: in every slot a tanh (special-function unit: one warp
+// instruction per 8 cycles), the bias add of the element 32 columns ahead, and the packing of a pair whose tanh was
+// issued 8 slots (64+ cycles) ago, so that the unit is fed back to back across the whole row while the adds, packs and
+// stores fill its shadow.  Done chunk by chunk (adds, 32 tanh, packs, then the next chunk) the unit idled during every
+// chunk's adds and packs: 4,700 cycles per tile for the two hidden layers against 2 x 1,024 of pure tanh issue.
 __device__ __noinline__ void hidden_epilogue(uint32_t taddr_row, const float* bias, uint8_t* A, int row) {
     asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory");
-    uint32_t r0[32], r1[32], r2[32], r3[32];
-    tmem_ld32_nowait(taddr_row, r0);
-    tmem_ld32_nowait(taddr_row + 32, r1);
+    float x[PH];
+    tmem_ld32_into<0>(taddr_row, x);
+    tmem_ld32_into<32>(taddr_row + 32, x);
     asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
-    tmem_ld32_nowait(taddr_row + 64, r2);
-    tmem_ld32_nowait(taddr_row + 96, r3);
-    epilogue_chunk(r0, bias, A, row, 0);
-    epilogue_chunk(r1, bias, A, row, 32);
-    asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
-    epilogue_chunk(r2, bias, A, row, 64);
-    epilogue_chunk(r3, bias, A, row, 96);
+    tmem_ld32_into<64>(taddr_row + 64, x);
+    tmem_ld32_into<96>(taddr_row + 96, x);
+#pragma unroll
+    for (int g = 0; g < 8; ++g) {  // prologue: bias of the first 32 columns
+        const float4 b4 = *reinterpret_cast<const float4*>(bias + g * 4);
+        x[4 * g] = fadd_v(x[4 * g], b4.x);
+        x[4 * g + 1] = fadd_v(x[4 * g + 1], b4.y);
+        x[4 * g + 2] = fadd_v(x[4 * g + 2], b4.z);
+        x[4 * g + 3] = fadd_v(x[4 * g + 3], b4.w);
+    }
+    uint32_t w[4];
+    float4 b4 = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+    for (int k = 0; k < PH; ++k) {
+        x[k] = tanh_v(x[k]);
+        if (k + 32 < PH) {
+            if (k + 32 == 64) asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");  // columns 64..127 have arrived long ago
+            if ((k & 3) == 0) b4 = *reinterpret_cast<const float4*>(bias + k + 32);
+            x[k + 32] = fadd_v(x[k + 32], (k & 3) == 0 ? b4.x : (k & 3) == 1 ? b4.y : (k & 3) == 2 ? b4.z : b4.w);
+        }
+        const int j = k - 9;  // pair (j, j + 1): the younger tanh was issued 8 slots ago
+        if (j >= 0 && (j & 1) == 0) {
+            w[(j >> 1) & 3] = pack_v(x[j], x[j + 1]);
+            if ((j & 7) == 6) *reinterpret_cast<uint4*>(A + op_off(row, j - 6, PH)) = make_uint4(w[0], w[1], w[2], w[3]);
+        }
+    }
+#pragma unroll
+    for (int j = PH - 8; j < PH; j += 2) w[(j >> 1) & 3] = pack_v(x[j], x[j + 1]);  // the pairs of the last 8 slots
+    *reinterpret_cast<uint4*>(A + op_off(row, PH - 8, PH)) = make_uint4(w[0], w[1], w[2], w[3]);
 }
 
 template <int OFF, int LEN>
